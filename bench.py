@@ -1,0 +1,347 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for BASELINE.json's metric: spin site-updates/ns of the shaken-dynamics hot path.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg4|cfg1|cfg2|cfg3|cfg5] [--impl reference]
+
+A *step* is one full shaken step over the whole workload: half-step 0 (eq. 15) and half-step 1 (eq. 16) of
+every site of every chain, with the observable sums fused in as the workload prescribes.  Default workload:
+BASELINE.json configs[3] ("cfg4": L=16384 int8, J=q=0.7, all +1, seed 3, six sums every step) -- the
+configuration the metric is quoted on.
+
+* ``value``     device-resident throughput: K steps timed with CUDA events on the stream the kernels run on.
+* ``e2e``       the same job through the C ABI with HOST buffers inside the timed region: shaken_set_spins of both
+                layers from pinned host memory, shaken_run(K steps), shaken_observables and shaken_get_spins(sigma)
+                back to the host.  Bytes per step are the totals divided by K.
+* ``roofline``  dominant kernel (the half-step kernel, 2K launches in the timed region): algorithmic bytes per
+                launch (2 B per site-update: read one source byte, write one target byte; 0.25 B bit-packed) over
+                its mean duration, against the measured HBM copy bandwidth of MEASURED_PEAKS.json.
+* ``cpu_baseline``  the oracle (oracle/, as it stands, single thread) timed on this box on a bounded sample.
+* ``--impl reference``  for this tier the reference arm IS the oracle: times it on the host cores, each step a
+                bounded band of rows of the same workload.
+
+N > 1 (torchrun): the workload is replicated as independent chains, rank r simulating global chain r of an
+N-chain batch (chains are independent units -- no data-path collective).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+METRIC = "spin site-updates/ns"
+UNIT = "site-updates/ns"
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--workload", default="cfg4")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--variant", type=int, default=0)
+    return ap.parse_args()
+
+
+def workload(name: str):
+    from paper_1908_07341_b200 import workloads
+
+    idx = {"cfg1": 1, "cfg2": 2, "cfg3": 3, "cfg4": 4, "cfg5": 5}[name]
+    return workloads.config(idx)
+
+
+def measured_peak():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            d = json.load(f)
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+# ----------------------------------------------------------------------------------------- clocks
+class ClockSampler:
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.samples = []
+        self._stop = threading.Event()
+        self._th = None
+
+    def _run(self):
+        while not self._stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.FIELDS}",
+                                      "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5).stdout
+                parts = [x.strip() for x in out.strip().splitlines()[0].split(",")]
+                self.samples.append(parts)
+            except Exception:
+                pass
+            self._stop.wait(0.05)
+
+    def start(self):
+        self._th = threading.Thread(target=self._run, daemon=True)
+        self._th.start()
+
+    def stop(self):
+        self._stop.set()
+        if self._th:
+            self._th.join(timeout=10)
+
+    def summary(self):
+        if not self.samples:
+            return None
+        sm = sorted(float(s[0]) for s in self.samples if s[0].replace(".", "").isdigit())
+        mx = [float(s[1]) for s in self.samples if s[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(len(s) > 3 + i and s[3 + i].lower().startswith("active") for s in self.samples)]
+        pw = [float(s[2]) for s in self.samples if s[2].replace(".", "").isdigit()]
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None, "reasons": reasons,
+                "power_w_max": max(pw) if pw else None, "samples": len(self.samples)}
+
+
+# ----------------------------------------------------------------------------------------- reference arm = oracle
+def oracle_sample_step(w, src, band_rows):
+    """One bounded 'step' of the oracle: both half-steps of `band_rows` rows of chain 0 of the workload."""
+    from oracle import shaken_oracle as so
+
+    a = so.half_step_rows(src, w.seed, 0, w.J[0], w.q[0], 0, 0, 0, band_rows)
+    b = so.half_step_rows(src, w.seed, 0, w.J[0], w.q[0], 0, 1, 0, band_rows)
+    return a, b
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    from oracle import shaken_oracle as so
+
+    so.build()
+    w = workload(args.workload)
+    L = w.L
+    band = max(1, min(L, (8 << 20) // L))                 # ~8 Mi sites per half-step
+    src = np.ones((L, L), dtype=np.int8) if w.init == 1 else np.where(
+        np.random.default_rng(w.seed).integers(0, 2, size=(L, L)) == 1, 1, -1).astype(np.int8)
+    for _ in range(max(args.warmup, 1)):
+        oracle_sample_step(w, src, band)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle_sample_step(w, src, band)
+    dt = time.perf_counter() - t0
+    updates = 2.0 * band * L * args.steps
+    v = updates / (dt * 1e9)
+    sample = f"{band} rows x {L} columns of one chain, both half-steps, per step ({2 * band * L} site updates)"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "int8", "data": "synthetic",
+        "config": {"workload": w.name, "L": L, "n_chains": w.n_chains, "note": "oracle/shaken_oracle.c on host cores, bounded sample per step"},
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+def cpu_baseline(w):
+    """The oracle as it stands, single thread, about 10-30 s of work on the same workload shape."""
+    from oracle import shaken_oracle as so
+
+    so.build()
+    L = w.L
+    band = max(1, min(L, (256 << 20) // L))               # up to 256 Mi sites per half-step
+    src = np.ones((L, L), dtype=np.int8)
+    so.half_step_rows(src, w.seed, 0, w.J[0], w.q[0], 0, 0, 0, min(band, 64))   # warm the code path
+    t0 = time.perf_counter()
+    so.half_step_rows(src, w.seed, 0, w.J[0], w.q[0], 0, 0, 0, band)
+    so.half_step_rows(src, w.seed, 0, w.J[0], w.q[0], 0, 1, 0, band)
+    dt = time.perf_counter() - t0
+    upd = 2.0 * band * L
+    return {"value": upd / (dt * 1e9), "unit": UNIT, "cores": 1, "kind": "oracle",
+            "sample": f"both half-steps of {band} rows x {L} columns of chain 0 ({int(upd)} site updates, {dt:.1f} s)",
+            "host_cores_available": os.cpu_count()}
+
+
+# ----------------------------------------------------------------------------------------- our arm
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    from paper_1908_07341_b200 import build as _build, shaken
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; libshaken has no CPU fallback")
+    if rank == 0:
+        _build.build()
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+        dist.barrier()
+
+    w = workload(args.workload)
+    K, W = args.steps, max(args.warmup, 3)
+    stream = torch.cuda.Stream(device=dev)
+    n_local = w.n_chains                                   # weak scaling: every rank runs the whole named workload
+    s = shaken.Shaken(w.L, n_local, w.seed, packed=w.packed, max_records=(K + W) // max(w.obs_every, 1) + 4,
+                      device=str(dev), stream=stream)
+    s.set_chain_offset(rank * n_local)
+    if args.variant:
+        s.set_variant(args.variant)
+    J, q = w.J_array(), w.q_array()
+    uniform = len(set(w.J)) == 1 and len(set(w.q)) == 1
+
+    def run(n):
+        if uniform:
+            s.run(w.J[0], w.q[0], n, w.obs_every)
+        else:
+            s.run_grid(J, q, n, w.obs_every)
+
+    s.init(w.init)
+    run(W)
+    s.synchronize()
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize(dev)
+
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0 = s.launch_count
+    e0.record(stream)
+    run(K)
+    e1.record(stream)
+    e1.synchronize()
+    torch.cuda.synchronize(dev)
+    ms = e0.elapsed_time(e1)
+    launches = s.launch_count - l0
+    if rank == 0:
+        # keep sampling a little if the region was shorter than a few sampler periods
+        if ms < 300:
+            run(max(1, int(K * 300 / max(ms, 1e-3))))
+            s.synchronize()
+        sampler.stop()
+    if world > 1:
+        t = torch.tensor([ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+        dist.barrier()
+
+    updates_per_rank = 2.0 * n_local * w.L * w.L * K
+    value = world * updates_per_rank / (ms * 1e6)
+
+    # ------------------------------------------------------------------ e2e through the C ABI with host buffers
+    e2e = None
+    if not args.no_e2e:
+        nsp = n_local * w.L * w.L
+        h_sigma = torch.empty(nsp, dtype=torch.int8).pin_memory()
+        h_tau = torch.empty(nsp, dtype=torch.int8).pin_memory()
+        h_out = torch.empty(nsp, dtype=torch.int8).pin_memory()
+        n_rec = K // max(w.obs_every, 1) if w.obs_every else 0
+        h_rec = torch.zeros(max(n_rec, 1) * n_local * 6, dtype=torch.int64).pin_memory()
+        s.get_spins_into(0, h_sigma.data_ptr())
+        s.get_spins_into(1, h_tau.data_ptr())
+        s.clear_records()
+        s.step = 0
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+        t0 = time.perf_counter()
+        s.set_spins_from(0, h_sigma.data_ptr())
+        s.set_spins_from(1, h_tau.data_ptr())
+        run(K)
+        got = s.observables_into(h_rec.data_ptr(), max(n_rec, 1))
+        s.get_spins_into(0, h_out.data_ptr())
+        torch.cuda.synchronize(dev)
+        dt = time.perf_counter() - t0
+        if world > 1:
+            t = torch.tensor([dt], device=dev, dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = float(t.item())
+        e2e = {"value": world * updates_per_rank / (dt * 1e9), "unit": UNIT,
+               "h2d_bytes_per_step": 2 * nsp / K, "d2h_bytes_per_step": (nsp + got * n_local * 48) / K,
+               "ms_total": dt * 1e3,
+               "what": "shaken_set_spins(sigma,tau) from pinned host + shaken_run(K) + shaken_observables + shaken_get_spins(sigma) to host"}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
+    # ------------------------------------------------------------------ roofline of the half-step kernel
+    peak, peak_src = measured_peak()
+    bytes_per_update = 0.25 if w.packed else 2.0
+    n_half_launches = 2 * K
+    alg_bytes_per_launch = bytes_per_update * n_local * w.L * w.L
+    avg_launch_ms = ms / n_half_launches                   # the trailing bond-sum launch (1 of 2K+1) is inside ms
+    achieved = alg_bytes_per_launch / (avg_launch_ms * 1e-3) / 1e9
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tpath):
+        try:
+            traffic = json.load(open(tpath)).get(w.name)
+        except Exception:
+            traffic = None
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": traffic, "peak_source": peak_src, "kernel": "half_step_pk" if w.packed else "half_step_i8",
+                "algorithmic_bytes_per_launch": alg_bytes_per_launch, "avg_launch_us": avg_launch_ms * 1e3}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "u32 bit-packed" if w.packed else "int8", "data": "synthetic",
+        "config": {"workload": w.name, "L": w.L, "n_chains_per_gpu": n_local, "J": w.J[0] if uniform else "grid",
+                   "q": w.q[0] if uniform else "grid", "obs_every": w.obs_every, "init": w.init, "seed": w.seed,
+                   "l2": "inputs larger than L2 (2 x %.0f MB per step)" % (shaken_bytes(w) / 1e6) if shaken_bytes(w) > 126e6
+                         else "working set fits L2 (launch/latency-bound regime)",
+                   "parallelism": "replicas (independent chains, no collective)" if world > 1 else "single GPU"},
+        "clocks": sampler.summary(),
+        "e2e": e2e,
+        "gpu_launches": int(launches),
+        "roofline": roofline,
+    }
+    if not args.no_cpu_baseline and world == 1:
+        line["cpu_baseline"] = cpu_baseline(w)
+    elif world > 1:
+        line["cpu_baseline"] = None
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def shaken_bytes(w):
+    n = w.n_chains * w.L * w.L
+    return n / 8 if w.packed else n
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

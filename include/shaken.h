@@ -1,0 +1,194 @@
+/*
+ * shaken.h -- C ABI of libshaken: the data-parallel half-step of the shaken dynamics
+ * (D'Autilia, Andrianaivo, Troiani, "Parallel simulation of two-dimensional Ising models using
+ * Probabilistic Cellular Automata", arXiv 1908.07341) on NVIDIA B200 (sm_100a).
+ *
+ * What one full step computes (PAPER.md = the paper's text; line numbers refer to it):
+ *   half-step 0 ("odd times", eq. (15); Alg. 2 collectDL :371-377):
+ *       tau'_x  = +1 with probability e^h / (2 cosh h),  h = J (sigma_{x down} + sigma_{x left}) + q sigma_x
+ *   half-step 1 ("even times", eq. (16); Alg. 1 collectUR :354-361):
+ *       sigma'_x = +1 with probability e^h / (2 cosh h),  h = J (tau'_{x up} + tau'_{x right}) + q tau'_x
+ *   for every site x of the L x L torus at once (eq. (3)-(4); local fields eq. (14) :157-160;
+ *   sampling rule "rand() < p" PAPER.md:174, Alg. 3 :413,:433).
+ *
+ * Conventions: x=(i,j) -> column c=i (contiguous), row r=j, site = r*L + c;
+ * up = r+1, right = c+1, down = r-1, left = c-1, all mod L.  rand() is the 32-bit word
+ *     rnd(seed, chain, g, site) = word (site & 3) of Philox4x32-10(key = (seed lo32, seed hi32),
+ *                                  counter = (site >> 2, chain, g lo32, g hi32)),   g = 2 t + half,
+ * t = 0-based global full-step index, and "rand() < p" is the integer compare  rnd < T[2k + c],
+ * k = number of +1 among the two J-neighbours, c = [same-site spin == +1], T = shaken_thresholds().
+ * Consequently spins and the int64 sums below are unique: a CPU oracle must match them bit for bit.
+ *
+ * Memory spaces.  Every pointer argument says HOST or DEVICE.  There are no torch types here; a Python
+ * binding passes tensor.data_ptr() values.  One context is single-threaded; distinct contexts are independent.
+ * No call throws, aborts or prints; every call returns 0 (SHAKEN_OK) or a negative error code, and
+ * shaken_last_error() gives a human-readable message for the most recent failure on that context.
+ * There is no CPU fallback: without a CUDA device every compute call fails with SHAKEN_ECUDA.
+ */
+#ifndef SHAKEN_H
+#define SHAKEN_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct shaken_ctx shaken_ctx;
+
+enum {
+    SHAKEN_OK = 0,
+    SHAKEN_EINVAL = -1, /* bad argument (size, mode, null pointer, non-finite coupling)            */
+    SHAKEN_ENOMEM = -2, /* host or device allocation failed                                        */
+    SHAKEN_ECUDA = -3,  /* CUDA runtime error (no device, launch failure, ...)                      */
+    SHAKEN_ESTATE = -4, /* call not valid in this state (e.g. run before buffers exist)             */
+    SHAKEN_ENOSPC = -5  /* record buffer too small for the records this run would append           */
+};
+
+/* layout flags of shaken_create */
+#define SHAKEN_INT8 0u   /* one int8 (+1 / -1) per spin, [chain][r][c]; requires L % 16 == 0        */
+#define SHAKEN_PACKED 1u /* 32 spins per uint32, bit b of word w of row r = site c = 32 w + b,
+                            bit 1 <-> +1; [chain][r][w]; requires L % 32 == 0                        */
+
+#define SHAKEN_N_OBS 6 /* record = (M_sigma, M_tau, E_J, E_q, C_x, C_y), see shaken_observables */
+
+/* init modes of shaken_init */
+#define SHAKEN_INIT_UP 1
+#define SHAKEN_INIT_DOWN (-1)
+#define SHAKEN_INIT_IID 0
+
+/*
+ * shaken_create: allocate a context for n_chains independent L x L tori (batched-chain layout,
+ * chain-major; the paper runs one (q,J) point per CPU thread).
+ *   out      HOST, receives the context.
+ *   L        16 <= L <= 65536, multiple of 16 (SHAKEN_INT8) or 32 (SHAKEN_PACKED).
+ *   n_chains 1 <= n_chains, n_chains * L * L < 2^40.
+ *   seed     Philox key.
+ * Only host metadata is allocated here.  Device buffers are either borrowed with shaken_bind() or
+ * allocated lazily by the library (cudaMalloc) at the first shaken_init / shaken_set_spins.
+ * Errors: SHAKEN_EINVAL, SHAKEN_ENOMEM.
+ */
+int shaken_create(shaken_ctx **out, int32_t L, int32_t n_chains, uint64_t seed, uint32_t flags);
+
+/* shaken_destroy: frees the context and only the device memory the library itself allocated. */
+int shaken_destroy(shaken_ctx *ctx);
+
+/* Bytes of ONE sublattice buffer (sigma or tau) in device layout: n_chains*L*L (int8) or n_chains*L*L/8. */
+size_t shaken_spin_bytes(const shaken_ctx *ctx);
+
+/* Bytes of one record for all chains: n_chains * 6 * sizeof(int64_t). */
+size_t shaken_record_bytes(const shaken_ctx *ctx);
+
+/*
+ * shaken_bind: borrow device memory and a stream from the caller (PyTorch is used only for this).
+ *   d_sigma, d_tau  DEVICE, each shaken_spin_bytes() bytes, 16-byte aligned; never freed by the library.
+ *   d_records       DEVICE, rec_bytes bytes, 8-byte aligned, capacity floor(rec_bytes / shaken_record_bytes())
+ *                   records; may be NULL with rec_bytes 0 (then the library allocates on demand).
+ *   cuda_stream     a cudaStream_t (NULL = the legacy default stream).  All work of this context is
+ *                   enqueued on it.
+ * The record buffer is zeroed (asynchronously) and the record count reset.  Spins are left untouched.
+ * Errors: SHAKEN_EINVAL (null/misaligned), SHAKEN_ECUDA.
+ */
+int shaken_bind(shaken_ctx *ctx, void *d_sigma, void *d_tau, void *d_records, size_t rec_bytes, void *cuda_stream);
+
+/* Make room for at least max_records records in a library-owned buffer (existing records are kept).
+ * Not allowed on a bound record buffer (SHAKEN_ESTATE). */
+int shaken_reserve_records(shaken_ctx *ctx, int64_t max_records);
+
+/*
+ * shaken_init: set sigma and tau of every chain and reset the step counter and the record count to 0.
+ *   mode  SHAKEN_INIT_UP: all +1;  SHAKEN_INIT_DOWN: all -1 (the paper's scan start; the
+ *         top/bottom chains of :238);  SHAKEN_INIT_IID: iid +-1, spin = +1 iff the init-stream word
+ *         Philox(key = seed, counter = (site>>2, chain, which, 0xFFFFFFFF))[site & 3] < 2^31,
+ *         which = 0 for sigma, 1 for tau.
+ */
+int shaken_init(shaken_ctx *ctx, int mode);
+
+/*
+ * shaken_run: advance every chain by n_steps full steps (2 half-steps each) with couplings J, q
+ * (any finite doubles; eq. (14)).  The global step counter t advances by n_steps.
+ * After every full step whose 1-based global index is a multiple of obs_every (0 = never) one record
+ * is appended (fused into the kernels, int64 atomics).  Work is enqueued on the context's stream and
+ * the call returns without waiting; shaken_observables / shaken_get_spins / shaken_synchronize wait.
+ * Errors: SHAKEN_EINVAL (non-finite J or q, negative counts), SHAKEN_ENOSPC (bound record buffer too
+ * small; nothing is run), SHAKEN_ESTATE (no spins yet), SHAKEN_ECUDA.
+ */
+int shaken_run(shaken_ctx *ctx, double J, double q, int64_t n_steps, int64_t obs_every);
+
+/* Same with one (J, q) per chain: J, q HOST arrays of n_chains doubles, read during the call only. */
+int shaken_run_grid(shaken_ctx *ctx, const double *J, const double *q, int64_t n_steps, int64_t obs_every);
+
+/*
+ * shaken_observables: wait for the stream, then copy min(n_records, max_records) records to
+ *   out  HOST, layout [record][chain][6] int64 =
+ *        M_sigma = sum_x sigma_x, M_tau = sum_x tau_x                      (eq. (17))
+ *        E_J = sum_x sigma_x (tau_{x up} + tau_{x right}), E_q = sum_x sigma_x tau_x
+ *                                               (H(sigma,tau) = -(J E_J + q E_q), eq. (5))
+ *        C_x = sum_x sigma_x sigma_{x right}, C_y = sum_x sigma_x sigma_{x up}
+ *                                               (square-lattice H(sigma) = -J (C_x + C_y))
+ *        all on the pair (sigma', tau') right after half-step 1.
+ * Returns the number of records copied, or a negative error code.
+ */
+int64_t shaken_observables(shaken_ctx *ctx, int64_t *out, int64_t max_records);
+
+/* Number of records currently stored (>= 0) or a negative error code. */
+int64_t shaken_num_records(const shaken_ctx *ctx);
+
+/* Forget all records (the buffer is zeroed on the stream). */
+int shaken_clear_records(shaken_ctx *ctx);
+
+/*
+ * State I/O (parity checks and checkpoint/resume).  which = 0: sigma, 1: tau.
+ *   host  HOST, n_chains*L*L int8 values +1 / -1, layout [chain][r][c] -- also for SHAKEN_PACKED
+ *         (the library converts on the device).  set_spins rejects other values with SHAKEN_EINVAL.
+ * Both calls synchronise the stream.
+ */
+int shaken_get_spins(shaken_ctx *ctx, int which, int8_t *host);
+int shaken_set_spins(shaken_ctx *ctx, int which, const int8_t *host);
+
+/* Global full-step counter t (the random numbers of a step depend on it, so run(a); run(b) == run(a+b)). */
+int shaken_get_step(const shaken_ctx *ctx, uint64_t *step);
+int shaken_set_step(shaken_ctx *ctx, uint64_t step);
+
+/*
+ * shaken_set_chain_offset: chain c of this context draws the random numbers of global chain first_chain + c
+ * (counter word 1).  Lets a batch of chains be sharded over several contexts / GPUs with results identical to
+ * one big batch (independent units, no exchange: SURVEY 8(e)).  Default 0.  first_chain + n_chains <= 2^32.
+ */
+int shaken_set_chain_offset(shaken_ctx *ctx, uint32_t first_chain);
+
+/* Wait until everything enqueued by this context has finished. */
+int shaken_synchronize(shaken_ctx *ctx);
+
+/*
+ * shaken_thresholds: the integer acceptance table for one (J, q), HOST out[6]:
+ *   T[2k + c] = round(2^32 * e^h / (2 cosh h)),  h = J (2k - 2) + q (2c - 1)
+ * evaluated as F(|h|) = clamp(floor(2^32 / (1 + exp(-2|h|)) + 0.5), 2^31, 2^32 - 1) in binary64 and
+ * mirrored for h < 0 (T(h) + T(-h) = 2^32 exactly).  Pure host arithmetic; no device needed.
+ */
+int shaken_thresholds(double J, double q, uint32_t out[6]);
+
+/*
+ * shaken_philox_words: test hook.  Runs the library's DEVICE Philox4x32-10 on n (counter, key) pairs:
+ *   ctr HOST [n][4] uint32, key HOST [n][2] uint32, out HOST [n][4] uint32.
+ */
+int shaken_philox_words(const uint32_t *ctr, const uint32_t *key, uint32_t *out, int64_t n);
+
+/* Number of kernels this context has launched so far (half-steps, init, conversions, reductions). */
+int64_t shaken_launch_count(const shaken_ctx *ctx);
+
+/* Kernel variant: 0 = automatic (default), other values select a specific code path for measurement
+ * (see DESIGN.md "Kernels").  Results never depend on the variant. */
+int shaken_set_variant(shaken_ctx *ctx, int variant);
+
+/* Message for the most recent error on this context ("" if none).  ctx may be NULL (creation errors). */
+const char *shaken_last_error(const shaken_ctx *ctx);
+
+/* Library version string, e.g. "libshaken 0.1 (sm_100a)". */
+const char *shaken_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SHAKEN_H */

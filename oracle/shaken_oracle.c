@@ -205,25 +205,44 @@ void oracle_measure(const int8_t *sigma, const int8_t *tau, int64_t L, int64_t o
     out[0] = Ms; out[1] = Mt; out[2] = EJ; out[3] = Eq; out[4] = Cx; out[5] = Cy;
 }
 
-/* One half-step of one chain.  half = 0: tau <- heat bath on the down/left field of sigma (eq. 15);
- * half = 1: sigma <- heat bath on the up/right field of tau (eq. 16).  src is read, dst written. */
-static void half_step(const oracle_ctx *o, int64_t ch, const uint32_t T[6], int half,
-                      const int8_t *src, int8_t *dst, uint64_t t)
+/* One half-step of one chain, rows r0 .. r0+nrows-1 of the target only (the whole lattice when r0 = 0,
+ * nrows = L).  half = 0: tau <- heat bath on the down/left field of sigma (eq. 15); half = 1: sigma <- heat
+ * bath on the up/right field of tau (eq. 16).  src (L x L) is read; dst_rows points at row r0 of the target. */
+static void half_step_rows(int64_t L, uint64_t seed, int complement, int64_t ch, const uint32_t T[6], int half,
+                           const int8_t *src, int8_t *dst_rows, uint64_t t, int64_t r0, int64_t nrows)
 {
-    int64_t L = o->L;
     int64_t d = half == 0 ? -1 : +1;
     uint64_t g = 2u * t + (uint64_t)half;
-    for (int64_t r = 0; r < L; ++r)
+    for (int64_t r = r0; r < r0 + nrows; ++r)
         for (int64_t c = 0; c < L; ++c) {
             int8_t vert = src[wrap(r + d, L) * L + c];      /* down (half 0) / up (half 1)    */
             int8_t horz = src[r * L + wrap(c + d, L)];      /* left (half 0) / right (half 1) */
             int8_t self = src[r * L + c];
             int k = (vert == 1) + (horz == 1);
             int idx = 2 * k + (self == 1);
-            uint32_t rw = rnd_word(o->seed, (uint32_t)ch, g, (uint64_t)(r * L + c));
-            if (o->complement) rw = ~rw;
-            dst[r * L + c] = rw < T[idx] ? 1 : -1;
+            uint32_t rw = rnd_word(seed, (uint32_t)ch, g, (uint64_t)(r * L + c));
+            if (complement) rw = ~rw;
+            dst_rows[(r - r0) * L + c] = rw < T[idx] ? 1 : -1;
         }
+}
+
+static void half_step(const oracle_ctx *o, int64_t ch, const uint32_t T[6], int half,
+                      const int8_t *src, int8_t *dst, uint64_t t)
+{
+    half_step_rows(o->L, o->seed, o->complement, ch, T, half, src, dst, t, 0, o->L);
+}
+
+/* Context-free form for full-size spot checks: rows r0 .. r0+nrows-1 of one half-step of chain `chain` at
+ * full-step index t, from a caller-supplied source sublattice (L x L, +-1).  Same per-site statement as above. */
+int oracle_half_step_rows(const int8_t *src, int8_t *dst_rows, int64_t L, uint64_t seed, int64_t chain,
+                          double J, double q, uint64_t t, int half, int64_t r0, int64_t nrows)
+{
+    if (!src || !dst_rows || L < 1 || (half != 0 && half != 1) || r0 < 0 || nrows < 0 || r0 + nrows > L)
+        return ORACLE_EINVAL;
+    uint32_t T[6];
+    oracle_thresholds(J, q, T);
+    half_step_rows(L, seed, 0, chain, T, half, src, dst_rows, t, r0, nrows);
+    return ORACLE_OK;
 }
 
 static int push_record(oracle_ctx *o)

@@ -77,6 +77,9 @@ def lib():
         L.oracle_get_step.restype = C.c_uint64
         L.oracle_set_step.argtypes = [p, C.c_uint64]
         L.oracle_set_step.restype = C.c_int
+        L.oracle_half_step_rows.argtypes = [p, p, C.c_int64, C.c_uint64, C.c_int64, C.c_double, C.c_double,
+                                            C.c_uint64, C.c_int, C.c_int64, C.c_int64]
+        L.oracle_half_step_rows.restype = C.c_int
         _lib = L
     return _lib
 
@@ -109,6 +112,21 @@ def measure(sigma: np.ndarray, tau: np.ndarray) -> np.ndarray:
     out = (C.c_int64 * 6)()
     lib().oracle_measure(s.ctypes.data, t.ctypes.data, L, out)
     return np.array(list(out), dtype=np.int64)
+
+
+def half_step_rows(src: np.ndarray, seed: int, chain: int, J: float, q: float, t: int, half: int,
+                   r0: int, nrows: int) -> np.ndarray:
+    """Rows r0 .. r0+nrows-1 of one half-step (0: eq. 15, 1: eq. 16) at full-step index t, computed from the
+    full L x L source sublattice ``src`` (+-1 int8).  For spot checks at sizes where a whole step is too slow."""
+    s = np.ascontiguousarray(src, dtype=np.int8)
+    L = s.shape[-1]
+    assert s.shape == (L, L)
+    out = np.empty((nrows, L), dtype=np.int8)
+    rc = lib().oracle_half_step_rows(s.ctypes.data, out.ctypes.data, L, int(seed) & 0xFFFFFFFFFFFFFFFF, int(chain),
+                                     float(J), float(q), int(t), int(half), int(r0), int(nrows))
+    if rc:
+        raise OracleError(f"oracle_half_step_rows failed: {rc}")
+    return out
 
 
 class OracleError(RuntimeError):

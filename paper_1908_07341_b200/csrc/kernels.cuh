@@ -1,0 +1,491 @@
+// kernels.cuh -- sm_100a kernels of libshaken: the shaken-dynamics half-step (eq. (15)-(16))
+// on int8 and bit-packed spins, with fused observable sums (eq. (17) :196, eq. (5) :81-84).
+//
+// Work decomposition (both layouts).  A *task* is a column strip of one warp: 32 lanes x one vector
+// (int8: 16 spins = one 16-byte load; packed: one 32-spin word) wide, `rows_per_task` rows high, of one chain.
+// A lane walks its strip row by row IN THE DIRECTION OF THE FIELD (half 0 reads down/left, so rows ascend
+// and the previous row in registers is the "down" neighbour; half 1 reads up/right, rows descend), which
+// leaves one halo row per task and, per row, the one spin left (right) of the lane's vector, taken from
+// an extra 4-byte load that hits the line the neighbouring lane just fetched.  The next row is loaded
+// before the current one is computed.  Warps loop over tasks with a grid sized to the machine.
+//
+// Acceptance ("rand() < p"): new spin = +1 iff rnd < T[idx], T looked up in shared memory
+// by a byte offset that is computed for 4 sites at a time with byte-SIMD integer arithmetic.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "philox.cuh"
+
+namespace shaken {
+
+constexpr int WARPS_PER_BLOCK = 8;
+constexpr int BLOCK_THREADS = WARPS_PER_BLOCK * 32;
+constexpr int MAX_ROWS_PER_TASK = 16;   // byte-wide observable counters overflow beyond 31 rows
+
+enum : int { F_OBS = 1, F_BONDS = 2, F_NOUPDATE = 4 };
+
+struct StepParams {
+    const void *src;        // sublattice that is read   (half 0: sigma, half 1: tau)
+    void *dst;              // sublattice that is redrawn (half 0: tau,   half 1: sigma)
+    int L;                  // lattice side
+    int nvec;               // vectors per row: L/16 (int8) or L/32 (packed)
+    int n_chains;
+    uint32_t chain0;        // global index of chain 0 of this context (Philox counter word 1 = chain0 + chain)
+    int rows_per_task;
+    int nseg;               // warp-wide strips per row = ceil(nvec / 32)
+    int nrb;                // row blocks = ceil(L / rows_per_task)
+    long long ntasks;       // n_chains * nrb * nseg
+    const uint32_t *gtab;   // per-chain tables [n_chains][8] in global memory, or nullptr: use utab
+    uint32_t utab[8];       // one table for all chains (kernel parameters live in constant memory)
+    long long *rec_cur;     // [n_chains][6] record of the step being computed (F_OBS) or nullptr
+    long long *rec_prev;    // [n_chains][6] record whose C_x, C_y are still owed (F_BONDS) or nullptr
+    StepKeys keys;
+};
+
+__device__ __forceinline__ uint4 ldg128(const void *p) { return __ldg(reinterpret_cast<const uint4 *>(p)); }
+__device__ __forceinline__ uint32_t ldg32(const void *p) { return __ldg(reinterpret_cast<const uint32_t *>(p)); }
+
+__device__ __forceinline__ int bytes_sum(uint32_t acc) { return (int)__dp4a(acc, 0x01010101u, 0u); }
+
+__device__ __forceinline__ void warp_add_to(long long *addr, int v)
+{
+    int s = __reduce_add_sync(0xFFFFFFFFu, v);
+    if ((threadIdx.x & 31) == 0 && s != 0) atomicAdd(reinterpret_cast<unsigned long long *>(addr), (unsigned long long)(long long)s);
+}
+
+// ===================================================================================================
+// int8 layout.  Spins are bytes 0x01 (+1) / 0xFF (-1); every bit 1..7 of a byte is the "minus" flag m.
+// Table order in shared memory: index i' = m_self + 2 (m_vert + m_horz), tab[i'] = T[5 - i'].
+// ===================================================================================================
+template <int HALF, int FLAGS>
+__global__ void __launch_bounds__(BLOCK_THREADS, 2) half_step_i8(const __grid_constant__ StepParams p)
+{
+    constexpr bool OBS = (FLAGS & F_OBS) != 0;
+    constexpr bool BONDS = (FLAGS & F_BONDS) != 0;
+    constexpr bool UPDATE = (FLAGS & F_NOUPDATE) == 0;
+    static_assert(!(BONDS && HALF == 1), "bond sums ride on half-step 0");
+
+    __shared__ uint32_t s_tab[WARPS_PER_BLOCK][8];
+    const int lane = threadIdx.x & 31;
+    const int warp = threadIdx.x >> 5;
+    uint32_t *tabw = s_tab[warp];
+
+    const int L = p.L;
+    const int L4 = L >> 2;
+    const int R = p.rows_per_task;
+    const size_t plane = (size_t)L * (size_t)L;
+
+    int cur_chain = -1;
+    ChainKeys ck = {0u, 0u};
+    int cnt0 = 0, cnt1 = 0, cnt2 = 0;   // half 1: M_sigma, E_J, E_q ; half 0: M_tau, C_x, C_y
+
+    auto flush = [&](int chain) {
+        if (HALF == 1) {
+            if (OBS) {
+                warp_add_to(p.rec_cur + (size_t)chain * 6 + 0, cnt0);
+                warp_add_to(p.rec_cur + (size_t)chain * 6 + 2, cnt1);
+                warp_add_to(p.rec_cur + (size_t)chain * 6 + 3, cnt2);
+            }
+        } else {
+            if (OBS) warp_add_to(p.rec_cur + (size_t)chain * 6 + 1, cnt0);
+            if (BONDS) {
+                warp_add_to(p.rec_prev + (size_t)chain * 6 + 4, cnt1);
+                warp_add_to(p.rec_prev + (size_t)chain * 6 + 5, cnt2);
+            }
+        }
+        cnt0 = cnt1 = cnt2 = 0;
+    };
+
+    const long long nw = (long long)gridDim.x * WARPS_PER_BLOCK;
+    for (long long task = (long long)blockIdx.x * WARPS_PER_BLOCK + warp; task < p.ntasks; task += nw) {
+        const int seg = (int)(task % p.nseg);
+        const long long t2 = task / p.nseg;
+        const int rb = (int)(t2 % p.nrb);
+        const int chain = (int)(t2 / p.nrb);
+        if (chain != cur_chain) {
+            if ((OBS || BONDS) && cur_chain >= 0) flush(cur_chain);
+            cur_chain = chain;
+            if (UPDATE) {
+                ck = make_chain_keys(p.keys, p.chain0 + (uint32_t)chain);
+                __syncwarp();
+                if (lane < 8) tabw[lane] = p.gtab ? p.gtab[(size_t)chain * 8 + lane] : p.utab[lane];
+                __syncwarp();
+            }
+        }
+        const int cv = seg * 32 + lane;
+        if (cv >= p.nvec) continue;
+
+        const int c0 = cv * 16;
+        const int r_first = rb * R;
+        const int r_last = min(L, r_first + R) - 1;
+        const int rows = r_last - r_first + 1;
+        const uint8_t *sbase = reinterpret_cast<const uint8_t *>(p.src) + (size_t)chain * plane;
+        uint8_t *dbase = reinterpret_cast<uint8_t *>(p.dst) + (size_t)chain * plane;
+
+        const int dir = HALF ? -1 : +1;
+        int r = HALF ? r_last : r_first;
+        const int rh = HALF ? (r_last + 1 == L ? 0 : r_last + 1) : (r_first == 0 ? L - 1 : r_first - 1);
+        const int ce = HALF ? (c0 + 16 == L ? 0 : c0 + 16) : (c0 == 0 ? L - 4 : c0 - 4);
+
+        uint4 vq = ldg128(sbase + (size_t)rh * L + c0);
+        uint4 cq = ldg128(sbase + (size_t)r * L + c0);
+        uint32_t e = ldg32(sbase + (size_t)r * L + ce);
+        uint32_t n = (uint32_t)r * (uint32_t)L4 + (uint32_t)cv * 4u;
+
+        uint32_t acc0 = 0, acc1 = 0, acc2 = 0, acc3 = 0;   // byte-wide partial counts (x2)
+
+        for (int i = 0; i < rows; ++i) {
+            uint4 nq = cq;
+            uint32_t en = e;
+            if (i + 1 < rows) {
+                const int rn = r + dir;
+                nq = ldg128(sbase + (size_t)rn * L + c0);
+                en = ldg32(sbase + (size_t)rn * L + ce);
+            }
+            const uint32_t w[4] = {cq.x, cq.y, cq.z, cq.w};
+            const uint32_t vw[4] = {vq.x, vq.y, vq.z, vq.w};
+            uint32_t ow[4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const uint32_t s = w[j];
+                const uint32_t v = vw[j];
+                uint32_t hh;
+                if (HALF == 0) hh = __funnelshift_l(j == 0 ? e : w[j - 1], s, 8);   // left neighbours
+                else           hh = __funnelshift_r(s, j == 3 ? e : w[j + 1], 8);   // right neighbours
+                uint32_t out = 0;
+                if (UPDATE) {
+                    const uint32_t off = (s & 0x04040404u) + (v & 0x08080808u) + (hh & 0x08080808u);
+                    uint32_t rw[4];
+                    philox_site_words(n + (uint32_t)j, p.keys, ck, rw);
+#pragma unroll
+                    for (int b = 0; b < 4; ++b) {
+                        const uint32_t o = (off >> (8 * b)) & 0xFFu;
+                        const uint32_t T = *reinterpret_cast<const uint32_t *>(reinterpret_cast<const char *>(tabw) + o);
+                        out |= (rw[b] < T ? 0x01u : 0xFFu) << (8 * b);
+                    }
+                    ow[j] = out;
+                }
+                if (HALF == 1) {
+                    if (OBS) {
+                        acc0 += out & 0x02020202u;            // minus count of sigma'
+                        acc1 += (out ^ v) & 0x02020202u;      // sigma'_x tau_{x up}    anti-aligned
+                        acc3 += (out ^ hh) & 0x02020202u;     // sigma'_x tau_{x right} anti-aligned
+                        acc2 += (out ^ s) & 0x02020202u;      // sigma'_x tau_x         anti-aligned
+                    }
+                } else {
+                    if (OBS) acc0 += out & 0x02020202u;       // minus count of tau'
+                    if (BONDS) {
+                        acc1 += (s ^ hh) & 0x02020202u;       // sigma_x sigma_{x left}  anti-aligned
+                        acc2 += (s ^ v) & 0x02020202u;        // sigma_x sigma_{x down}  anti-aligned
+                    }
+                }
+            }
+            if (UPDATE) *reinterpret_cast<uint4 *>(dbase + (size_t)r * L + c0) = make_uint4(ow[0], ow[1], ow[2], ow[3]);
+            vq = cq; cq = nq; e = en;
+            r += dir;
+            n += (uint32_t)(dir * L4);
+        }
+        if (OBS || BONDS) {
+            const int ns = rows * 16;
+            if (HALF == 1) {
+                if (OBS) {
+                    cnt0 += ns - bytes_sum(acc0);
+                    cnt1 += 2 * ns - bytes_sum(acc1) - bytes_sum(acc3);
+                    cnt2 += ns - bytes_sum(acc2);
+                }
+            } else {
+                if (OBS) cnt0 += ns - bytes_sum(acc0);
+                if (BONDS) {
+                    cnt1 += ns - bytes_sum(acc1);
+                    cnt2 += ns - bytes_sum(acc2);
+                }
+            }
+        }
+    }
+    if ((OBS || BONDS) && cur_chain >= 0) flush(cur_chain);
+}
+
+// ===================================================================================================
+// Bit-packed layout: 32 spins per word, bit 1 <-> +1.  A word is spread into eight byte-SIMD registers
+// Y4[k] = 4 * (bits k, 8+k, 16+k, 24+k), so that the left (right) neighbour of site 8m+k is byte m of
+// Y4[k-1] (Y4[k+1]) with no shift; only k = 0 (k = 7) needs a byte funnel shift and the neighbouring word.
+// Table order: natural, index = c + 2 (v + h) = 2k + c.
+// ===================================================================================================
+__device__ __forceinline__ void spread4(uint32_t W, uint32_t Y4[8])
+{
+#pragma unroll
+    for (int k = 0; k < 8; ++k) Y4[k] = (k <= 2 ? (W << (2 - k)) : (W >> (k - 2))) & 0x04040404u;
+}
+
+template <int HALF, int FLAGS>
+__global__ void __launch_bounds__(BLOCK_THREADS, 2) half_step_pk(const __grid_constant__ StepParams p)
+{
+    constexpr bool OBS = (FLAGS & F_OBS) != 0;
+    constexpr bool BONDS = (FLAGS & F_BONDS) != 0;
+    constexpr bool UPDATE = (FLAGS & F_NOUPDATE) == 0;
+    static_assert(!(BONDS && HALF == 1), "bond sums ride on half-step 0");
+
+    __shared__ uint32_t s_tab[WARPS_PER_BLOCK][8];
+    const int lane = threadIdx.x & 31;
+    const int warp = threadIdx.x >> 5;
+    uint32_t *tabw = s_tab[warp];
+
+    const int L = p.L;
+    const int L4 = L >> 2;
+    const int W = p.nvec;                 // words per row
+    const int R = p.rows_per_task;
+    const size_t plane = (size_t)L * (size_t)W;
+
+    int cur_chain = -1;
+    ChainKeys ck = {0u, 0u};
+    int cnt0 = 0, cnt1 = 0, cnt2 = 0;
+
+    auto flush = [&](int chain) {
+        if (HALF == 1) {
+            if (OBS) {
+                warp_add_to(p.rec_cur + (size_t)chain * 6 + 0, cnt0);
+                warp_add_to(p.rec_cur + (size_t)chain * 6 + 2, cnt1);
+                warp_add_to(p.rec_cur + (size_t)chain * 6 + 3, cnt2);
+            }
+        } else {
+            if (OBS) warp_add_to(p.rec_cur + (size_t)chain * 6 + 1, cnt0);
+            if (BONDS) {
+                warp_add_to(p.rec_prev + (size_t)chain * 6 + 4, cnt1);
+                warp_add_to(p.rec_prev + (size_t)chain * 6 + 5, cnt2);
+            }
+        }
+        cnt0 = cnt1 = cnt2 = 0;
+    };
+
+    const long long nw = (long long)gridDim.x * WARPS_PER_BLOCK;
+    for (long long task = (long long)blockIdx.x * WARPS_PER_BLOCK + warp; task < p.ntasks; task += nw) {
+        const int seg = (int)(task % p.nseg);
+        const long long t2 = task / p.nseg;
+        const int rb = (int)(t2 % p.nrb);
+        const int chain = (int)(t2 / p.nrb);
+        if (chain != cur_chain) {
+            if ((OBS || BONDS) && cur_chain >= 0) flush(cur_chain);
+            cur_chain = chain;
+            if (UPDATE) {
+                ck = make_chain_keys(p.keys, p.chain0 + (uint32_t)chain);
+                __syncwarp();
+                if (lane < 8) tabw[lane] = p.gtab ? p.gtab[(size_t)chain * 8 + lane] : p.utab[lane];
+                __syncwarp();
+            }
+        }
+        const int cv = seg * 32 + lane;
+        if (cv >= W) continue;
+
+        const int r_first = rb * R;
+        const int r_last = min(L, r_first + R) - 1;
+        const int rows = r_last - r_first + 1;
+        const uint32_t *sbase = reinterpret_cast<const uint32_t *>(p.src) + (size_t)chain * plane;
+        uint32_t *dbase = reinterpret_cast<uint32_t *>(p.dst) + (size_t)chain * plane;
+
+        const int dir = HALF ? -1 : +1;
+        int r = HALF ? r_last : r_first;
+        const int rh = HALF ? (r_last + 1 == L ? 0 : r_last + 1) : (r_first == 0 ? L - 1 : r_first - 1);
+        const int ce = HALF ? (cv + 1 == W ? 0 : cv + 1) : (cv == 0 ? W - 1 : cv - 1);
+
+        uint32_t V = __ldg(sbase + (size_t)rh * W + cv);
+        uint32_t S = __ldg(sbase + (size_t)r * W + cv);
+        uint32_t e = __ldg(sbase + (size_t)r * W + ce);
+        uint32_t n = (uint32_t)r * (uint32_t)L4 + (uint32_t)cv * 8u;
+
+        uint32_t Yv[8];
+        if (UPDATE) spread4(V, Yv);
+        int a0 = 0, a1 = 0, a2 = 0;     // popcount partials of this task
+
+        for (int i = 0; i < rows; ++i) {
+            uint32_t Sn = S, en = e;
+            if (i + 1 < rows) {
+                const int rn = r + dir;
+                Sn = __ldg(sbase + (size_t)rn * W + cv);
+                en = __ldg(sbase + (size_t)rn * W + ce);
+            }
+            // horizontal neighbour plane: left (half 0) or right (half 1)
+            const uint32_t Hp = HALF == 0 ? ((S << 1) | (e >> 31)) : ((S >> 1) | (e << 31));
+            uint32_t out = 0;
+            if (UPDATE) {
+                uint32_t Y[8];
+                spread4(S, Y);
+                uint32_t off[8];
+#pragma unroll
+                for (int k = 0; k < 8; ++k) {
+                    uint32_t H;
+                    if (HALF == 0) H = k >= 1 ? Y[k - 1] : ((Y[7] << 8) | ((e >> 31) << 2));
+                    else           H = k <= 6 ? Y[k + 1] : ((Y[0] >> 8) | ((e & 1u) << 26));
+                    off[k] = Y[k] + 2u * (Yv[k] + H);
+                }
+#pragma unroll
+                for (int q = 0; q < 8; ++q) {
+                    uint32_t rw[4];
+                    philox_site_words(n + (uint32_t)q, p.keys, ck, rw);
+#pragma unroll
+                    for (int b = 0; b < 4; ++b) {
+                        const int site = 4 * q + b, m = site >> 3, k = site & 7;
+                        const uint32_t o = (off[k] >> (8 * m)) & 0xFFu;
+                        const uint32_t T = *reinterpret_cast<const uint32_t *>(reinterpret_cast<const char *>(tabw) + o);
+                        out |= (rw[b] < T ? 1u : 0u) << site;
+                    }
+                }
+                dbase[(size_t)r * W + cv] = out;
+#pragma unroll
+                for (int k = 0; k < 8; ++k) Yv[k] = Y[k];
+            }
+            if (HALF == 1) {
+                if (OBS) {
+                    a0 += __popc(out);
+                    a1 += __popc(out ^ V) + __popc(out ^ Hp);
+                    a2 += __popc(out ^ S);
+                }
+            } else {
+                if (OBS) a0 += __popc(out);
+                if (BONDS) {
+                    a1 += __popc(S ^ Hp);
+                    a2 += __popc(S ^ V);
+                }
+            }
+            V = S; S = Sn; e = en;
+            r += dir;
+            n += (uint32_t)(dir * L4);
+        }
+        if (OBS || BONDS) {
+            const int ns = rows * 32;
+            if (HALF == 1) {
+                if (OBS) {
+                    cnt0 += 2 * a0 - ns;
+                    cnt1 += 2 * ns - 2 * a1;
+                    cnt2 += ns - 2 * a2;
+                }
+            } else {
+                if (OBS) cnt0 += 2 * a0 - ns;
+                if (BONDS) {
+                    cnt1 += ns - 2 * a1;
+                    cnt2 += ns - 2 * a2;
+                }
+            }
+        }
+    }
+    if ((OBS || BONDS) && cur_chain >= 0) flush(cur_chain);
+}
+
+// ===================================================================================================
+// Initialisation, layout conversion, validation, test hook
+// ===================================================================================================
+
+// iid start: spin = +1 iff init-stream word < 2^31; counter = (site>>2, chain, which, 0xFFFFFFFF).
+// One thread per Philox call (4 sites) per sublattice.  packed: 8 calls per word handled by one thread.
+__global__ void init_iid_i8(uint8_t *sigma, uint8_t *tau, int n_chains, uint32_t chain0, long long calls_per_chain, uint32_t k0, uint32_t k1)
+{
+    const long long total = (long long)n_chains * calls_per_chain;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
+        const uint32_t chain = chain0 + (uint32_t)(i / calls_per_chain);
+        const uint32_t n = (uint32_t)(i % calls_per_chain);
+#pragma unroll
+        for (int which = 0; which < 2; ++which) {
+            uint32_t w[4];
+            philox4x32_10(n, chain, (uint32_t)which, 0xFFFFFFFFu, k0, k1, w);
+            uint32_t out = 0;
+#pragma unroll
+            for (int b = 0; b < 4; ++b) out |= (w[b] < 0x80000000u ? 0x01u : 0xFFu) << (8 * b);
+            reinterpret_cast<uint32_t *>(which ? tau : sigma)[i] = out;
+        }
+    }
+}
+
+__global__ void init_iid_pk(uint32_t *sigma, uint32_t *tau, int n_chains, uint32_t chain0, long long words_per_chain, uint32_t k0, uint32_t k1)
+{
+    const long long total = (long long)n_chains * words_per_chain;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
+        const uint32_t chain = chain0 + (uint32_t)(i / words_per_chain);
+        const uint32_t wd = (uint32_t)(i % words_per_chain);
+#pragma unroll
+        for (int which = 0; which < 2; ++which) {
+            uint32_t out = 0;
+            for (int q = 0; q < 8; ++q) {
+                uint32_t w[4];
+                philox4x32_10(wd * 8u + (uint32_t)q, chain, (uint32_t)which, 0xFFFFFFFFu, k0, k1, w);
+#pragma unroll
+                for (int b = 0; b < 4; ++b) out |= (w[b] < 0x80000000u ? 1u : 0u) << (4 * q + b);
+            }
+            (which ? tau : sigma)[i] = out;
+        }
+    }
+}
+
+// packed words -> +-1 bytes (one thread per word, 32 bytes out)
+__global__ void unpack_words(const uint32_t *pk, uint8_t *bytes, long long n_words)
+{
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n_words; i += (long long)gridDim.x * blockDim.x) {
+        const uint32_t w = pk[i];
+        uint4 o[2];
+        uint32_t *ow = reinterpret_cast<uint32_t *>(o);
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            uint32_t x = 0;
+#pragma unroll
+            for (int b = 0; b < 4; ++b) x |= (((w >> (4 * j + b)) & 1u) ? 0x01u : 0xFFu) << (8 * b);
+            ow[j] = x;
+        }
+        reinterpret_cast<uint4 *>(bytes)[2 * i] = o[0];
+        reinterpret_cast<uint4 *>(bytes)[2 * i + 1] = o[1];
+    }
+}
+
+// +-1 bytes -> packed words; counts bytes that are neither 0x01 nor 0xFF
+__global__ void pack_words(const uint8_t *bytes, uint32_t *pk, long long n_words, unsigned long long *bad)
+{
+    unsigned int nbad = 0;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n_words; i += (long long)gridDim.x * blockDim.x) {
+        const uint4 a = reinterpret_cast<const uint4 *>(bytes)[2 * i];
+        const uint4 b4 = reinterpret_cast<const uint4 *>(bytes)[2 * i + 1];
+        const uint32_t in[8] = {a.x, a.y, a.z, a.w, b4.x, b4.y, b4.z, b4.w};
+        uint32_t w = 0;
+#pragma unroll
+        for (int j = 0; j < 8; ++j)
+#pragma unroll
+            for (int b = 0; b < 4; ++b) {
+                const uint32_t x = (in[j] >> (8 * b)) & 0xFFu;
+                if (x == 0x01u) w |= 1u << (4 * j + b);
+                else if (x != 0xFFu) ++nbad;
+            }
+        pk[i] = w;
+    }
+    if (nbad) atomicAdd(bad, (unsigned long long)nbad);
+}
+
+// counts bytes that are neither 0x01 nor 0xFF (16 bytes per thread-iteration)
+__global__ void validate_bytes(const uint8_t *bytes, long long n_vec, unsigned long long *bad)
+{
+    unsigned int nbad = 0;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n_vec; i += (long long)gridDim.x * blockDim.x) {
+        const uint4 a = reinterpret_cast<const uint4 *>(bytes)[i];
+        const uint32_t in[4] = {a.x, a.y, a.z, a.w};
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            // valid bytes: 0x01 or 0xFF  <=>  bit 0 set and bits 1..7 all equal
+            const uint32_t x = in[j];
+            const uint32_t m = (x >> 1) & 0x01010101u;          // bit 1 of each byte
+            const uint32_t expect = (m * 0xFEu) | 0x01010101u;  // 0xFF where minus, 0x01 where plus
+            const uint32_t d = x ^ expect;
+            if (d) {
+#pragma unroll
+                for (int b = 0; b < 4; ++b) nbad += ((d >> (8 * b)) & 0xFFu) != 0;
+            }
+        }
+    }
+    if (nbad) atomicAdd(bad, (unsigned long long)nbad);
+}
+
+__global__ void philox_hook(const uint32_t *ctr, const uint32_t *key, uint32_t *out, long long n)
+{
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        uint32_t w[4];
+        philox4x32_10(ctr[4 * i], ctr[4 * i + 1], ctr[4 * i + 2], ctr[4 * i + 3], key[2 * i], key[2 * i + 1], w);
+        out[4 * i] = w[0]; out[4 * i + 1] = w[1]; out[4 * i + 2] = w[2]; out[4 * i + 3] = w[3];
+    }
+}
+
+} // namespace shaken

@@ -1,0 +1,596 @@
+// shaken.cu -- host side of libshaken: the C ABI of include/shaken.h.
+//
+// The host does three things: (a1) turns (J, q) into six integer thresholds per chain (PAPER.md:174 heat-bath
+// rule on the integer scale), (a4) drives the step loop -- two kernel launches per full step, eq. (15) then
+// eq. (16) (Alg. 3 :411-433) -- and (a9) moves int64 records and spins across the boundary.
+// Every arithmetic step of the path runs in the kernels of kernels.cuh.  No CPU fallback exists.
+#include "../../include/shaken.h"
+
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <new>
+#include <vector>
+
+#include "kernels.cuh"
+
+using namespace shaken;
+
+struct shaken_ctx {
+    int L = 0;
+    int n_chains = 0;
+    uint64_t seed = 0;
+    uint32_t flags = 0;
+    bool packed = false;
+
+    void *d_sigma = nullptr, *d_tau = nullptr;
+    bool own_spins = false;
+    long long *d_rec = nullptr;
+    int64_t rec_cap = 0;          // in records
+    bool own_rec = false;
+    bool rec_bound = false;
+    int64_t n_rec = 0;
+    uint32_t *d_tab = nullptr;    // [n_chains][8] per-chain tables for shaken_run_grid
+    unsigned long long *d_bad = nullptr;
+    void *d_stage = nullptr;      // staging for packed <-> int8 conversion
+    size_t stage_bytes = 0;
+
+    cudaStream_t stream = nullptr;
+    uint64_t step = 0;
+    uint32_t chain0 = 0;
+    bool have_spins = false;
+    int num_sms = 0;
+    int variant = 0;
+    int64_t launches = 0;
+    char err[512] = {0};
+};
+
+static thread_local char g_err[512] = {0};
+
+static int fail(shaken_ctx *c, int code, const char *fmt, ...)
+{
+    char *dst = c ? c->err : g_err;
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(dst, 512, fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define CU(call)                                                                                          \
+    do {                                                                                                  \
+        cudaError_t e_ = (call);                                                                          \
+        if (e_ != cudaSuccess) return fail(ctx, SHAKEN_ECUDA, "%s: %s", #call, cudaGetErrorString(e_));   \
+    } while (0)
+
+// ---------------------------------------------------------------------------------------------------
+// (a1) thresholds.  P(+|h) = e^h / (2 cosh h) = 1 / (1 + e^{-2h})  (Alg. 3 "exp(h)/2cosh(h)").
+// ---------------------------------------------------------------------------------------------------
+static uint32_t threshold_nonneg(double a)
+{
+    const double p = 1.0 / (1.0 + exp(-2.0 * a));
+    double v = floor(ldexp(p, 32) + 0.5);
+    if (v < 2147483648.0) v = 2147483648.0;
+    if (v > 4294967295.0) v = 4294967295.0;
+    return (uint32_t)v;
+}
+
+static uint32_t threshold_of_field(double h)
+{
+    if (h >= 0.0) return threshold_nonneg(h);
+    return (uint32_t)(4294967296.0 - (double)threshold_nonneg(-h));
+}
+
+extern "C" int shaken_thresholds(double J, double q, uint32_t out[6])
+{
+    if (!out || !isfinite(J) || !isfinite(q)) return fail(nullptr, SHAKEN_EINVAL, "shaken_thresholds: bad argument");
+    for (int k = 0; k < 3; ++k)
+        for (int c = 0; c < 2; ++c) {
+            const double h = (double)(2 * k - 2) * J + (double)(2 * c - 1) * q;   // eq. (14)
+            out[2 * k + c] = threshold_of_field(h);
+        }
+    return SHAKEN_OK;
+}
+
+// table in the order the kernel indexes it (kernels.cuh): int8 uses the minus-count index i' = 5 - idx
+static void kernel_table(double J, double q, bool packed, uint32_t tab[8])
+{
+    uint32_t T[6];
+    shaken_thresholds(J, q, T);
+    for (int i = 0; i < 6; ++i) tab[i] = packed ? T[i] : T[5 - i];
+    tab[6] = tab[7] = 0;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// context
+// ---------------------------------------------------------------------------------------------------
+extern "C" const char *shaken_version(void) { return "libshaken 0.1 (sm_100a)"; }
+
+extern "C" const char *shaken_last_error(const shaken_ctx *ctx) { return ctx ? ctx->err : g_err; }
+
+extern "C" int shaken_create(shaken_ctx **out, int32_t L, int32_t n_chains, uint64_t seed, uint32_t flags)
+{
+    if (!out) return fail(nullptr, SHAKEN_EINVAL, "shaken_create: out is NULL");
+    *out = nullptr;
+    if (flags != SHAKEN_INT8 && flags != SHAKEN_PACKED) return fail(nullptr, SHAKEN_EINVAL, "shaken_create: unknown flags %u", flags);
+    const bool packed = flags == SHAKEN_PACKED;
+    const int mult = packed ? 32 : 16;
+    if (L < 16 || L > 65536 || L % mult != 0)
+        return fail(nullptr, SHAKEN_EINVAL, "shaken_create: L=%d must be a multiple of %d in [16, 65536]", L, mult);
+    if (n_chains < 1 || (double)n_chains * (double)L * (double)L >= 1099511627776.0)
+        return fail(nullptr, SHAKEN_EINVAL, "shaken_create: n_chains=%d out of range", n_chains);
+    shaken_ctx *c = new (std::nothrow) shaken_ctx();
+    if (!c) return fail(nullptr, SHAKEN_ENOMEM, "shaken_create: out of host memory");
+    c->L = L;
+    c->n_chains = n_chains;
+    c->seed = seed;
+    c->flags = flags;
+    c->packed = packed;
+    *out = c;
+    return SHAKEN_OK;
+}
+
+extern "C" int shaken_destroy(shaken_ctx *ctx)
+{
+    if (!ctx) return SHAKEN_OK;
+    if (ctx->have_spins || ctx->d_rec || ctx->d_tab) cudaStreamSynchronize(ctx->stream);
+    if (ctx->own_spins) { cudaFree(ctx->d_sigma); cudaFree(ctx->d_tau); }
+    if (ctx->own_rec) cudaFree(ctx->d_rec);
+    cudaFree(ctx->d_tab);
+    cudaFree(ctx->d_bad);
+    cudaFree(ctx->d_stage);
+    delete ctx;
+    return SHAKEN_OK;
+}
+
+extern "C" size_t shaken_spin_bytes(const shaken_ctx *ctx)
+{
+    if (!ctx) return 0;
+    const size_t n = (size_t)ctx->n_chains * (size_t)ctx->L * (size_t)ctx->L;
+    return ctx->packed ? n / 8 : n;
+}
+
+extern "C" size_t shaken_record_bytes(const shaken_ctx *ctx)
+{
+    return ctx ? (size_t)ctx->n_chains * SHAKEN_N_OBS * sizeof(int64_t) : 0;
+}
+
+static int ensure_device(shaken_ctx *ctx)
+{
+    if (ctx->num_sms) return SHAKEN_OK;
+    int dev = 0;
+    CU(cudaGetDevice(&dev));
+    int sms = 0;
+    CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    ctx->num_sms = sms;
+    CU(cudaMalloc(&ctx->d_bad, sizeof(unsigned long long)));
+    return SHAKEN_OK;
+}
+
+static int ensure_spins(shaken_ctx *ctx)
+{
+    int rc = ensure_device(ctx);
+    if (rc) return rc;
+    if (ctx->d_sigma && ctx->d_tau) return SHAKEN_OK;
+    const size_t nb = shaken_spin_bytes(ctx);
+    void *a = nullptr, *b = nullptr;
+    if (cudaMalloc(&a, nb) != cudaSuccess || cudaMalloc(&b, nb) != cudaSuccess) {
+        cudaFree(a);
+        cudaGetLastError();
+        return fail(ctx, SHAKEN_ENOMEM, "cudaMalloc of 2 x %zu bytes failed", nb);
+    }
+    ctx->d_sigma = a;
+    ctx->d_tau = b;
+    ctx->own_spins = true;
+    // defined content before any init: all +1
+    CU(cudaMemsetAsync(a, ctx->packed ? 0xFF : 0x01, nb, ctx->stream));
+    CU(cudaMemsetAsync(b, ctx->packed ? 0xFF : 0x01, nb, ctx->stream));
+    return SHAKEN_OK;
+}
+
+extern "C" int shaken_bind(shaken_ctx *ctx, void *d_sigma, void *d_tau, void *d_records, size_t rec_bytes, void *cuda_stream)
+{
+    if (!ctx) return fail(nullptr, SHAKEN_EINVAL, "shaken_bind: ctx is NULL");
+    if (!d_sigma || !d_tau || ((uintptr_t)d_sigma & 15) || ((uintptr_t)d_tau & 15) || d_sigma == d_tau)
+        return fail(ctx, SHAKEN_EINVAL, "shaken_bind: sigma/tau must be distinct, non-NULL, 16-byte aligned device pointers");
+    if ((d_records == nullptr) != (rec_bytes == 0) || ((uintptr_t)d_records & 7))
+        return fail(ctx, SHAKEN_EINVAL, "shaken_bind: records pointer / size mismatch or misaligned");
+    int rc = ensure_device(ctx);
+    if (rc) return rc;
+    if (ctx->have_spins || ctx->d_rec) CU(cudaStreamSynchronize(ctx->stream));
+    if (ctx->own_spins) { cudaFree(ctx->d_sigma); cudaFree(ctx->d_tau); ctx->own_spins = false; }
+    if (ctx->own_rec) { cudaFree(ctx->d_rec); ctx->own_rec = false; }
+    ctx->d_sigma = d_sigma;
+    ctx->d_tau = d_tau;
+    ctx->stream = (cudaStream_t)cuda_stream;
+    ctx->d_rec = (long long *)d_records;
+    ctx->rec_cap = d_records ? (int64_t)(rec_bytes / shaken_record_bytes(ctx)) : 0;
+    ctx->rec_bound = d_records != nullptr;
+    ctx->n_rec = 0;
+    ctx->have_spins = true;   // the caller's buffers hold whatever the caller put there
+    if (d_records) CU(cudaMemsetAsync(d_records, 0, (size_t)ctx->rec_cap * shaken_record_bytes(ctx), ctx->stream));
+    return SHAKEN_OK;
+}
+
+static int grow_records(shaken_ctx *ctx, int64_t need)
+{
+    if (need <= ctx->rec_cap) return SHAKEN_OK;
+    if (ctx->rec_bound) return fail(ctx, SHAKEN_ENOSPC, "bound record buffer holds %lld records, %lld needed", (long long)ctx->rec_cap, (long long)need);
+    int rc = ensure_device(ctx);
+    if (rc) return rc;
+    int64_t cap = ctx->rec_cap ? ctx->rec_cap : 64;
+    while (cap < need) cap *= 2;
+    const size_t rb = shaken_record_bytes(ctx);
+    long long *p = nullptr;
+    if (cudaMalloc(&p, (size_t)cap * rb) != cudaSuccess) {
+        cudaGetLastError();
+        return fail(ctx, SHAKEN_ENOMEM, "cudaMalloc of %zu record bytes failed", (size_t)cap * rb);
+    }
+    CU(cudaMemsetAsync(p, 0, (size_t)cap * rb, ctx->stream));
+    if (ctx->d_rec && ctx->n_rec > 0)
+        CU(cudaMemcpyAsync(p, ctx->d_rec, (size_t)ctx->n_rec * rb, cudaMemcpyDeviceToDevice, ctx->stream));
+    if (ctx->d_rec) {
+        CU(cudaStreamSynchronize(ctx->stream));
+        cudaFree(ctx->d_rec);
+    }
+    ctx->d_rec = p;
+    ctx->rec_cap = cap;
+    ctx->own_rec = true;
+    return SHAKEN_OK;
+}
+
+extern "C" int shaken_reserve_records(shaken_ctx *ctx, int64_t max_records)
+{
+    if (!ctx || max_records < 0) return fail(ctx, SHAKEN_EINVAL, "shaken_reserve_records: bad argument");
+    if (ctx->rec_bound) return fail(ctx, SHAKEN_ESTATE, "shaken_reserve_records: record buffer is bound");
+    return grow_records(ctx, max_records);
+}
+
+extern "C" int64_t shaken_num_records(const shaken_ctx *ctx) { return ctx ? ctx->n_rec : SHAKEN_EINVAL; }
+
+extern "C" int shaken_clear_records(shaken_ctx *ctx)
+{
+    if (!ctx) return fail(nullptr, SHAKEN_EINVAL, "shaken_clear_records: ctx is NULL");
+    if (ctx->d_rec && ctx->n_rec > 0)
+        CU(cudaMemsetAsync(ctx->d_rec, 0, (size_t)ctx->n_rec * shaken_record_bytes(ctx), ctx->stream));
+    ctx->n_rec = 0;
+    return SHAKEN_OK;
+}
+
+extern "C" int shaken_get_step(const shaken_ctx *ctx, uint64_t *step)
+{
+    if (!ctx || !step) return SHAKEN_EINVAL;
+    *step = ctx->step;
+    return SHAKEN_OK;
+}
+
+extern "C" int shaken_set_step(shaken_ctx *ctx, uint64_t step)
+{
+    if (!ctx) return SHAKEN_EINVAL;
+    ctx->step = step;
+    return SHAKEN_OK;
+}
+
+extern "C" int shaken_set_chain_offset(shaken_ctx *ctx, uint32_t first_chain)
+{
+    if (!ctx) return fail(nullptr, SHAKEN_EINVAL, "shaken_set_chain_offset: ctx is NULL");
+    if ((uint64_t)first_chain + (uint64_t)ctx->n_chains > 4294967296ull)
+        return fail(ctx, SHAKEN_EINVAL, "shaken_set_chain_offset: first_chain + n_chains exceeds 2^32");
+    ctx->chain0 = first_chain;
+    return SHAKEN_OK;
+}
+
+extern "C" int shaken_synchronize(shaken_ctx *ctx)
+{
+    if (!ctx) return fail(nullptr, SHAKEN_EINVAL, "shaken_synchronize: ctx is NULL");
+    CU(cudaStreamSynchronize(ctx->stream));
+    return SHAKEN_OK;
+}
+
+extern "C" int64_t shaken_launch_count(const shaken_ctx *ctx) { return ctx ? ctx->launches : SHAKEN_EINVAL; }
+
+extern "C" int shaken_set_variant(shaken_ctx *ctx, int variant)
+{
+    if (!ctx || variant < 0) return SHAKEN_EINVAL;
+    ctx->variant = variant;
+    return SHAKEN_OK;
+}
+
+static int grid_for(const shaken_ctx *ctx, long long work_items, int per_thread_items = 1)
+{
+    long long blocks = (work_items + (long long)256 * per_thread_items - 1) / ((long long)256 * per_thread_items);
+    const long long cap = (long long)ctx->num_sms * 16;
+    if (blocks > cap) blocks = cap;
+    if (blocks < 1) blocks = 1;
+    return (int)blocks;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// (a2) init
+// ---------------------------------------------------------------------------------------------------
+extern "C" int shaken_init(shaken_ctx *ctx, int mode)
+{
+    if (!ctx) return fail(nullptr, SHAKEN_EINVAL, "shaken_init: ctx is NULL");
+    if (mode != SHAKEN_INIT_UP && mode != SHAKEN_INIT_DOWN && mode != SHAKEN_INIT_IID)
+        return fail(ctx, SHAKEN_EINVAL, "shaken_init: mode %d is not +1, -1 or 0", mode);
+    int rc = ensure_spins(ctx);
+    if (rc) return rc;
+    const size_t nb = shaken_spin_bytes(ctx);
+    if (mode == SHAKEN_INIT_IID) {
+        const uint32_t k0 = (uint32_t)ctx->seed, k1 = (uint32_t)(ctx->seed >> 32);
+        const long long sites = (long long)ctx->L * ctx->L;
+        if (ctx->packed) {
+            const long long wpc = sites / 32;
+            init_iid_pk<<<grid_for(ctx, wpc * ctx->n_chains), 256, 0, ctx->stream>>>((uint32_t *)ctx->d_sigma, (uint32_t *)ctx->d_tau, ctx->n_chains, ctx->chain0, wpc, k0, k1);
+        } else {
+            const long long cpc = sites / 4;
+            init_iid_i8<<<grid_for(ctx, cpc * ctx->n_chains), 256, 0, ctx->stream>>>((uint8_t *)ctx->d_sigma, (uint8_t *)ctx->d_tau, ctx->n_chains, ctx->chain0, cpc, k0, k1);
+        }
+        ctx->launches++;
+        CU(cudaGetLastError());
+    } else {
+        const int up = mode == SHAKEN_INIT_UP;
+        const int byte = ctx->packed ? (up ? 0xFF : 0x00) : (up ? 0x01 : 0xFF);
+        CU(cudaMemsetAsync(ctx->d_sigma, byte, nb, ctx->stream));
+        CU(cudaMemsetAsync(ctx->d_tau, byte, nb, ctx->stream));
+    }
+    ctx->have_spins = true;
+    ctx->step = 0;
+    return shaken_clear_records(ctx);
+}
+
+// ---------------------------------------------------------------------------------------------------
+// (a3)-(a8) the step loop
+// ---------------------------------------------------------------------------------------------------
+template <int HALF, int FLAGS>
+static cudaError_t launch_half(const shaken_ctx *ctx, const StepParams &p, int grid)
+{
+    if (ctx->packed) half_step_pk<HALF, FLAGS><<<grid, BLOCK_THREADS, 0, ctx->stream>>>(p);
+    else half_step_i8<HALF, FLAGS><<<grid, BLOCK_THREADS, 0, ctx->stream>>>(p);
+    return cudaGetLastError();
+}
+
+static int choose_rows_per_task(const shaken_ctx *ctx, int nseg)
+{
+    // enough tasks to fill the machine a few times over, strips as tall as possible otherwise
+    const long long want = (long long)ctx->num_sms * 2 * WARPS_PER_BLOCK * 4;
+    int R = MAX_ROWS_PER_TASK;
+    while (R > 2 && (long long)ctx->n_chains * nseg * ((ctx->L + R - 1) / R) < want) R >>= 1;
+    return R;
+}
+
+static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool uniform, int64_t n_steps, int64_t obs_every)
+{
+    if (n_steps < 0 || obs_every < 0) return fail(ctx, SHAKEN_EINVAL, "shaken_run: negative count");
+    const int nJ = uniform ? 1 : ctx->n_chains;
+    for (int i = 0; i < nJ; ++i)
+        if (!isfinite(J[i]) || !isfinite(q[i])) return fail(ctx, SHAKEN_EINVAL, "shaken_run: non-finite coupling for chain %d", i);
+    if (!ctx->have_spins || !ctx->d_sigma) return fail(ctx, SHAKEN_ESTATE, "shaken_run: no spins yet (call shaken_init or shaken_set_spins)");
+    int rc = ensure_device(ctx);
+    if (rc) return rc;
+    if (n_steps == 0) return SHAKEN_OK;
+
+    // records this run appends
+    int64_t n_new = 0;
+    if (obs_every > 0) n_new = (int64_t)((ctx->step + (uint64_t)n_steps) / (uint64_t)obs_every - ctx->step / (uint64_t)obs_every);
+    if (n_new > 0) {
+        rc = grow_records(ctx, ctx->n_rec + n_new);
+        if (rc) return rc;
+    }
+
+    StepParams p;
+    memset(&p, 0, sizeof(p));
+    p.L = ctx->L;
+    p.nvec = ctx->packed ? ctx->L / 32 : ctx->L / 16;
+    p.n_chains = ctx->n_chains;
+    p.chain0 = ctx->chain0;
+    p.nseg = (p.nvec + 31) / 32;
+    p.rows_per_task = choose_rows_per_task(ctx, p.nseg);
+    p.nrb = (ctx->L + p.rows_per_task - 1) / p.rows_per_task;
+    p.ntasks = (long long)ctx->n_chains * p.nrb * p.nseg;
+
+    if (uniform) {
+        kernel_table(J[0], q[0], ctx->packed, p.utab);
+        p.gtab = nullptr;
+    } else {
+        if (!ctx->d_tab && cudaMalloc(&ctx->d_tab, (size_t)ctx->n_chains * 8 * sizeof(uint32_t)) != cudaSuccess) {
+            cudaGetLastError();
+            return fail(ctx, SHAKEN_ENOMEM, "cudaMalloc of the threshold tables failed");
+        }
+        std::vector<uint32_t> h((size_t)ctx->n_chains * 8);
+        for (int i = 0; i < ctx->n_chains; ++i) kernel_table(J[i], q[i], ctx->packed, &h[(size_t)i * 8]);
+        // pageable source: the copy is staged before the call returns, so h may go out of scope
+        CU(cudaMemcpyAsync(ctx->d_tab, h.data(), h.size() * sizeof(uint32_t), cudaMemcpyHostToDevice, ctx->stream));
+        CU(cudaStreamSynchronize(ctx->stream));
+        p.gtab = ctx->d_tab;
+    }
+
+    const long long blocks_needed = (p.ntasks + WARPS_PER_BLOCK - 1) / WARPS_PER_BLOCK;
+    const long long cap = (long long)ctx->num_sms * 4;
+    const int grid = (int)(blocks_needed < cap ? blocks_needed : cap);
+    const size_t rec_stride = (size_t)ctx->n_chains * SHAKEN_N_OBS;
+
+    long long *pending = nullptr;   // record that still lacks C_x, C_y
+    for (int64_t s = 0; s < n_steps; ++s) {
+        const uint64_t t = ctx->step;
+        const bool rec = obs_every > 0 && (t + 1) % (uint64_t)obs_every == 0;
+        long long *cur = rec ? ctx->d_rec + (size_t)ctx->n_rec * rec_stride : nullptr;
+        cudaError_t e;
+        // half-step 0: tau <- sigma  (eq. 15)
+        p.src = ctx->d_sigma;
+        p.dst = ctx->d_tau;
+        p.rec_cur = cur;
+        p.rec_prev = pending;
+        make_step_keys(ctx->seed, 2 * t, p.keys);
+        if (rec && pending) e = launch_half<0, F_OBS | F_BONDS>(ctx, p, grid);
+        else if (rec) e = launch_half<0, F_OBS>(ctx, p, grid);
+        else if (pending) e = launch_half<0, F_BONDS>(ctx, p, grid);
+        else e = launch_half<0, 0>(ctx, p, grid);
+        if (e != cudaSuccess) return fail(ctx, SHAKEN_ECUDA, "half-step 0 launch: %s", cudaGetErrorString(e));
+        pending = nullptr;
+        // half-step 1: sigma <- tau  (eq. 16)
+        p.src = ctx->d_tau;
+        p.dst = ctx->d_sigma;
+        p.rec_prev = nullptr;
+        make_step_keys(ctx->seed, 2 * t + 1, p.keys);
+        if (rec) e = launch_half<1, F_OBS>(ctx, p, grid);
+        else e = launch_half<1, 0>(ctx, p, grid);
+        if (e != cudaSuccess) return fail(ctx, SHAKEN_ECUDA, "half-step 1 launch: %s", cudaGetErrorString(e));
+        ctx->launches += 2;
+        ctx->step = t + 1;
+        if (rec) {
+            pending = cur;
+            ctx->n_rec++;
+        }
+    }
+    if (pending) {
+        // the last step was recorded: its sigma-layer bond sums are taken by a read-only pass over sigma
+        p.src = ctx->d_sigma;
+        p.dst = nullptr;
+        p.rec_cur = nullptr;
+        p.rec_prev = pending;
+        cudaError_t e = launch_half<0, F_BONDS | F_NOUPDATE>(ctx, p, grid);
+        if (e != cudaSuccess) return fail(ctx, SHAKEN_ECUDA, "bond-sum launch: %s", cudaGetErrorString(e));
+        ctx->launches++;
+    }
+    return SHAKEN_OK;
+}
+
+extern "C" int shaken_run(shaken_ctx *ctx, double J, double q, int64_t n_steps, int64_t obs_every)
+{
+    if (!ctx) return fail(nullptr, SHAKEN_EINVAL, "shaken_run: ctx is NULL");
+    return run_impl(ctx, &J, &q, true, n_steps, obs_every);
+}
+
+extern "C" int shaken_run_grid(shaken_ctx *ctx, const double *J, const double *q, int64_t n_steps, int64_t obs_every)
+{
+    if (!ctx) return fail(nullptr, SHAKEN_EINVAL, "shaken_run_grid: ctx is NULL");
+    if (!J || !q) return fail(ctx, SHAKEN_EINVAL, "shaken_run_grid: J or q is NULL");
+    return run_impl(ctx, J, q, false, n_steps, obs_every);
+}
+
+// ---------------------------------------------------------------------------------------------------
+// (a9) records and state I/O
+// ---------------------------------------------------------------------------------------------------
+extern "C" int64_t shaken_observables(shaken_ctx *ctx, int64_t *out, int64_t max_records)
+{
+    if (!ctx || max_records < 0) return fail(ctx, SHAKEN_EINVAL, "shaken_observables: bad argument");
+    const int64_t n = ctx->n_rec < max_records ? ctx->n_rec : max_records;
+    if (n > 0) {
+        if (!out) return fail(ctx, SHAKEN_EINVAL, "shaken_observables: out is NULL");
+        cudaError_t e = cudaMemcpyAsync(out, ctx->d_rec, (size_t)n * shaken_record_bytes(ctx), cudaMemcpyDeviceToHost, ctx->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+        if (e != cudaSuccess) return fail(ctx, SHAKEN_ECUDA, "shaken_observables: %s", cudaGetErrorString(e));
+    } else {
+        cudaError_t e = cudaStreamSynchronize(ctx->stream);
+        if (e != cudaSuccess) return fail(ctx, SHAKEN_ECUDA, "shaken_observables: %s", cudaGetErrorString(e));
+    }
+    return n;
+}
+
+static int ensure_stage(shaken_ctx *ctx, size_t bytes)
+{
+    if (ctx->stage_bytes >= bytes) return SHAKEN_OK;
+    cudaFree(ctx->d_stage);
+    ctx->d_stage = nullptr;
+    ctx->stage_bytes = 0;
+    if (cudaMalloc(&ctx->d_stage, bytes) != cudaSuccess) {
+        cudaGetLastError();
+        return fail(ctx, SHAKEN_ENOMEM, "cudaMalloc of %zu staging bytes failed", bytes);
+    }
+    ctx->stage_bytes = bytes;
+    return SHAKEN_OK;
+}
+
+static const size_t STAGE_SITES = (size_t)64 << 20;   // conversion chunk: 64 Mi spins
+
+extern "C" int shaken_get_spins(shaken_ctx *ctx, int which, int8_t *host)
+{
+    if (!ctx || !host || (which != 0 && which != 1)) return fail(ctx, SHAKEN_EINVAL, "shaken_get_spins: bad argument");
+    if (!ctx->have_spins || !ctx->d_sigma) return fail(ctx, SHAKEN_ESTATE, "shaken_get_spins: no spins yet");
+    const size_t n = (size_t)ctx->n_chains * ctx->L * ctx->L;
+    const void *src = which ? ctx->d_tau : ctx->d_sigma;
+    if (!ctx->packed) {
+        CU(cudaMemcpyAsync(host, src, n, cudaMemcpyDeviceToHost, ctx->stream));
+        CU(cudaStreamSynchronize(ctx->stream));
+        return SHAKEN_OK;
+    }
+    const size_t chunk = n < STAGE_SITES ? n : STAGE_SITES;
+    int rc = ensure_stage(ctx, chunk);
+    if (rc) return rc;
+    for (size_t off = 0; off < n; off += chunk) {
+        const size_t m = n - off < chunk ? n - off : chunk;
+        unpack_words<<<grid_for(ctx, (long long)(m / 32)), 256, 0, ctx->stream>>>((const uint32_t *)src + off / 32, (uint8_t *)ctx->d_stage, (long long)(m / 32));
+        ctx->launches++;
+        CU(cudaGetLastError());
+        CU(cudaMemcpyAsync(host + off, ctx->d_stage, m, cudaMemcpyDeviceToHost, ctx->stream));
+        CU(cudaStreamSynchronize(ctx->stream));
+    }
+    return SHAKEN_OK;
+}
+
+extern "C" int shaken_set_spins(shaken_ctx *ctx, int which, const int8_t *host)
+{
+    if (!ctx || !host || (which != 0 && which != 1)) return fail(ctx, SHAKEN_EINVAL, "shaken_set_spins: bad argument");
+    int rc = ensure_spins(ctx);
+    if (rc) return rc;
+    const size_t n = (size_t)ctx->n_chains * ctx->L * ctx->L;
+    void *dst = which ? ctx->d_tau : ctx->d_sigma;
+    CU(cudaMemsetAsync(ctx->d_bad, 0, sizeof(unsigned long long), ctx->stream));
+    if (!ctx->packed) {
+        CU(cudaMemcpyAsync(dst, host, n, cudaMemcpyHostToDevice, ctx->stream));
+        validate_bytes<<<grid_for(ctx, (long long)(n / 16)), 256, 0, ctx->stream>>>((const uint8_t *)dst, (long long)(n / 16), ctx->d_bad);
+        ctx->launches++;
+        CU(cudaGetLastError());
+    } else {
+        const size_t chunk = n < STAGE_SITES ? n : STAGE_SITES;
+        rc = ensure_stage(ctx, chunk);
+        if (rc) return rc;
+        for (size_t off = 0; off < n; off += chunk) {
+            const size_t m = n - off < chunk ? n - off : chunk;
+            CU(cudaMemcpyAsync(ctx->d_stage, host + off, m, cudaMemcpyHostToDevice, ctx->stream));
+            pack_words<<<grid_for(ctx, (long long)(m / 32)), 256, 0, ctx->stream>>>((const uint8_t *)ctx->d_stage, (uint32_t *)dst + off / 32, (long long)(m / 32), ctx->d_bad);
+            ctx->launches++;
+            CU(cudaGetLastError());
+            CU(cudaStreamSynchronize(ctx->stream));   // the staging buffer is reused by the next chunk
+        }
+    }
+    unsigned long long bad = 0;
+    CU(cudaMemcpyAsync(&bad, ctx->d_bad, sizeof(bad), cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    ctx->have_spins = true;
+    if (bad) return fail(ctx, SHAKEN_EINVAL, "shaken_set_spins: %llu values are neither +1 nor -1 (sublattice content is now unspecified)", bad);
+    return SHAKEN_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// test hook
+// ---------------------------------------------------------------------------------------------------
+extern "C" int shaken_philox_words(const uint32_t *ctr, const uint32_t *key, uint32_t *out, int64_t n)
+{
+    shaken_ctx *ctx = nullptr;
+    if (!ctr || !key || !out || n < 0) return fail(nullptr, SHAKEN_EINVAL, "shaken_philox_words: bad argument");
+    if (n == 0) return SHAKEN_OK;
+    uint32_t *dc = nullptr, *dk = nullptr, *dout = nullptr;
+    cudaError_t e = cudaMalloc(&dc, (size_t)n * 16);
+    if (e == cudaSuccess) e = cudaMalloc(&dk, (size_t)n * 8);
+    if (e == cudaSuccess) e = cudaMalloc(&dout, (size_t)n * 16);
+    if (e == cudaSuccess) e = cudaMemcpy(dc, ctr, (size_t)n * 16, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(dk, key, (size_t)n * 8, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) {
+        long long blocks = (n + 255) / 256;
+        if (blocks > 4096) blocks = 4096;
+        philox_hook<<<(int)blocks, 256>>>(dc, dk, dout, (long long)n);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaMemcpy(out, dout, (size_t)n * 16, cudaMemcpyDeviceToHost);
+    cudaFree(dc);
+    cudaFree(dk);
+    cudaFree(dout);
+    if (e != cudaSuccess) return fail(ctx, SHAKEN_ECUDA, "shaken_philox_words: %s", cudaGetErrorString(e));
+    return SHAKEN_OK;
+}

@@ -1,0 +1,288 @@
+"""Thin Python binding of libshaken (include/shaken.h): same names, argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of ``csrc/``; this module loads ``libshaken.so`` with
+ctypes and passes plain pointers and sizes.  PyTorch is used only to own device memory and the stream
+(``Shaken(..., use_torch=True)`` borrows two int8/int32 tensors and an int64 record tensor through
+``shaken_bind``); without torch the library allocates with cudaMalloc itself.
+
+There is no CPU fallback: if the shared library has not been built, importing :func:`lib` raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libshaken.so")
+
+OK, EINVAL, ENOMEM, ECUDA, ESTATE, ENOSPC = 0, -1, -2, -3, -4, -5
+INT8, PACKED = 0, 1
+INIT_UP, INIT_DOWN, INIT_IID = 1, -1, 0
+N_OBS = 6
+OBS_NAMES = ("M_sigma", "M_tau", "E_J", "E_q", "C_x", "C_y")
+
+# every symbol include/shaken.h declares: (name, restype, argtypes)
+_p = C.c_void_p
+SIGNATURES = {
+    "shaken_create": (C.c_int, [C.POINTER(_p), C.c_int32, C.c_int32, C.c_uint64, C.c_uint32]),
+    "shaken_destroy": (C.c_int, [_p]),
+    "shaken_spin_bytes": (C.c_size_t, [_p]),
+    "shaken_record_bytes": (C.c_size_t, [_p]),
+    "shaken_bind": (C.c_int, [_p, _p, _p, _p, C.c_size_t, _p]),
+    "shaken_reserve_records": (C.c_int, [_p, C.c_int64]),
+    "shaken_init": (C.c_int, [_p, C.c_int]),
+    "shaken_run": (C.c_int, [_p, C.c_double, C.c_double, C.c_int64, C.c_int64]),
+    "shaken_run_grid": (C.c_int, [_p, _p, _p, C.c_int64, C.c_int64]),
+    "shaken_observables": (C.c_int64, [_p, _p, C.c_int64]),
+    "shaken_num_records": (C.c_int64, [_p]),
+    "shaken_clear_records": (C.c_int, [_p]),
+    "shaken_get_spins": (C.c_int, [_p, C.c_int, _p]),
+    "shaken_set_spins": (C.c_int, [_p, C.c_int, _p]),
+    "shaken_get_step": (C.c_int, [_p, C.POINTER(C.c_uint64)]),
+    "shaken_set_step": (C.c_int, [_p, C.c_uint64]),
+    "shaken_set_chain_offset": (C.c_int, [_p, C.c_uint32]),
+    "shaken_synchronize": (C.c_int, [_p]),
+    "shaken_thresholds": (C.c_int, [C.c_double, C.c_double, C.POINTER(C.c_uint32)]),
+    "shaken_philox_words": (C.c_int, [_p, _p, _p, C.c_int64]),
+    "shaken_launch_count": (C.c_int64, [_p]),
+    "shaken_set_variant": (C.c_int, [_p, C.c_int]),
+    "shaken_last_error": (C.c_char_p, [_p]),
+    "shaken_version": (C.c_char_p, []),
+}
+
+_lib = None
+
+
+class ShakenError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"libshaken error {code}: {msg}")
+        self.code = code
+
+
+def lib():
+    """Load libshaken.so (built by ``python -m paper_1908_07341_b200.build``).  Fails loudly if absent."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(
+                f"{LIB_PATH} is missing: build it with `python -m paper_1908_07341_b200.build` "
+                "(nvcc, sm_100a).  libshaken has no CPU fallback."
+            )
+        L = C.CDLL(LIB_PATH)
+        for name, (res, args) in SIGNATURES.items():
+            fn = getattr(L, name)
+            fn.restype = res
+            fn.argtypes = args
+        _lib = L
+    return _lib
+
+
+def version() -> str:
+    return lib().shaken_version().decode()
+
+
+def thresholds(J: float, q: float) -> np.ndarray:
+    """Host-side integer acceptance table T[2k+c] (shaken_thresholds)."""
+    t = (C.c_uint32 * 6)()
+    rc = lib().shaken_thresholds(float(J), float(q), t)
+    if rc:
+        raise ShakenError(rc, lib().shaken_last_error(None).decode())
+    return np.array(list(t), dtype=np.uint32)
+
+
+def philox_words(ctr: np.ndarray, key: np.ndarray) -> np.ndarray:
+    """Device Philox4x32-10 of n (counter, key) pairs (test hook)."""
+    c = np.ascontiguousarray(ctr, dtype=np.uint32).reshape(-1, 4)
+    k = np.ascontiguousarray(key, dtype=np.uint32).reshape(-1, 2)
+    assert c.shape[0] == k.shape[0]
+    out = np.empty_like(c)
+    rc = lib().shaken_philox_words(c.ctypes.data, k.ctypes.data, out.ctypes.data, c.shape[0])
+    if rc:
+        raise ShakenError(rc, lib().shaken_last_error(None).decode())
+    return out
+
+
+class Shaken:
+    """One libshaken context: n_chains independent L x L tori."""
+
+    def __init__(self, L: int, n_chains: int = 1, seed: int = 0, packed: bool = False,
+                 use_torch: bool = True, max_records: int = 0, device: str = "cuda:0", stream=None):
+        self.L, self.n_chains, self.seed, self.packed = int(L), int(n_chains), int(seed), bool(packed)
+        self._h = _p()
+        self._lib = lib()
+        rc = self._lib.shaken_create(C.byref(self._h), self.L, self.n_chains, self.seed & (2**64 - 1),
+                                     PACKED if packed else INT8)
+        if rc:
+            self._h = _p()
+            raise ShakenError(rc, self._lib.shaken_last_error(None).decode())
+        self._tensors = None
+        if use_torch:
+            import torch
+
+            if not torch.cuda.is_available():
+                self.close()
+                raise RuntimeError("libshaken needs a CUDA device (there is no CPU fallback)")
+            dev = torch.device(device)
+            nb = int(self._lib.shaken_spin_bytes(self._h))
+            with torch.cuda.device(dev):
+                sigma = torch.empty(nb, dtype=torch.int8, device=dev)
+                tau = torch.empty(nb, dtype=torch.int8, device=dev)
+                rec = torch.zeros(max(int(max_records), 1) * self.n_chains * N_OBS, dtype=torch.int64, device=dev)
+                st = stream if stream is not None else torch.cuda.current_stream(dev)
+                self._tensors = (sigma, tau, rec, st)
+                self._ck(self._lib.shaken_bind(self._h, sigma.data_ptr(), tau.data_ptr(), rec.data_ptr(),
+                                               rec.numel() * 8, st.cuda_stream))
+        elif max_records:
+            self._ck(self._lib.shaken_reserve_records(self._h, int(max_records)))
+
+    # ------------------------------------------------------------------ plumbing
+    def _ck(self, rc):
+        if rc < 0:
+            raise ShakenError(int(rc), self._lib.shaken_last_error(self._h).decode())
+        return rc
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._lib.shaken_destroy(self._h)
+            self._h = _p()
+        self._tensors = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()
+
+    @property
+    def n_sites(self) -> int:
+        return self.L * self.L
+
+    @property
+    def torch_tensors(self):
+        """(sigma, tau, records, stream) borrowed by the library, or None."""
+        return self._tensors
+
+    # ------------------------------------------------------------------ the calls of include/shaken.h
+    def init(self, mode: int):
+        self._ck(self._lib.shaken_init(self._h, int(mode)))
+
+    def run(self, J: float, q: float, n_steps: int, obs_every: int = 0):
+        self._ck(self._lib.shaken_run(self._h, float(J), float(q), int(n_steps), int(obs_every)))
+
+    def run_grid(self, J, q, n_steps: int, obs_every: int = 0):
+        Ja = np.ascontiguousarray(J, dtype=np.float64)
+        qa = np.ascontiguousarray(q, dtype=np.float64)
+        if Ja.shape != (self.n_chains,) or qa.shape != (self.n_chains,):
+            raise ValueError("J and q must have one entry per chain")
+        self._ck(self._lib.shaken_run_grid(self._h, Ja.ctypes.data, qa.ctypes.data, int(n_steps), int(obs_every)))
+
+    def observables(self, max_records: Optional[int] = None, out: Optional[np.ndarray] = None) -> np.ndarray:
+        n = int(self._ck(self._lib.shaken_num_records(self._h)))
+        if max_records is not None:
+            n = min(n, int(max_records))
+        if out is None:
+            out = np.zeros((n, self.n_chains, N_OBS), dtype=np.int64)
+        got = self._ck(self._lib.shaken_observables(self._h, out.ctypes.data, n))
+        return out[:got]
+
+    @property
+    def num_records(self) -> int:
+        return int(self._ck(self._lib.shaken_num_records(self._h)))
+
+    def clear_records(self):
+        self._ck(self._lib.shaken_clear_records(self._h))
+
+    def get_spins(self, which: int, out: Optional[np.ndarray] = None) -> np.ndarray:
+        if out is None:
+            out = np.empty((self.n_chains, self.L, self.L), dtype=np.int8)
+        assert out.dtype == np.int8 and out.size == self.n_chains * self.n_sites and out.flags.c_contiguous
+        self._ck(self._lib.shaken_get_spins(self._h, int(which), out.ctypes.data))
+        return out
+
+    def set_spins(self, which: int, spins: np.ndarray):
+        s = np.ascontiguousarray(spins, dtype=np.int8)
+        if s.size != self.n_chains * self.n_sites:
+            raise ValueError("wrong number of spins")
+        self._ck(self._lib.shaken_set_spins(self._h, int(which), s.ctypes.data))
+
+    def get_spins_into(self, which: int, host_ptr: int):
+        """Raw-pointer form (e.g. a pinned torch tensor's data_ptr())."""
+        self._ck(self._lib.shaken_get_spins(self._h, int(which), host_ptr))
+
+    def set_spins_from(self, which: int, host_ptr: int):
+        self._ck(self._lib.shaken_set_spins(self._h, int(which), host_ptr))
+
+    def observables_into(self, host_ptr: int, max_records: int) -> int:
+        return int(self._ck(self._lib.shaken_observables(self._h, host_ptr, int(max_records))))
+
+    @property
+    def step(self) -> int:
+        v = C.c_uint64()
+        self._ck(self._lib.shaken_get_step(self._h, C.byref(v)))
+        return int(v.value)
+
+    @step.setter
+    def step(self, v: int):
+        self._ck(self._lib.shaken_set_step(self._h, int(v)))
+
+    def set_chain_offset(self, first_chain: int):
+        self._ck(self._lib.shaken_set_chain_offset(self._h, int(first_chain)))
+
+    def synchronize(self):
+        self._ck(self._lib.shaken_synchronize(self._h))
+
+    @property
+    def launch_count(self) -> int:
+        return int(self._lib.shaken_launch_count(self._h))
+
+    def set_variant(self, v: int):
+        self._ck(self._lib.shaken_set_variant(self._h, int(v)))
+
+
+# ---------------------------------------------------------------------- (a9) derived statistics, host side
+def derived_stats(M, n_sites: int) -> dict:
+    """Mean and variance of the magnetisation m = M / n_sites over the recorded window,
+    plus <|m|>, <m^2>, <m^4> and the Binder cumulant U = 1 - <m^4> / (3 <m^2>^2).
+
+    The power sums are exact Python integers (M^4 overflows int64 from L = 512 on, so they are never formed
+    on the device); each quantity is ONE correctly rounded integer division at the end."""
+    vals = [int(v) for v in np.asarray(M).ravel()]
+    n = len(vals)
+    if n == 0:
+        raise ValueError("no records")
+    N = int(n_sites)
+    p1 = pa = p2 = p4 = 0
+    for v in vals:
+        sq = v * v
+        p1 += v
+        pa += -v if v < 0 else v
+        p2 += sq
+        p4 += sq * sq
+    res = {
+        "n": n,
+        "m": p1 / (n * N),
+        "abs_m": pa / (n * N),
+        "m2": p2 / (n * N * N),
+        "m4": p4 / (n * N**4),
+        "var_m": (n * p2 - p1 * p1) / (n * n * N * N),
+    }
+    if p2:
+        num, den = 3 * p2 * p2 - n * p4, 3 * p2 * p2
+        res["binder"] = num / den
+    else:
+        res["binder"] = float("nan")
+    return res
+
+
+def energy(J: float, q: float, E_J: int, E_q: int) -> float:
+    """H(sigma, tau) = -(J E_J + q E_q), eq. (5)."""
+    return -(float(J) * float(int(E_J)) + float(q) * float(int(E_q)))

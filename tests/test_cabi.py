@@ -1,0 +1,94 @@
+"""CPU-only checks of the boundary: the C-ABI library loads, exports every symbol include/shaken.h declares,
+and its host-side logic (argument validation, threshold table, derived statistics) behaves as documented.
+No compute call is made here (there is no GPU in this container)."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+from paper_1908_07341_b200 import shaken, workloads
+from tests import pins
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def declared_symbols():
+    text = open(os.path.join(ROOT, "include", "shaken.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(shaken_[a-z0-9_]+)\s*\(", text)))
+
+
+def test_library_exports_every_declared_symbol():
+    lib = shaken.lib()
+    names = declared_symbols()
+    assert len(names) >= 20
+    for n in names:
+        assert hasattr(lib, n), n
+    # and the binding knows every one of them (same names on both sides)
+    assert set(names) == set(shaken.SIGNATURES)
+    assert "sm_100a" in shaken.version()
+
+
+def test_create_validates_arguments_without_a_device():
+    lib = shaken.lib()
+    h = C.c_void_p()
+    for L, n, flags in [(15, 1, 0), (24, 1, 0), (48, 1, 1), (8, 1, 0), (65552, 1, 0), (64, 0, 0), (64, 1, 7)]:
+        assert lib.shaken_create(C.byref(h), L, n, 1, flags) == shaken.EINVAL, (L, n, flags)
+        assert not h.value
+        assert lib.shaken_last_error(None) != b""
+    assert lib.shaken_create(C.byref(h), 48, 3, 1, 0) == 0
+    assert lib.shaken_spin_bytes(h) == 3 * 48 * 48
+    assert lib.shaken_record_bytes(h) == 3 * 6 * 8
+    assert lib.shaken_num_records(h) == 0
+    step = C.c_uint64(99)
+    assert lib.shaken_get_step(h, C.byref(step)) == 0 and step.value == 0
+    assert lib.shaken_set_step(h, 12345678901234) == 0
+    assert lib.shaken_get_step(h, C.byref(step)) == 0 and step.value == 12345678901234
+    # run before any spins exist: ESTATE, not a crash; bad couplings: EINVAL
+    assert lib.shaken_run(h, 0.5, float("nan"), 1, 0) == shaken.EINVAL
+    assert lib.shaken_run(h, 0.5, 0.5, -1, 0) == shaken.EINVAL
+    assert lib.shaken_run(h, 0.5, 0.5, 1, 0) == shaken.ESTATE
+    assert b"no spins" in lib.shaken_last_error(h)
+    assert lib.shaken_bind(h, None, None, None, 0, None) == shaken.EINVAL
+    assert lib.shaken_destroy(h) == 0
+    assert lib.shaken_create(C.byref(h), 64, 2, 1, 1) == 0
+    assert lib.shaken_spin_bytes(h) == 2 * 64 * 64 // 8
+    assert lib.shaken_destroy(h) == 0
+
+
+COUPLINGS = [(0.5, 0.5), (0.6585, 0.6585), (0.7, 0.7), (0.45, 10.0), (0.44, 0.66), (1.2, 20.0), (0.0, 0.0),
+             (0.0, 1.0), (1.0, 0.0), (-0.3, 0.4), (2.0, 0.03)]
+
+
+def test_library_threshold_table_against_exact_decimal_arithmetic():
+    """The library's own host table (not the oracle's) against 60-digit decimal evaluation of
+    round(2^32 e^h / (2 cosh h)) -- same pin as the oracle's, applied independently."""
+    for J, q in COUPLINGS:
+        T = shaken.thresholds(J, q)
+        ex = pins.exact_table(J, q)
+        for i in range(6):
+            if int(T[i]) != int(ex[i]):
+                frac = float(pins.exact_threshold_real(pins.field(J, q, i // 2, i % 2)) % 1)
+                assert abs(frac - 0.5) < 4e-6 and abs(int(T[i]) - int(ex[i])) == 1
+        assert int(T[0]) + int(T[5]) == 2**32 and int(T[1]) + int(T[4]) == 2**32 and int(T[2]) + int(T[3]) == 2**32
+    J, q = workloads.grid_couplings()
+    for a, b in list(zip(J, q))[::37]:
+        assert np.array_equal(shaken.thresholds(a, b).astype(np.uint64), pins.exact_table(a, b))
+    with pytest.raises(shaken.ShakenError):
+        shaken.thresholds(float("inf"), 0.1)
+
+
+def test_derived_stats_exact_small_case_and_large_values():
+    """(a9) host statistics: hand-computed case, and no overflow where M^4 exceeds int64 (L >= 512)."""
+    st = shaken.derived_stats([2, -2, 4, 0], 4)
+    assert st["m"] == 0.25 and st["abs_m"] == 0.5 and st["m2"] == 24 / (4 * 16) and st["m4"] == (16 + 16 + 256) / (4 * 256)
+    assert st["var_m"] == 24 / 64 - 0.25**2
+    assert abs(st["binder"] - (1 - st["m4"] / (3 * st["m2"] ** 2))) < 1e-15
+    N = 32768 * 32768
+    M = [N, N - 2, -(N - 4)]
+    st = shaken.derived_stats(M, N)
+    assert abs(st["m4"] - 1.0) < 1e-8 and abs(st["abs_m"] - 1.0) < 1e-8
+    assert abs(st["binder"] - 2.0 / 3.0) < 1e-8
+    assert shaken.energy(0.5, 2.0, 10, -3) == -(0.5 * 10 + 2.0 * -3)

@@ -1,0 +1,272 @@
+"""Parity tests proper (``-m gpu``): the CUDA path, called through the C ABI, against the CPU oracle on the same
+seeded inputs -- bit-exact spins and int64 records, derived doubles within 1e-12 relative (BASELINE.json).
+
+Sizes are chosen so the oracle finishes in seconds while the lattice still spans several warp strips, several
+row blocks and a ragged tail (L/16 not a multiple of 32).  Full-size checks are in test_gpu_fullsize.py."""
+import ctypes as C
+import math
+import os
+
+import numpy as np
+import pytest
+
+from oracle import shaken_oracle as so
+from paper_1908_07341_b200 import shaken, workloads
+from tests import conftest
+
+pytestmark = pytest.mark.gpu
+
+REL = 1e-12   # BASELINE.json north_star: derived double-precision quantities agree within 1e-12 relative
+
+
+def assert_same_state(s: shaken.Shaken, o: so.Oracle, what=""):
+    assert s.step == o.step, what
+    assert np.array_equal(s.get_spins(0), o.get_spins(0)), f"sigma differs {what}"
+    assert np.array_equal(s.get_spins(1), o.get_spins(1)), f"tau differs {what}"
+    assert np.array_equal(s.observables(), o.observables()), f"records differ {what}"
+
+
+# ----------------------------------------------------------------------------- RNG
+def test_device_philox_matches_curand_device_function_and_oracle():
+    """Third-party pin on the GPU box: cuRAND's device function curand_Philox4x32_10 (all four counter words and
+    both key words free) against the library's Philox AND the oracle's, 2^20 random (counter, key) pairs plus
+    edge patterns.  This is the pin for counter word 3, which cuRAND's host generator cannot reach."""
+    path = conftest.build_curand_ref()
+    assert path and os.path.exists(path), "tests/libcurandref.so missing (nvcc needed)"
+    ref = C.CDLL(path)
+    ref.curand_ref_philox.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_longlong]
+    ref.curand_ref_philox.restype = C.c_int
+    rng = np.random.default_rng(2024)
+    n = 1 << 20
+    ctr = rng.integers(0, 2**32, size=(n, 4), dtype=np.uint64).astype(np.uint32)
+    key = rng.integers(0, 2**32, size=(n, 2), dtype=np.uint64).astype(np.uint32)
+    edge = np.array([[0, 0, 0, 0], [0xFFFFFFFF] * 4, [1, 0, 0, 0], [0, 0, 0, 1], [0, 0, 5, 0xFFFFFFFF], [7, 2, 0, 0xFFFFFFFF]],
+                    dtype=np.uint32)
+    ctr[: len(edge)] = edge
+    key[:3] = [[0, 0], [0xFFFFFFFF, 0xFFFFFFFF], [1, 0]]
+    want = np.empty_like(ctr)
+    assert ref.curand_ref_philox(ctr.ctypes.data, key.ctypes.data, want.ctypes.data, n) == 0
+    got = shaken.philox_words(ctr, key)
+    assert np.array_equal(got, want)
+    for i in list(range(64)) + list(rng.integers(0, n, size=2000)):
+        assert np.array_equal(so.philox4x32_10(ctr[i], key[i]), want[i]), i
+
+
+def test_threshold_tables_of_library_and_oracle_are_identical():
+    """SURVEY 8(c) point 7: the two sides evaluate exp() with the same libm here, but diff the tables anyway."""
+    J, q = workloads.grid_couplings()
+    for a, b in list(zip(J, q)) + [(0.5, 0.5), (0.6585, 0.6585), (0.7, 0.7), (0.45, 10.0), (0.44, 0.66), (-0.2, 0.3)]:
+        assert np.array_equal(shaken.thresholds(a, b), so.thresholds(a, b)), (a, b)
+
+
+# ----------------------------------------------------------------------------- int8 layout
+@pytest.mark.parametrize("L,n_chains,J,q,init,steps,obs", [
+    (16, 1, 0.5, 0.5, 0, 5, 1),          # smallest lattice: one 16-byte vector per row
+    (48, 2, 0.3, 1.1, 0, 6, 2),          # 3 lanes of a warp active
+    (64, 1, 0.5, 0.5, 0, 50, 1),         # cfg 1 shape
+    (528, 1, 0.6585, 0.6585, 1, 4, 1),   # 33 vectors per row: two strips, ragged tail; all +1 start
+    (1024, 1, 0.44, 0.66, -1, 3, 3),     # the paper's benchmark couplings, all -1 start (:200)
+    (272, 3, 0.45, 10.0, 0, 5, 1),       # saturated thresholds (cfg 5 couplings)
+    (64, 2, 0.0, 0.0, 1, 3, 1),          # J = q = 0: pure coin flips
+    (64, 1, -0.4, 0.7, 0, 4, 1),         # antiferromagnetic J (threshold order reversed)
+])
+def test_int8_runs_match_oracle_bit_for_bit(L, n_chains, J, q, init, steps, obs):
+    seed = 1000 + L
+    o = so.Oracle(L, n_chains, seed)
+    o.init(init)
+    o.run(J, q, steps, obs)
+    with shaken.Shaken(L, n_chains, seed, packed=False, max_records=steps) as s:
+        s.init(init)
+        s.run(J, q, steps, obs)
+        assert_same_state(s, o, f"L={L}")
+
+
+@pytest.mark.parametrize("L,n_chains,J,q,init,steps,obs", [
+    (32, 1, 0.5, 0.5, 0, 5, 1),          # one word per row
+    (96, 2, 0.3, 1.1, 0, 6, 2),          # 3 words per row
+    (1056, 1, 0.45, 10.0, 0, 3, 1),      # 33 words per row: two strips, ragged tail; cfg 5 couplings
+    (256, 3, 0.6585, 0.6585, -1, 5, 1),
+    (64, 1, -0.4, 0.7, 0, 4, 1),
+])
+def test_packed_runs_match_oracle_bit_for_bit(L, n_chains, J, q, init, steps, obs):
+    seed = 2000 + L
+    o = so.Oracle(L, n_chains, seed)
+    o.init(init)
+    o.run(J, q, steps, obs)
+    with shaken.Shaken(L, n_chains, seed, packed=True, max_records=steps) as s:
+        s.init(init)
+        s.run(J, q, steps, obs)
+        assert_same_state(s, o, f"packed L={L}")
+
+
+def test_int8_and_packed_layouts_give_identical_spins_and_records():
+    L, n_chains, seed = 160, 2, 9
+    outs = []
+    for packed in (False, True):
+        with shaken.Shaken(L, n_chains, seed, packed=packed, max_records=8) as s:
+            s.init(0)
+            s.run(0.4, 0.8, 7, 1)
+            outs.append((s.get_spins(0), s.get_spins(1), s.observables()))
+    for a, b in zip(*outs):
+        assert np.array_equal(a, b)
+
+
+# ----------------------------------------------------------------------------- batched chains, grids
+def test_grid_of_couplings_matches_oracle_and_chains_are_independent():
+    """cfg 3 shape at reduced size: per-chain (J, q) tables, 4 replicas per point share couplings but not
+    randomness; chain c of a batch equals the same chain index run alone (counter word 1 = chain)."""
+    L, seed = 64, 11
+    J, q = workloads.grid_couplings()
+    J, q = np.array(J[::16]), np.array(q[::16])          # 32 chains across the whole grid incl. q = 10, 20
+    n = len(J)
+    o = so.Oracle(L, n, seed)
+    o.init(0)
+    o.run_grid(J, q, 12, 1)
+    with shaken.Shaken(L, n, seed, max_records=12) as s:
+        s.init(0)
+        s.run_grid(J, q, 12, 1)
+        assert_same_state(s, o, "grid")
+        rec = s.observables()
+    with shaken.Shaken(L, n, seed, packed=True, max_records=12) as s:
+        s.init(0)
+        s.run_grid(J, q, 12, 1)
+        assert_same_state(s, o, "grid packed")
+    # derived statistics (a9) within 1e-12 relative of the oracle's
+    for ch in (0, 7, 31):
+        a = shaken.derived_stats(rec[2:, ch, 0], L * L)
+        b = so.derived_stats(o.observables()[2:, ch, 0], L * L)
+        for k in ("m", "abs_m", "m2", "m4", "var_m", "binder"):
+            assert a[k] == b[k] or abs(a[k] - b[k]) <= REL * abs(b[k]), (ch, k, a[k], b[k])
+        e1 = shaken.energy(J[ch], q[ch], rec[-1, ch, 2], rec[-1, ch, 3])
+        e2 = so.energy(J[ch], q[ch], o.observables()[-1, ch, 2], o.observables()[-1, ch, 3])
+        assert abs(e1 - e2) <= REL * abs(e2)
+
+
+def test_run_is_resumable_and_step_counter_drives_the_randomness():
+    """run(a); run(b) == run(a+b) bit for bit; set_step + set_spins restores a checkpoint."""
+    L, seed, J, q = 96, 5, 0.5, 0.4
+    with shaken.Shaken(L, 2, seed, max_records=16) as a, shaken.Shaken(L, 2, seed, max_records=16) as b:
+        a.init(0)
+        b.init(0)
+        a.run(J, q, 9, 3)
+        b.run(J, q, 4, 3)
+        b.run(J, q, 5, 3)
+        assert np.array_equal(a.get_spins(0), b.get_spins(0)) and np.array_equal(a.get_spins(1), b.get_spins(1))
+        assert np.array_equal(a.observables(), b.observables()) and a.num_records == 3 and a.step == 9
+        # checkpoint: copy state of a into a fresh context, continue both
+        with shaken.Shaken(L, 2, seed, use_torch=False) as c:
+            c.set_spins(0, a.get_spins(0))
+            c.set_spins(1, a.get_spins(1))
+            c.step = a.step
+            a.run(J, q, 3, 0)
+            c.run(J, q, 3, 0)
+            assert np.array_equal(a.get_spins(0), c.get_spins(0)) and np.array_equal(a.get_spins(1), c.get_spins(1))
+        # a different seed (either key word) changes the trajectory
+        for other in (seed + 1, seed + (1 << 32)):
+            with shaken.Shaken(L, 2, other) as d:
+                d.init(1)
+                d.run(J, q, 1, 0)
+                with shaken.Shaken(L, 2, seed) as e:
+                    e.init(1)
+                    e.run(J, q, 1, 0)
+                    assert not np.array_equal(d.get_spins(0), e.get_spins(0))
+
+
+def test_large_step_index_uses_both_counter_words():
+    """g = 2t + half spills into counter word 3 when t >= 2^31."""
+    L, seed = 32, 3
+    t0 = (1 << 31) - 2
+    o = so.Oracle(L, 1, seed)
+    o.init(0)
+    o.step = t0
+    o.run(0.5, 0.5, 4, 1)
+    for packed in (False, True):
+        with shaken.Shaken(L, 1, seed, packed=packed, max_records=4) as s:
+            s.init(0)
+            s.step = t0
+            s.run(0.5, 0.5, 4, 1)
+            assert_same_state(s, o, "large t")
+
+
+def test_state_io_roundtrip_and_validation():
+    rng = np.random.default_rng(0)
+    for packed, L in ((False, 48), (True, 96)):
+        with shaken.Shaken(L, 2, 1, packed=packed) as s:
+            x = rng.choice(np.array([-1, 1], dtype=np.int8), size=(2, L, L))
+            y = rng.choice(np.array([-1, 1], dtype=np.int8), size=(2, L, L))
+            s.set_spins(0, x)
+            s.set_spins(1, y)
+            assert np.array_equal(s.get_spins(0), x) and np.array_equal(s.get_spins(1), y)
+            bad = x.copy()
+            bad[1, 3, 5] = 0
+            with pytest.raises(shaken.ShakenError) as ei:
+                s.set_spins(0, bad)
+            assert ei.value.code == shaken.EINVAL
+            bad[1, 3, 5] = 3
+            with pytest.raises(shaken.ShakenError):
+                s.set_spins(1, bad)
+
+
+def test_observables_on_known_configurations_and_record_bookkeeping():
+    """All +1 start, frozen couplings: M = L^2, E_q = L^2, E_J = C_x + C_y = 2 L^2 on every record."""
+    L = 64
+    for packed in (False, True):
+        with shaken.Shaken(L, 1, 4, packed=packed, use_torch=False) as s:
+            s.init(1)
+            s.run(0.0, 30.0, 3, 1)          # q = 30: T saturated, each half-step copies the other layer
+            rec = s.observables()
+            assert rec.shape == (3, 1, 6)
+            N = L * L
+            # flip probability 2^-32 per site per half-step: the all +1 state survives 3 steps
+            assert np.array_equal(rec[:, 0], np.array([[N, N, 2 * N, N, N, N]] * 3))
+            s.clear_records()
+            assert s.num_records == 0
+            s.run(0.0, 30.0, 2, 2)
+            assert s.num_records == 1 and s.step == 5
+            s.init(-1)
+            assert s.step == 0 and s.num_records == 0
+            s.run(0.0, 30.0, 1, 1)
+            assert np.array_equal(s.observables()[0, 0], np.array([-N, -N, 2 * N, N, N, N]))
+
+
+def test_bound_record_buffer_reports_enospc_before_doing_any_work():
+    with shaken.Shaken(32, 1, 1, max_records=2) as s:
+        s.init(0)
+        s.run(0.5, 0.5, 2, 1)
+        before = s.get_spins(0).copy()
+        with pytest.raises(shaken.ShakenError) as ei:
+            s.run(0.5, 0.5, 1, 1)
+        assert ei.value.code == shaken.ENOSPC
+        assert s.step == 2 and np.array_equal(s.get_spins(0), before)
+        s.run(0.5, 0.5, 3, 0)                 # no records wanted: fine
+        assert s.step == 5
+
+
+def test_records_against_brute_force_from_downloaded_spins():
+    """Third implementation of the six sums (numpy roll) on the GPU's own final state."""
+    from tests import pins
+
+    L = 112
+    with shaken.Shaken(L, 2, 8, max_records=4) as s:
+        s.init(0)
+        s.run(0.6, 0.3, 4, 4)
+        rec = s.observables()
+        sg, ta = s.get_spins(0), s.get_spins(1)
+        for ch in range(2):
+            assert np.array_equal(rec[0, ch], pins.brute_observables(sg[ch], ta[ch]))
+
+
+def test_cfg1_full_length():
+    """BASELINE.json configs[0], complete: L=64, J=q=0.5, iid start, seed 1, 1000 steps, records every step."""
+    w = workloads.config(1)
+    o = so.Oracle(w.L, 1, w.seed)
+    o.init(w.init)
+    o.run(w.J[0], w.q[0], w.n_steps, w.obs_every)
+    with shaken.Shaken(w.L, 1, w.seed, max_records=w.n_steps) as s:
+        s.init(w.init)
+        s.run(w.J[0], w.q[0], w.n_steps, w.obs_every)
+        assert_same_state(s, o, "cfg1")
+        a = shaken.derived_stats(s.observables()[:, 0, 0], w.n_sites)
+        b = so.derived_stats(o.observables()[:, 0, 0], w.n_sites)
+        for k in a:
+            assert a[k] == b[k] or abs(a[k] - b[k]) <= REL * abs(b[k])

@@ -169,3 +169,29 @@ def test_iid_init_against_curand_words():
                 w = so.philox4x32_10((call, ch, which, 0xFFFFFFFF), key)
                 exp = np.where(w < 2**31, 1, -1)
                 assert np.array_equal(arr[ch].reshape(-1)[4 * call: 4 * call + 4], exp)
+
+
+@needs_curand
+def test_row_restricted_half_step_against_numpy_brute_force_with_curand_words():
+    """oracle.half_step_rows (used for full-size spot checks on the GPU box) is the same per-site statement
+    restricted to a band of rows: pinned on a small torus against eq. (15)/(16) with numpy roll, exact decimal
+    thresholds and cuRAND's words; also equal to the context's full half-steps."""
+    L, seed, chain, J, q, t = 12, 77, 3, 0.45, 0.9, 5
+    rng = np.random.default_rng(3)
+    src = rng.choice(np.array([-1, 1], dtype=np.int8), size=(L, L))
+    table = pins.exact_table(J, q)
+    for half in (0, 1):
+        full = pins.brute_half_step(src, half, table, pins.curand_site_words(seed, chain, 2 * t + half, L * L))
+        for r0, nrows in [(0, L), (0, 1), (L - 1, 1), (4, 5)]:
+            got = so.half_step_rows(src, seed, chain, J, q, t, half, r0, nrows)
+            assert np.array_equal(got, full[r0:r0 + nrows]), (half, r0, nrows)
+    # and the context path: one full step from (src, anything) = half 0 then half 1
+    o = so.Oracle(L, chain + 1, seed)
+    s0 = np.ones((chain + 1, L, L), dtype=np.int8)
+    s0[chain] = src
+    o.set_spins(0, s0)
+    o.step = t
+    o.run(J, q, 1, 0)
+    tau = so.half_step_rows(src, seed, chain, J, q, t, 0, 0, L)
+    assert np.array_equal(o.get_spins(1)[chain], tau)
+    assert np.array_equal(o.get_spins(0)[chain], so.half_step_rows(tau, seed, chain, J, q, t, 1, 0, L))
