@@ -237,9 +237,12 @@ def run_ours(args):
     ms = e0.elapsed_time(e1)
     launches = s.launch_count - l0
     if rank == 0:
-        # keep sampling a little if the region was shorter than a few sampler periods
-        if ms < 300:
-            run(max(1, int(K * 300 / max(ms, 1e-3))))
+        # nvidia-smi needs ~50 ms per sample: keep the same launch sequence running right after the timed region
+        # until at least 0.5 s of load has been sampled (records are discarded; obs cadence unchanged)
+        t_end = time.perf_counter() + max(0.5 - ms * 1e-3, 0.0)
+        while time.perf_counter() < t_end:
+            s.clear_records()
+            run(K)
             s.synchronize()
         sampler.stop()
     if world > 1:

@@ -1,0 +1,197 @@
+// kernel_i8.cuh -- the int8-spin half-step kernel.
+//
+// Spins are bytes 0x01 (+1) / 0xFF (-1): bit 0 is always 1 and every bit 1..7 of a byte is the "minus" flag m.
+//
+// Pipe budget on sm_100a (measured, profiles/r1_ubench.md): a 32x32->64 multiply (IMAD.WIDE) costs two slots
+// of the 64-lane/clk FMA-heavy pipe, so the 18 multiplies of one hoisted Philox call (4 sites) alone cap the
+// kernel at 64 / 9 = 7.1 site-updates per clock per SM.  Everything else is therefore kept OFF that pipe:
+// field/index arithmetic is byte-SIMD logic on the ALU pipe (4 sites per instruction), the threshold comes
+// from shared memory through the LSU, the compare is ISETP plus one predicated XOR.
+//
+// Index encoding.  For one 32-bit word (4 sites) with self word s, vertical neighbour word v and horizontal
+// neighbour word h (byte funnel shift of s with the adjacent word):
+//   z = bitwise select of (s, h, v) = {bits 0,1: 0, bit 3: m_s, bit 4: m_h, bits 2,5,6,7: m_v} per byte: three
+//   LOP3, no addition.  The byte is directly the BYTE OFFSET of the threshold in a 256-byte shared-memory table
+//   in which only the 8 reachable words are filled (8 distinct banks: the lookup never conflicts).
+//   EXTRACT_PRMT : one PRMT per site moves its byte of z into a register (ALU pipe).
+//   EXTRACT_SMEM : the four z words go to a per-thread shared-memory slot and come back one byte at a time
+//                  (LDS.U8): LSU slots instead of ALU slots.
+#pragma once
+#include "kernels_common.cuh"
+
+namespace shaken {
+
+enum : int { EXTRACT_PRMT = 0, EXTRACT_SMEM = 1 };
+
+// byte the EXTRACT_SMEM encoding produces for minus flags (ms, mh, mv)
+__host__ __device__ constexpr uint32_t smem_code(int ms, int mh, int mv)
+{
+    return ((uint32_t)ms << 3) | ((uint32_t)mh << 4) | (mv ? 0xE4u : 0u);
+}
+
+// out ^= c if a < b (unsigned): one ISETP and one predicated LOP3 on the ALU pipe
+__device__ __forceinline__ uint32_t xor_if_less(uint32_t out, uint32_t a, uint32_t b, uint32_t c)
+{
+    asm("{\n\t.reg .pred p;\n\tsetp.lo.u32 p, %1, %2;\n\t@p xor.b32 %0, %0, %3;\n\t}" : "+r"(out) : "r"(a), "r"(b), "r"(c));
+    return out;
+}
+
+template <int HALF, int FLAGS, int EXTRACT, int MINB>
+__global__ void __launch_bounds__(BLOCK_THREADS, MINB) half_step_i8(const __grid_constant__ StepParams p)
+{
+    constexpr bool OBS = (FLAGS & F_OBS) != 0;
+    constexpr bool BONDS = (FLAGS & F_BONDS) != 0;
+    constexpr bool UPDATE = (FLAGS & F_NOUPDATE) == 0;
+    static_assert(!(BONDS && HALF == 1), "bond sums ride on half-step 0");
+
+    __shared__ uint32_t s_tab[64];
+    __shared__ uint32_t s_idx[EXTRACT == EXTRACT_SMEM ? 4 : 1][BLOCK_THREADS];
+
+    const int lane = threadIdx.x & 31;
+    const int warp = threadIdx.x >> 5;
+    const int L = p.L;
+    const int L4 = L >> 2;
+    const int R = p.rows_per_task;
+    const size_t plane = (size_t)L * (size_t)L;
+    const int tpc = p.nrb * p.nseg;                                  // warp tasks per chain
+    const int bpc = (tpc + WARPS_PER_BLOCK - 1) / WARPS_PER_BLOCK;   // block tasks per chain
+
+    int cur_chain = -1;
+    ChainKeys ck = {0u, 0u};
+    int cnt0 = 0, cnt1 = 0, cnt2 = 0;   // half 1: M_sigma, E_J, E_q ; half 0: M_tau, C_x, C_y
+
+    auto flush = [&](int chain) {
+        if (HALF == 1) {
+            if (OBS) {
+                warp_add_to(p.rec_cur + (size_t)chain * 6 + 0, cnt0);
+                warp_add_to(p.rec_cur + (size_t)chain * 6 + 2, cnt1);
+                warp_add_to(p.rec_cur + (size_t)chain * 6 + 3, cnt2);
+            }
+        } else {
+            if (OBS) warp_add_to(p.rec_cur + (size_t)chain * 6 + 1, cnt0);
+            if (BONDS) {
+                warp_add_to(p.rec_prev + (size_t)chain * 6 + 4, cnt1);
+                warp_add_to(p.rec_prev + (size_t)chain * 6 + 5, cnt2);
+            }
+        }
+        cnt0 = cnt1 = cnt2 = 0;
+    };
+
+    for (long long bt = blockIdx.x; bt < p.ntasks; bt += gridDim.x) {
+        const int chain = (int)(bt / bpc);
+        const int lt = (int)(bt % bpc) * WARPS_PER_BLOCK + warp;     // this warp's task inside the chain
+        if (chain != cur_chain) {                                    // block-uniform
+            if ((OBS || BONDS) && cur_chain >= 0) flush(cur_chain);
+            cur_chain = chain;
+            if (UPDATE) {
+                ck = make_chain_keys(p.keys, p.chain0 + (uint32_t)chain);
+                __syncthreads();                                     // everyone is done with the old table
+                if (threadIdx.x < 8) {
+                    const int t = threadIdx.x;
+                    const int ms = t & 1, mh = (t >> 1) & 1, mv = t >> 2;
+                    const int idx = 2 * (2 - mh - mv) + (1 - ms);              // T[2k + c]
+                    s_tab[smem_code(ms, mh, mv) >> 2] = p.gtab ? p.gtab[(size_t)chain * 8 + idx] : p.utab[idx];
+                }
+                __syncthreads();
+            }
+        }
+        const int seg = lt % p.nseg;
+        const int rb = lt / p.nseg;
+        const int cv = seg * 32 + lane;
+        if (lt < tpc && cv < p.nvec) {
+            const int c0 = cv * 16;
+            const int r_first = rb * R;
+            const int r_last = min(L, r_first + R) - 1;
+            const int rows = r_last - r_first + 1;
+            const uint8_t *sbase = reinterpret_cast<const uint8_t *>(p.src) + (size_t)chain * plane;
+            uint8_t *dbase = reinterpret_cast<uint8_t *>(p.dst) + (size_t)chain * plane;
+
+            const int dir = HALF ? -1 : +1;
+            int r = HALF ? r_last : r_first;
+            const int rh = HALF ? (r_last + 1 == L ? 0 : r_last + 1) : (r_first == 0 ? L - 1 : r_first - 1);
+            const int ce = HALF ? (c0 + 16 == L ? 0 : c0 + 16) : (c0 == 0 ? L - 4 : c0 - 4);
+
+            // running pointers (one 64-bit add each per row; no multiplies on the FMA pipe inside the loop)
+            const ptrdiff_t stride = (ptrdiff_t)dir * L;
+            const uint8_t *pc = sbase + (size_t)r * L + c0;          // this lane's 16 spins of the current row
+            const uint8_t *pe = sbase + (size_t)r * L + ce;          // the word holding the horizontal edge spin
+            uint8_t *pd = dbase + (size_t)r * L + c0;
+            uint32_t n = (uint32_t)r * (uint32_t)L4 + (uint32_t)cv * 4u;
+            const uint32_t nstep = (uint32_t)(dir * L4);
+            uint32_t *const my_idx = &s_idx[0][threadIdx.x];
+
+
+            // one row: cq = this row, vq = vertical neighbour row, e = edge word; loads the next row into (nq, en)
+            auto do_row = [&](const uint4 &cq, const uint4 &vq, const uint32_t e, uint4 &nq, uint32_t &en, const bool more) {
+                if (more) {
+                    nq = ldg128(pc + stride);
+                    en = ldg32(pe + stride);
+                }
+                const uint32_t w[4] = {cq.x, cq.y, cq.z, cq.w};
+                const uint32_t vw[4] = {vq.x, vq.y, vq.z, vq.w};
+                uint32_t hw[4], zw[4], ow[4];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    if (HALF == 0) hw[j] = __funnelshift_l(j == 0 ? e : w[j - 1], w[j], 8);   // left neighbours
+                    else           hw[j] = __funnelshift_r(w[j], j == 3 ? e : w[j + 1], 8);   // right neighbours
+                    if (UPDATE) {
+                        const uint32_t y = (hw[j] & 0x10101010u) | (vw[j] & ~0x10101010u);
+                        zw[j] = ((w[j] & 0x08080808u) | (y & ~0x08080808u)) & 0xFCFCFCFCu;
+                        if (EXTRACT == EXTRACT_SMEM) *reinterpret_cast<volatile uint32_t *>(my_idx + j * BLOCK_THREADS) = zw[j];
+                    }
+                }
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    uint32_t out = 0xFFFFFFFFu;
+                    if (UPDATE) {
+                        uint32_t rw[4];
+                        philox_site_words(n + (uint32_t)j, p.keys, ck, rw);
+#pragma unroll
+                        for (int b = 0; b < 4; ++b) {
+                            uint32_t code;
+                            if (EXTRACT == EXTRACT_SMEM)
+                                code = reinterpret_cast<volatile const uint8_t *>(my_idx + j * BLOCK_THREADS)[b];
+                            else
+                                code = b == 3 ? (zw[j] >> 24) : __byte_perm(zw[j], 0u, 0x4440u + b);
+                            const uint32_t T = *reinterpret_cast<const uint32_t *>(reinterpret_cast<const char *>(s_tab) + code);
+                            out = xor_if_less(out, rw[b], T, 0xFEu << (8 * b));
+                        }
+                        ow[j] = out;
+                    }
+                    // observables: spins are signed bytes +-1, so a sum of spin products over 4 sites is ONE
+                    // signed 8-bit dot product (IDP.4A) accumulated in int32 -- exact, no masks, no flushes
+                    const int s = (int)w[j], v = (int)vw[j], hh = (int)hw[j], o = (int)out;
+                    if (HALF == 1) {
+                        if (OBS) {
+                            cnt0 = __dp4a(o, 0x01010101, cnt0);   // M_sigma  = sum sigma'_x
+                            cnt1 = __dp4a(o, v, cnt1);            // E_J     += sum sigma'_x tau_{x up}
+                            cnt1 = __dp4a(o, hh, cnt1);           //          + sum sigma'_x tau_{x right}
+                            cnt2 = __dp4a(o, s, cnt2);            // E_q      = sum sigma'_x tau_x
+                        }
+                    } else {
+                        if (OBS) cnt0 = __dp4a(o, 0x01010101, cnt0);   // M_tau = sum tau'_x
+                        if (BONDS) {
+                            cnt1 = __dp4a(s, hh, cnt1);           // C_x = sum sigma_x sigma_{x left}
+                            cnt2 = __dp4a(s, v, cnt2);            // C_y = sum sigma_x sigma_{x down}
+                        }
+                    }
+                }
+                if (UPDATE) *reinterpret_cast<uint4 *>(pd) = make_uint4(ow[0], ow[1], ow[2], ow[3]);
+                pc += stride; pe += stride; pd += stride;
+                n += nstep;
+            };
+
+            // three row buffers rotate roles (vertical neighbour / current / prefetched) without register moves
+            uint4 B0 = ldg128(sbase + (size_t)rh * L + c0), B1 = ldg128(pc), B2 = B1;
+            uint32_t e0 = 0, e1 = ldg32(pe), e2 = 0;
+            for (int i = 0;;) {
+                do_row(B1, B0, e1, B2, e2, i + 1 < rows); if (++i == rows) break;
+                do_row(B2, B1, e2, B0, e0, i + 1 < rows); if (++i == rows) break;
+                do_row(B0, B2, e0, B1, e1, i + 1 < rows); if (++i == rows) break;
+            }
+        }
+    }
+    if ((OBS || BONDS) && cur_chain >= 0) flush(cur_chain);
+}
+
+} // namespace shaken

@@ -1,210 +1,10 @@
-// kernels.cuh -- sm_100a kernels of libshaken: the shaken-dynamics half-step (eq. (15)-(16))
-// on int8 and bit-packed spins, with fused observable sums (eq. (17) :196, eq. (5) :81-84).
-//
-// Work decomposition (both layouts).  A *task* is a column strip of one warp: 32 lanes x one vector
-// (int8: 16 spins = one 16-byte load; packed: one 32-spin word) wide, `rows_per_task` rows high, of one chain.
-// A lane walks its strip row by row IN THE DIRECTION OF THE FIELD (half 0 reads down/left, so rows ascend
-// and the previous row in registers is the "down" neighbour; half 1 reads up/right, rows descend), which
-// leaves one halo row per task and, per row, the one spin left (right) of the lane's vector, taken from
-// an extra 4-byte load that hits the line the neighbouring lane just fetched.  The next row is loaded
-// before the current one is computed.  Warps loop over tasks with a grid sized to the machine.
-//
-// Acceptance ("rand() < p"): new spin = +1 iff rnd < T[idx], T looked up in shared memory
-// by a byte offset that is computed for 4 sites at a time with byte-SIMD integer arithmetic.
+// kernels.cuh -- bit-packed half-step kernel, initialisation, layout conversion, validation, test hook.
+// (The int8 half-step kernel is in kernel_i8.cuh; shared declarations in kernels_common.cuh.)
 #pragma once
-#include <cuda_runtime.h>
-#include <stdint.h>
-
-#include "philox.cuh"
+#include "kernels_common.cuh"
+#include "kernel_i8.cuh"
 
 namespace shaken {
-
-constexpr int WARPS_PER_BLOCK = 8;
-constexpr int BLOCK_THREADS = WARPS_PER_BLOCK * 32;
-constexpr int MAX_ROWS_PER_TASK = 16;   // byte-wide observable counters overflow beyond 31 rows
-
-enum : int { F_OBS = 1, F_BONDS = 2, F_NOUPDATE = 4 };
-
-struct StepParams {
-    const void *src;        // sublattice that is read   (half 0: sigma, half 1: tau)
-    void *dst;              // sublattice that is redrawn (half 0: tau,   half 1: sigma)
-    int L;                  // lattice side
-    int nvec;               // vectors per row: L/16 (int8) or L/32 (packed)
-    int n_chains;
-    uint32_t chain0;        // global index of chain 0 of this context (Philox counter word 1 = chain0 + chain)
-    int rows_per_task;
-    int nseg;               // warp-wide strips per row = ceil(nvec / 32)
-    int nrb;                // row blocks = ceil(L / rows_per_task)
-    long long ntasks;       // n_chains * nrb * nseg
-    const uint32_t *gtab;   // per-chain tables [n_chains][8] in global memory, or nullptr: use utab
-    uint32_t utab[8];       // one table for all chains (kernel parameters live in constant memory)
-    long long *rec_cur;     // [n_chains][6] record of the step being computed (F_OBS) or nullptr
-    long long *rec_prev;    // [n_chains][6] record whose C_x, C_y are still owed (F_BONDS) or nullptr
-    StepKeys keys;
-};
-
-__device__ __forceinline__ uint4 ldg128(const void *p) { return __ldg(reinterpret_cast<const uint4 *>(p)); }
-__device__ __forceinline__ uint32_t ldg32(const void *p) { return __ldg(reinterpret_cast<const uint32_t *>(p)); }
-
-__device__ __forceinline__ int bytes_sum(uint32_t acc) { return (int)__dp4a(acc, 0x01010101u, 0u); }
-
-__device__ __forceinline__ void warp_add_to(long long *addr, int v)
-{
-    int s = __reduce_add_sync(0xFFFFFFFFu, v);
-    if ((threadIdx.x & 31) == 0 && s != 0) atomicAdd(reinterpret_cast<unsigned long long *>(addr), (unsigned long long)(long long)s);
-}
-
-// ===================================================================================================
-// int8 layout.  Spins are bytes 0x01 (+1) / 0xFF (-1); every bit 1..7 of a byte is the "minus" flag m.
-// Table order in shared memory: index i' = m_self + 2 (m_vert + m_horz), tab[i'] = T[5 - i'].
-// ===================================================================================================
-template <int HALF, int FLAGS>
-__global__ void __launch_bounds__(BLOCK_THREADS, 2) half_step_i8(const __grid_constant__ StepParams p)
-{
-    constexpr bool OBS = (FLAGS & F_OBS) != 0;
-    constexpr bool BONDS = (FLAGS & F_BONDS) != 0;
-    constexpr bool UPDATE = (FLAGS & F_NOUPDATE) == 0;
-    static_assert(!(BONDS && HALF == 1), "bond sums ride on half-step 0");
-
-    __shared__ uint32_t s_tab[WARPS_PER_BLOCK][8];
-    const int lane = threadIdx.x & 31;
-    const int warp = threadIdx.x >> 5;
-    uint32_t *tabw = s_tab[warp];
-
-    const int L = p.L;
-    const int L4 = L >> 2;
-    const int R = p.rows_per_task;
-    const size_t plane = (size_t)L * (size_t)L;
-
-    int cur_chain = -1;
-    ChainKeys ck = {0u, 0u};
-    int cnt0 = 0, cnt1 = 0, cnt2 = 0;   // half 1: M_sigma, E_J, E_q ; half 0: M_tau, C_x, C_y
-
-    auto flush = [&](int chain) {
-        if (HALF == 1) {
-            if (OBS) {
-                warp_add_to(p.rec_cur + (size_t)chain * 6 + 0, cnt0);
-                warp_add_to(p.rec_cur + (size_t)chain * 6 + 2, cnt1);
-                warp_add_to(p.rec_cur + (size_t)chain * 6 + 3, cnt2);
-            }
-        } else {
-            if (OBS) warp_add_to(p.rec_cur + (size_t)chain * 6 + 1, cnt0);
-            if (BONDS) {
-                warp_add_to(p.rec_prev + (size_t)chain * 6 + 4, cnt1);
-                warp_add_to(p.rec_prev + (size_t)chain * 6 + 5, cnt2);
-            }
-        }
-        cnt0 = cnt1 = cnt2 = 0;
-    };
-
-    const long long nw = (long long)gridDim.x * WARPS_PER_BLOCK;
-    for (long long task = (long long)blockIdx.x * WARPS_PER_BLOCK + warp; task < p.ntasks; task += nw) {
-        const int seg = (int)(task % p.nseg);
-        const long long t2 = task / p.nseg;
-        const int rb = (int)(t2 % p.nrb);
-        const int chain = (int)(t2 / p.nrb);
-        if (chain != cur_chain) {
-            if ((OBS || BONDS) && cur_chain >= 0) flush(cur_chain);
-            cur_chain = chain;
-            if (UPDATE) {
-                ck = make_chain_keys(p.keys, p.chain0 + (uint32_t)chain);
-                __syncwarp();
-                if (lane < 8) tabw[lane] = p.gtab ? p.gtab[(size_t)chain * 8 + lane] : p.utab[lane];
-                __syncwarp();
-            }
-        }
-        const int cv = seg * 32 + lane;
-        if (cv >= p.nvec) continue;
-
-        const int c0 = cv * 16;
-        const int r_first = rb * R;
-        const int r_last = min(L, r_first + R) - 1;
-        const int rows = r_last - r_first + 1;
-        const uint8_t *sbase = reinterpret_cast<const uint8_t *>(p.src) + (size_t)chain * plane;
-        uint8_t *dbase = reinterpret_cast<uint8_t *>(p.dst) + (size_t)chain * plane;
-
-        const int dir = HALF ? -1 : +1;
-        int r = HALF ? r_last : r_first;
-        const int rh = HALF ? (r_last + 1 == L ? 0 : r_last + 1) : (r_first == 0 ? L - 1 : r_first - 1);
-        const int ce = HALF ? (c0 + 16 == L ? 0 : c0 + 16) : (c0 == 0 ? L - 4 : c0 - 4);
-
-        uint4 vq = ldg128(sbase + (size_t)rh * L + c0);
-        uint4 cq = ldg128(sbase + (size_t)r * L + c0);
-        uint32_t e = ldg32(sbase + (size_t)r * L + ce);
-        uint32_t n = (uint32_t)r * (uint32_t)L4 + (uint32_t)cv * 4u;
-
-        uint32_t acc0 = 0, acc1 = 0, acc2 = 0, acc3 = 0;   // byte-wide partial counts (x2)
-
-        for (int i = 0; i < rows; ++i) {
-            uint4 nq = cq;
-            uint32_t en = e;
-            if (i + 1 < rows) {
-                const int rn = r + dir;
-                nq = ldg128(sbase + (size_t)rn * L + c0);
-                en = ldg32(sbase + (size_t)rn * L + ce);
-            }
-            const uint32_t w[4] = {cq.x, cq.y, cq.z, cq.w};
-            const uint32_t vw[4] = {vq.x, vq.y, vq.z, vq.w};
-            uint32_t ow[4];
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                const uint32_t s = w[j];
-                const uint32_t v = vw[j];
-                uint32_t hh;
-                if (HALF == 0) hh = __funnelshift_l(j == 0 ? e : w[j - 1], s, 8);   // left neighbours
-                else           hh = __funnelshift_r(s, j == 3 ? e : w[j + 1], 8);   // right neighbours
-                uint32_t out = 0;
-                if (UPDATE) {
-                    const uint32_t off = (s & 0x04040404u) + (v & 0x08080808u) + (hh & 0x08080808u);
-                    uint32_t rw[4];
-                    philox_site_words(n + (uint32_t)j, p.keys, ck, rw);
-#pragma unroll
-                    for (int b = 0; b < 4; ++b) {
-                        const uint32_t o = (off >> (8 * b)) & 0xFFu;
-                        const uint32_t T = *reinterpret_cast<const uint32_t *>(reinterpret_cast<const char *>(tabw) + o);
-                        out |= (rw[b] < T ? 0x01u : 0xFFu) << (8 * b);
-                    }
-                    ow[j] = out;
-                }
-                if (HALF == 1) {
-                    if (OBS) {
-                        acc0 += out & 0x02020202u;            // minus count of sigma'
-                        acc1 += (out ^ v) & 0x02020202u;      // sigma'_x tau_{x up}    anti-aligned
-                        acc3 += (out ^ hh) & 0x02020202u;     // sigma'_x tau_{x right} anti-aligned
-                        acc2 += (out ^ s) & 0x02020202u;      // sigma'_x tau_x         anti-aligned
-                    }
-                } else {
-                    if (OBS) acc0 += out & 0x02020202u;       // minus count of tau'
-                    if (BONDS) {
-                        acc1 += (s ^ hh) & 0x02020202u;       // sigma_x sigma_{x left}  anti-aligned
-                        acc2 += (s ^ v) & 0x02020202u;        // sigma_x sigma_{x down}  anti-aligned
-                    }
-                }
-            }
-            if (UPDATE) *reinterpret_cast<uint4 *>(dbase + (size_t)r * L + c0) = make_uint4(ow[0], ow[1], ow[2], ow[3]);
-            vq = cq; cq = nq; e = en;
-            r += dir;
-            n += (uint32_t)(dir * L4);
-        }
-        if (OBS || BONDS) {
-            const int ns = rows * 16;
-            if (HALF == 1) {
-                if (OBS) {
-                    cnt0 += ns - bytes_sum(acc0);
-                    cnt1 += 2 * ns - bytes_sum(acc1) - bytes_sum(acc3);
-                    cnt2 += ns - bytes_sum(acc2);
-                }
-            } else {
-                if (OBS) cnt0 += ns - bytes_sum(acc0);
-                if (BONDS) {
-                    cnt1 += ns - bytes_sum(acc1);
-                    cnt2 += ns - bytes_sum(acc2);
-                }
-            }
-        }
-    }
-    if ((OBS || BONDS) && cur_chain >= 0) flush(cur_chain);
-}
 
 // ===================================================================================================
 // Bit-packed layout: 32 spins per word, bit 1 <-> +1.  A word is spread into eight byte-SIMD registers

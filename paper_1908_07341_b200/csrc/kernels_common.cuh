@@ -1,0 +1,57 @@
+// kernels_common.cuh -- sm_100a kernels of libshaken: the shaken-dynamics half-step (eq. (15)-(16))
+// on int8 and bit-packed spins, with fused observable sums (eq. (17) :196, eq. (5) :81-84).
+//
+// Work decomposition (both layouts).  A *task* is a column strip of one warp: 32 lanes x one vector
+// (int8: 16 spins = one 16-byte load; packed: one 32-spin word) wide, `rows_per_task` rows high, of one chain.
+// A lane walks its strip row by row IN THE DIRECTION OF THE FIELD (half 0 reads down/left, so rows ascend
+// and the previous row in registers is the "down" neighbour; half 1 reads up/right, rows descend), which
+// leaves one halo row per task and, per row, the one spin left (right) of the lane's vector, taken from
+// an extra 4-byte load that hits the line the neighbouring lane just fetched.  The next row is loaded
+// before the current one is computed.  Warps loop over tasks with a grid sized to the machine.
+//
+// Acceptance ("rand() < p"): new spin = +1 iff rnd < T[idx], T looked up in shared memory
+// by a byte offset that is computed for 4 sites at a time with byte-SIMD integer arithmetic.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "philox.cuh"
+
+namespace shaken {
+
+constexpr int WARPS_PER_BLOCK = 8;
+constexpr int BLOCK_THREADS = WARPS_PER_BLOCK * 32;
+constexpr int MAX_ROWS_PER_TASK = 16;   // byte-wide observable counters overflow beyond 31 rows
+
+enum : int { F_OBS = 1, F_BONDS = 2, F_NOUPDATE = 4 };
+
+struct StepParams {
+    const void *src;        // sublattice that is read   (half 0: sigma, half 1: tau)
+    void *dst;              // sublattice that is redrawn (half 0: tau,   half 1: sigma)
+    int L;                  // lattice side
+    int nvec;               // vectors per row: L/16 (int8) or L/32 (packed)
+    int n_chains;
+    uint32_t chain0;        // global index of chain 0 of this context (Philox counter word 1 = chain0 + chain)
+    int rows_per_task;
+    int nseg;               // warp-wide strips per row = ceil(nvec / 32)
+    int nrb;                // row blocks = ceil(L / rows_per_task)
+    long long ntasks;       // n_chains * nrb * nseg
+    const uint32_t *gtab;   // per-chain tables [n_chains][8] in global memory, or nullptr: use utab
+    uint32_t utab[8];       // one table for all chains (kernel parameters live in constant memory)
+    long long *rec_cur;     // [n_chains][6] record of the step being computed (F_OBS) or nullptr
+    long long *rec_prev;    // [n_chains][6] record whose C_x, C_y are still owed (F_BONDS) or nullptr
+    StepKeys keys;
+};
+
+__device__ __forceinline__ uint4 ldg128(const void *p) { return __ldg(reinterpret_cast<const uint4 *>(p)); }
+__device__ __forceinline__ uint32_t ldg32(const void *p) { return __ldg(reinterpret_cast<const uint32_t *>(p)); }
+
+__device__ __forceinline__ int bytes_sum(uint32_t acc) { return (int)__dp4a(acc, 0x01010101u, 0u); }
+
+__device__ __forceinline__ void warp_add_to(long long *addr, int v)
+{
+    int s = __reduce_add_sync(0xFFFFFFFFu, v);
+    if ((threadIdx.x & 31) == 0 && s != 0) atomicAdd(reinterpret_cast<unsigned long long *>(addr), (unsigned long long)(long long)s);
+}
+
+} // namespace shaken

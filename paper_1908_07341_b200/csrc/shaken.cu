@@ -96,12 +96,10 @@ extern "C" int shaken_thresholds(double J, double q, uint32_t out[6])
     return SHAKEN_OK;
 }
 
-// table in the order the kernel indexes it (kernels.cuh): int8 uses the minus-count index i' = 5 - idx
-static void kernel_table(double J, double q, bool packed, uint32_t tab[8])
+// table as the kernels read it: natural order T[2k + c], padded to 8 words
+static void kernel_table(double J, double q, uint32_t tab[8])
 {
-    uint32_t T[6];
-    shaken_thresholds(J, q, T);
-    for (int i = 0; i < 6; ++i) tab[i] = packed ? T[i] : T[5 - i];
+    shaken_thresholds(J, q, tab);
     tab[6] = tab[7] = 0;
 }
 
@@ -350,7 +348,8 @@ template <int HALF, int FLAGS>
 static cudaError_t launch_half(const shaken_ctx *ctx, const StepParams &p, int grid)
 {
     if (ctx->packed) half_step_pk<HALF, FLAGS><<<grid, BLOCK_THREADS, 0, ctx->stream>>>(p);
-    else half_step_i8<HALF, FLAGS><<<grid, BLOCK_THREADS, 0, ctx->stream>>>(p);
+    else if (ctx->variant == 1) half_step_i8<HALF, FLAGS, EXTRACT_PRMT, 2><<<grid, BLOCK_THREADS, 0, ctx->stream>>>(p);
+    else half_step_i8<HALF, FLAGS, EXTRACT_SMEM, 2><<<grid, BLOCK_THREADS, 0, ctx->stream>>>(p);
     return cudaGetLastError();
 }
 
@@ -391,10 +390,12 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
     p.nseg = (p.nvec + 31) / 32;
     p.rows_per_task = choose_rows_per_task(ctx, p.nseg);
     p.nrb = (ctx->L + p.rows_per_task - 1) / p.rows_per_task;
-    p.ntasks = (long long)ctx->n_chains * p.nrb * p.nseg;
+    p.ntasks = (long long)ctx->n_chains * p.nrb * p.nseg;                      // warp tasks (packed kernel)
+    if (!ctx->packed)                                                             // int8 kernel: block tasks
+        p.ntasks = (long long)ctx->n_chains * (((long long)p.nrb * p.nseg + WARPS_PER_BLOCK - 1) / WARPS_PER_BLOCK);
 
     if (uniform) {
-        kernel_table(J[0], q[0], ctx->packed, p.utab);
+        kernel_table(J[0], q[0], p.utab);
         p.gtab = nullptr;
     } else {
         if (!ctx->d_tab && cudaMalloc(&ctx->d_tab, (size_t)ctx->n_chains * 8 * sizeof(uint32_t)) != cudaSuccess) {
@@ -402,15 +403,15 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
             return fail(ctx, SHAKEN_ENOMEM, "cudaMalloc of the threshold tables failed");
         }
         std::vector<uint32_t> h((size_t)ctx->n_chains * 8);
-        for (int i = 0; i < ctx->n_chains; ++i) kernel_table(J[i], q[i], ctx->packed, &h[(size_t)i * 8]);
+        for (int i = 0; i < ctx->n_chains; ++i) kernel_table(J[i], q[i], &h[(size_t)i * 8]);
         // pageable source: the copy is staged before the call returns, so h may go out of scope
         CU(cudaMemcpyAsync(ctx->d_tab, h.data(), h.size() * sizeof(uint32_t), cudaMemcpyHostToDevice, ctx->stream));
         CU(cudaStreamSynchronize(ctx->stream));
         p.gtab = ctx->d_tab;
     }
 
-    const long long blocks_needed = (p.ntasks + WARPS_PER_BLOCK - 1) / WARPS_PER_BLOCK;
-    const long long cap = (long long)ctx->num_sms * 4;
+    const long long blocks_needed = ctx->packed ? (p.ntasks + WARPS_PER_BLOCK - 1) / WARPS_PER_BLOCK : p.ntasks;
+    const long long cap = (long long)ctx->num_sms * 2;   // two resident 256-thread blocks per SM (launch bounds)
     const int grid = (int)(blocks_needed < cap ? blocks_needed : cap);
     const size_t rec_stride = (size_t)ctx->n_chains * SHAKEN_N_OBS;
 
