@@ -29,13 +29,6 @@ __host__ __device__ constexpr uint32_t smem_code(int ms, int mh, int mv)
     return ((uint32_t)ms << 3) | ((uint32_t)mh << 4) | (mv ? 0xE4u : 0u);
 }
 
-// out ^= c if a < b (unsigned): one ISETP and one predicated LOP3 on the ALU pipe
-__device__ __forceinline__ uint32_t xor_if_less(uint32_t out, uint32_t a, uint32_t b, uint32_t c)
-{
-    asm("{\n\t.reg .pred p;\n\tsetp.lo.u32 p, %1, %2;\n\t@p xor.b32 %0, %0, %3;\n\t}" : "+r"(out) : "r"(a), "r"(b), "r"(c));
-    return out;
-}
-
 template <int HALF, int FLAGS, int EXTRACT, int MINB>
 __global__ void __launch_bounds__(BLOCK_THREADS, MINB) half_step_i8(const __grid_constant__ StepParams p)
 {

@@ -54,4 +54,11 @@ __device__ __forceinline__ void warp_add_to(long long *addr, int v)
     if ((threadIdx.x & 31) == 0 && s != 0) atomicAdd(reinterpret_cast<unsigned long long *>(addr), (unsigned long long)(long long)s);
 }
 
+// out ^= c if a < b (unsigned): one ISETP and one predicated LOP3
+__device__ __forceinline__ uint32_t xor_if_less(uint32_t out, uint32_t a, uint32_t b, uint32_t c)
+{
+    asm("{\n\t.reg .pred p;\n\tsetp.lo.u32 p, %1, %2;\n\t@p xor.b32 %0, %0, %3;\n\t}" : "+r"(out) : "r"(a), "r"(b), "r"(c));
+    return out;
+}
+
 } // namespace shaken

@@ -390,9 +390,8 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
     p.nseg = (p.nvec + 31) / 32;
     p.rows_per_task = choose_rows_per_task(ctx, p.nseg);
     p.nrb = (ctx->L + p.rows_per_task - 1) / p.rows_per_task;
-    p.ntasks = (long long)ctx->n_chains * p.nrb * p.nseg;                      // warp tasks (packed kernel)
-    if (!ctx->packed)                                                             // int8 kernel: block tasks
-        p.ntasks = (long long)ctx->n_chains * (((long long)p.nrb * p.nseg + WARPS_PER_BLOCK - 1) / WARPS_PER_BLOCK);
+    // block tasks: WARPS_PER_BLOCK consecutive warp strips of one chain
+    p.ntasks = (long long)ctx->n_chains * (((long long)p.nrb * p.nseg + WARPS_PER_BLOCK - 1) / WARPS_PER_BLOCK);
 
     if (uniform) {
         kernel_table(J[0], q[0], p.utab);
@@ -410,7 +409,7 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
         p.gtab = ctx->d_tab;
     }
 
-    const long long blocks_needed = ctx->packed ? (p.ntasks + WARPS_PER_BLOCK - 1) / WARPS_PER_BLOCK : p.ntasks;
+    const long long blocks_needed = p.ntasks;
     const long long cap = (long long)ctx->num_sms * 2;   // two resident 256-thread blocks per SM (launch bounds)
     const int grid = (int)(blocks_needed < cap ? blocks_needed : cap);
     const size_t rec_stride = (size_t)ctx->n_chains * SHAKEN_N_OBS;
