@@ -4,6 +4,7 @@
 #include "kernels_common.cuh"
 #include "kernel_i8.cuh"
 #include "kernel_pk.cuh"
+#include "kernel_small.cuh"
 
 namespace shaken {
 

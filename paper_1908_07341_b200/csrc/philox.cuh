@@ -92,16 +92,18 @@ __device__ __forceinline__ ChainKeys make_chain_keys(const StepKeys &K, uint32_t
     return c;
 }
 
-// The four random words of sites 4n .. 4n+3.
-__device__ __forceinline__ void philox_site_words(uint32_t n, const StepKeys &K, const ChainKeys &C, uint32_t r[4])
+// The four random words of sites 4n .. 4n+3.  xa2, xb0: the per-half-step uniform words (StepKeys::xa2, ::xb0,
+// or the same values computed on the device by a kernel that loops over steps itself).
+__device__ __forceinline__ void philox_site_words(uint32_t n, const StepKeys &K, const uint32_t xa2, const uint32_t xb0,
+                                                  const ChainKeys &C, uint32_t r[4])
 {
     uint32_t h0, l0, h1, l1;
     // round 0: c = (n, chain, g_lo, g_hi)
     mul_wide(PHILOX_M0, n, h0, l0);
-    uint32_t a2 = h0 ^ K.xa2, a3 = l0;
+    uint32_t a2 = h0 ^ xa2, a3 = l0;
     // round 1: c = (a0 [uniform], a1 [uniform], a2, a3)
     mul_wide(PHILOX_M1, a2, h1, l1);
-    uint32_t c0 = h1 ^ K.xb0, c1 = l1, c2 = a3 ^ C.xb2;          // c3 = lo(M0*a0), folded into xd2
+    uint32_t c0 = h1 ^ xb0, c1 = l1, c2 = a3 ^ C.xb2;            // c3 = lo(M0*a0), folded into xd2
     // round 2
     mul_wide(PHILOX_M0, c0, h0, l0);
     mul_wide(PHILOX_M1, c2, h1, l1);
@@ -119,6 +121,26 @@ __device__ __forceinline__ void philox_site_words(uint32_t n, const StepKeys &K,
         c3 = l0;
     }
     r[0] = c0; r[1] = c1; r[2] = c2; r[3] = c3;
+}
+
+__device__ __forceinline__ void philox_site_words(uint32_t n, const StepKeys &K, const ChainKeys &C, uint32_t r[4])
+{
+    philox_site_words(n, K, K.xa2, K.xb0, C, r);
+}
+
+// Device-side form of the per-half-step part of make_step_keys + make_chain_keys, for kernels that advance
+// several steps in one launch: K supplies only the round keys k0[], k1[] (functions of the seed).
+__device__ __forceinline__ void device_half_step_keys(const StepKeys &K, uint64_t g, uint32_t chain, uint32_t &xa2, uint32_t &xb0, ChainKeys &C)
+{
+    uint32_t hi, lo;
+    mul_wide(PHILOX_M1, (uint32_t)g, hi, lo);
+    xa2 = (uint32_t)(g >> 32) ^ K.k1[0];
+    xb0 = lo ^ K.k0[1];
+    const uint32_t a0 = hi ^ chain ^ K.k0[0];
+    uint32_t h, l;
+    mul_wide(PHILOX_M0, a0, h, l);
+    C.xb2 = h ^ K.k1[1];
+    C.xd2 = l ^ K.k1[2];
 }
 
 } // namespace shaken

@@ -409,6 +409,34 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
         p.gtab = ctx->d_tab;
     }
 
+    // small-lattice path: one CTA per chain keeps both sublattices in shared memory for the whole run
+    if (!ctx->packed && ctx->L <= SMALL_L_MAX && ctx->variant != 3) {
+        SmallParams sp;
+        memset(&sp, 0, sizeof(sp));
+        sp.sigma = (uint8_t *)ctx->d_sigma;
+        sp.tau = (uint8_t *)ctx->d_tau;
+        sp.L = ctx->L;
+        sp.n_chains = ctx->n_chains;
+        sp.chain0 = ctx->chain0;
+        sp.t0 = ctx->step;
+        sp.n_steps = n_steps;
+        sp.obs_every = obs_every;
+        sp.rec = ctx->d_rec ? ctx->d_rec + (size_t)ctx->n_rec * ctx->n_chains * SHAKEN_N_OBS : nullptr;
+        sp.gtab = p.gtab;
+        memcpy(sp.utab, p.utab, sizeof(sp.utab));
+        make_step_keys(ctx->seed, 0, sp.keys);
+        const int ncalls = ctx->L * ctx->L / 4;
+        int threads = ncalls < SMALL_THREADS ? ((ncalls + 31) / 32) * 32 : SMALL_THREADS;
+        const size_t smem = (size_t)2 * ctx->L * ctx->L;
+        if (smem > 48 * 1024) CU(cudaFuncSetAttribute(small_run_i8, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        small_run_i8<<<ctx->n_chains, threads, smem, ctx->stream>>>(sp);
+        CU(cudaGetLastError());
+        ctx->launches++;
+        ctx->step += (uint64_t)n_steps;
+        ctx->n_rec += n_new;
+        return SHAKEN_OK;
+    }
+
     const long long blocks_needed = p.ntasks;
     const long long cap = (long long)ctx->num_sms * 2;   // two resident 256-thread blocks per SM (launch bounds)
     const int grid = (int)(blocks_needed < cap ? blocks_needed : cap);

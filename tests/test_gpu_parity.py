@@ -270,3 +270,23 @@ def test_cfg1_full_length():
         b = so.derived_stats(o.observables()[:, 0, 0], w.n_sites)
         for k in a:
             assert a[k] == b[k] or abs(a[k] - b[k]) <= REL * abs(b[k])
+
+
+@pytest.mark.parametrize("L,n_chains", [(16, 1), (48, 3), (64, 2), (128, 2)])
+def test_small_lattice_path_and_generic_kernels_both_match_oracle(L, n_chains):
+    """L <= 128 runs in the one-CTA-per-chain persistent kernel (kernel_small.cuh); variant 3 forces the generic
+    strip kernels and variant 1 the PRMT extraction.  All must equal the oracle, records included, also when a
+    run is split and obs_every does not divide the split."""
+    seed = 77 + L
+    J = np.linspace(0.2, 0.9, n_chains)
+    q = np.linspace(1.5, 0.1, n_chains)
+    o = so.Oracle(L, n_chains, seed)
+    o.init(0)
+    o.run_grid(J, q, 11, 3)
+    for variant in (0, 1, 3):
+        with shaken.Shaken(L, n_chains, seed, max_records=8) as s:
+            s.set_variant(variant)
+            s.init(0)
+            s.run_grid(J, q, 4, 3)
+            s.run_grid(J, q, 7, 3)
+            assert_same_state(s, o, f"L={L} variant={variant}")
