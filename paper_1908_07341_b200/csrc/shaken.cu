@@ -349,6 +349,9 @@ static cudaError_t launch_half(const shaken_ctx *ctx, const StepParams &p, int g
 {
     if (ctx->packed) half_step_pk<HALF, FLAGS><<<grid, BLOCK_THREADS, 0, ctx->stream>>>(p);
     else if (ctx->variant == 1) half_step_i8<HALF, FLAGS, EXTRACT_PRMT, 2><<<grid, BLOCK_THREADS, 0, ctx->stream>>>(p);
+    else if (ctx->variant == 4) half_step_i8<HALF, FLAGS, EXTRACT_SMEM, 3><<<grid, BLOCK_THREADS, 0, ctx->stream>>>(p);
+    else if (ctx->variant == 5) half_step_i8<HALF, FLAGS, EXTRACT_SMEM, 4><<<grid, BLOCK_THREADS, 0, ctx->stream>>>(p);
+    else if (ctx->variant == 6) half_step_i8<HALF, FLAGS, EXTRACT_PRMT, 3><<<grid, BLOCK_THREADS, 0, ctx->stream>>>(p);
     else half_step_i8<HALF, FLAGS, EXTRACT_SMEM, 2><<<grid, BLOCK_THREADS, 0, ctx->stream>>>(p);
     return cudaGetLastError();
 }
@@ -438,7 +441,8 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
     }
 
     const long long blocks_needed = p.ntasks;
-    const long long cap = (long long)ctx->num_sms * 2;   // two resident 256-thread blocks per SM (launch bounds)
+    const int resident = ctx->variant == 5 ? 4 : (ctx->variant == 4 || ctx->variant == 6) ? 3 : 2;
+    const long long cap = (long long)ctx->num_sms * resident;   // resident 256-thread blocks per SM (launch bounds)
     const int grid = (int)(blocks_needed < cap ? blocks_needed : cap);
     const size_t rec_stride = (size_t)ctx->n_chains * SHAKEN_N_OBS;
 
