@@ -142,6 +142,30 @@ def test_grid_of_couplings_matches_oracle_and_chains_are_independent():
         assert abs(e1 - e2) <= REL * abs(e2)
 
 
+def test_batch_sharded_over_two_contexts_equals_the_single_batch():
+    """a batch split into per-rank contexts with shaken_set_chain_offset is bit-identical to
+    the single batch (here both 'ranks' run one after the other on the one GPU; no kernel waits on another)."""
+    from paper_1908_07341_b200 import parallel
+
+    L, n, seed, steps = 128 + 16, 5, 29, 7                # above the small-lattice path, ragged strip
+    J = np.array([0.2, 0.45, 0.7, 0.05, 1.1])
+    q = np.array([0.3, 10.0, 0.7, 2.0, 0.1])
+    o = so.Oracle(L, n, seed)
+    o.init(0)
+    o.run_grid(J, q, steps, 1)
+    want_rec, want_sigma = o.observables(), o.get_spins(0)
+    for packed in (False,) if L % 32 else (False, True):
+        for world in (2, 3):
+            for rank in range(world):
+                first, count = parallel.chain_shard(n, world, rank)
+                Jl, ql = parallel.shard_couplings(J, q, world, rank)
+                with parallel.open_shard(L, n, seed, world, rank, packed=packed, max_records=steps) as s:
+                    s.init(0)
+                    s.run_grid(Jl, ql, steps, 1)
+                    assert np.array_equal(s.observables(), want_rec[:, first:first + count]), (world, rank)
+                    assert np.array_equal(s.get_spins(0), want_sigma[first:first + count]), (world, rank)
+
+
 def test_run_is_resumable_and_step_counter_drives_the_randomness():
     """run(a); run(b) == run(a+b) bit for bit; set_step + set_spins restores a checkpoint."""
     L, seed, J, q = 96, 5, 0.5, 0.4
