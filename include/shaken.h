@@ -178,8 +178,9 @@ int shaken_philox_words(const uint32_t *ctr, const uint32_t *key, uint32_t *out,
 /* Number of kernels this context has launched so far (half-steps, init, conversions, reductions). */
 int64_t shaken_launch_count(const shaken_ctx *ctx);
 
-/* Kernel variant: 0 = automatic (default), other values select a specific code path for measurement
- * (see DESIGN.md "Kernels").  Results never depend on the variant. */
+/* Kernel variant: 0 = automatic (default); other values select a specific code path for measurement and tests
+ * (DESIGN.md "Kernels"): 1 PRMT index extraction, 2 the round-1 v2 kernel, 3 generic strip kernels also for L <= 128,
+ * 4 shared-memory index extraction, 5 paired lookup, 6 IDP extraction.  Results never depend on the variant. */
 int shaken_set_variant(shaken_ctx *ctx, int variant);
 
 /* Message for the most recent error on this context ("" if none).  ctx may be NULL (creation errors). */

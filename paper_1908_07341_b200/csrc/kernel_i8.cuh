@@ -21,7 +21,7 @@
 
 namespace shaken {
 
-enum : int { EXTRACT_PRMT = 0, EXTRACT_SMEM = 1 };
+enum : int { EXTRACT_PRMT = 0, EXTRACT_SMEM = 1, EXTRACT_IDP = 2, EXTRACT_PAIR = 3, PACK_ADD = 16, PREFETCH2 = 32 };
 
 // byte the EXTRACT_SMEM encoding produces for minus flags (ms, mh, mv)
 __host__ __device__ constexpr uint32_t smem_code(int ms, int mh, int mv)
@@ -29,9 +29,12 @@ __host__ __device__ constexpr uint32_t smem_code(int ms, int mh, int mv)
     return ((uint32_t)ms << 3) | ((uint32_t)mh << 4) | (mv ? 0xE4u : 0u);
 }
 
-template <int HALF, int FLAGS, int EXTRACT, int MINB>
+template <int HALF, int FLAGS, int EXTRACT_, int MINB>
 __global__ void __launch_bounds__(BLOCK_THREADS, MINB) half_step_i8(const __grid_constant__ StepParams p)
 {
+    constexpr int EXTRACT = EXTRACT_ & 15;
+    constexpr bool PACKADD = (EXTRACT_ & PACK_ADD) != 0;
+    constexpr int AHEAD = (EXTRACT_ & PREFETCH2) ? 2 : 1;   // rows between a load and its first use
     constexpr bool OBS = (FLAGS & F_OBS) != 0;
     constexpr bool BONDS = (FLAGS & F_BONDS) != 0;
     constexpr bool UPDATE = (FLAGS & F_NOUPDATE) == 0;
@@ -39,6 +42,10 @@ __global__ void __launch_bounds__(BLOCK_THREADS, MINB) half_step_i8(const __grid
 
     __shared__ uint32_t s_tab[64];
     __shared__ uint32_t s_idx[EXTRACT == EXTRACT_SMEM ? 4 : 1][BLOCK_THREADS];
+    // EXTRACT_PAIR: thresholds of TWO sites per lookup.  Entry e = c_even + 8 c_odd (c = m_self + 2 m_horizontal +
+    // 4 m_vertical) holds {T(c_even), T(c_odd)}, replicated per lane: lane l reads 8 bytes at e * 256 + l * 8, i.e.
+    // always banks 2l, 2l+1 -- conflict-free for any mix of indices.  16 KiB per block.
+    __shared__ uint2 s_pair[EXTRACT == EXTRACT_PAIR ? 64 : 1][32];
 
     const int lane = threadIdx.x & 31;
     const int warp = threadIdx.x >> 5;
@@ -79,7 +86,20 @@ __global__ void __launch_bounds__(BLOCK_THREADS, MINB) half_step_i8(const __grid
             if (UPDATE) {
                 ck = make_chain_keys(p.keys, p.chain0 + (uint32_t)chain);
                 __syncthreads();                                     // everyone is done with the old table
-                if (threadIdx.x < 8) {
+                if (EXTRACT == EXTRACT_PAIR) {
+                    for (int t = threadIdx.x; t < 64 * 32; t += BLOCK_THREADS) {
+                        const int e = t >> 5;
+                        uint32_t T2[2];
+#pragma unroll
+                        for (int h = 0; h < 2; ++h) {
+                            const int c = h ? (e >> 3) : (e & 7);
+                            const int ms = c & 1, mh = (c >> 1) & 1, mv = c >> 2;
+                            const int idx = 2 * (2 - mh - mv) + (1 - ms);      // T[2k + c]
+                            T2[h] = p.gtab ? p.gtab[(size_t)chain * 8 + idx] : p.utab[idx];
+                        }
+                        s_pair[e][t & 31] = make_uint2(T2[0], T2[1]);
+                    }
+                } else if (threadIdx.x < 8) {
                     const int t = threadIdx.x;
                     const int ms = t & 1, mh = (t >> 1) & 1, mv = t >> 2;
                     const int idx = 2 * (2 - mh - mv) + (1 - ms);              // T[2k + c]
@@ -111,14 +131,15 @@ __global__ void __launch_bounds__(BLOCK_THREADS, MINB) half_step_i8(const __grid
             uint8_t *pd = dbase + (size_t)r * L + c0;
             uint32_t n = (uint32_t)r * (uint32_t)L4 + (uint32_t)cv * 4u;
             const uint32_t nstep = (uint32_t)(dir * L4);
-            uint32_t *const my_idx = &s_idx[0][threadIdx.x];
+            uint32_t *const my_idx = &s_idx[0][EXTRACT == EXTRACT_SMEM ? threadIdx.x : 0];
+            const uint32_t lane8 = (uint32_t)lane * 8u;
 
 
             // one row: cq = this row, vq = vertical neighbour row, e = edge word; loads the next row into (nq, en)
             auto do_row = [&](const uint4 &cq, const uint4 &vq, const uint32_t e, uint4 &nq, uint32_t &en, const bool more) {
                 if (more) {
-                    nq = ldg128(pc + stride);
-                    en = ldg32(pe + stride);
+                    nq = ldg128(pc + AHEAD * stride);
+                    en = ldg32(pe + AHEAD * stride);
                 }
                 const uint32_t w[4] = {cq.x, cq.y, cq.z, cq.w};
                 const uint32_t vw[4] = {vq.x, vq.y, vq.z, vq.w};
@@ -127,7 +148,11 @@ __global__ void __launch_bounds__(BLOCK_THREADS, MINB) half_step_i8(const __grid
                 for (int j = 0; j < 4; ++j) {
                     if (HALF == 0) hw[j] = __funnelshift_l(j == 0 ? e : w[j - 1], w[j], 8);   // left neighbours
                     else           hw[j] = __funnelshift_r(w[j], j == 3 ? e : w[j + 1], 8);   // right neighbours
-                    if (UPDATE) {
+                    if (UPDATE && EXTRACT == EXTRACT_PAIR) {
+                        // code bits (m_self, m_horizontal, m_vertical) at bits 1-3 of even bytes, 5-7 of odd bytes
+                        const uint32_t y = (hw[j] & 0x40044004u) | (vw[j] & ~0x40044004u);
+                        zw[j] = ((w[j] & 0x20022002u) | (y & ~0x20022002u)) & 0xE00EE00Eu;
+                    } else if (UPDATE) {
                         const uint32_t y = (hw[j] & 0x10101010u) | (vw[j] & ~0x10101010u);
                         zw[j] = ((w[j] & 0x08080808u) | (y & ~0x08080808u)) & 0xFCFCFCFCu;
                         if (EXTRACT == EXTRACT_SMEM) *reinterpret_cast<volatile uint32_t *>(my_idx + j * BLOCK_THREADS) = zw[j];
@@ -135,19 +160,35 @@ __global__ void __launch_bounds__(BLOCK_THREADS, MINB) half_step_i8(const __grid
                 }
 #pragma unroll
                 for (int j = 0; j < 4; ++j) {
-                    uint32_t out = 0xFFFFFFFFu;
+                    uint32_t out = PACKADD ? 0x01010101u : 0xFFFFFFFFu;
                     if (UPDATE) {
                         uint32_t rw[4];
                         philox_site_words(n + (uint32_t)j, p.keys, ck, rw);
+                        uint32_t Tp[4];
+                        if (EXTRACT == EXTRACT_PAIR) {
+                            // one IDP.4A per pair forms the whole byte offset: (2 c_even) * 128 + (32 c_odd) * 64 + lane * 8
+                            const uint32_t o01 = __dp4a(zw[j], 0x00004080u, lane8), o23 = __dp4a(zw[j], 0x40800000u, lane8);
+                            const uint2 t01 = *reinterpret_cast<const uint2 *>(reinterpret_cast<const char *>(s_pair) + o01);
+                            const uint2 t23 = *reinterpret_cast<const uint2 *>(reinterpret_cast<const char *>(s_pair) + o23);
+                            Tp[0] = t01.x; Tp[1] = t01.y; Tp[2] = t23.x; Tp[3] = t23.y;
+                        }
 #pragma unroll
                         for (int b = 0; b < 4; ++b) {
+                            if (EXTRACT == EXTRACT_PAIR) {
+                                if (PACKADD) out = add_if_not_less(out, rw[b], Tp[b], 0xFEu << (8 * b));
+                                else out = xor_if_less(out, rw[b], Tp[b], 0xFEu << (8 * b));
+                                continue;
+                            }
                             uint32_t code;
                             if (EXTRACT == EXTRACT_SMEM)
                                 code = reinterpret_cast<volatile const uint8_t *>(my_idx + j * BLOCK_THREADS)[b];
+                            else if (EXTRACT == EXTRACT_IDP)
+                                code = __dp4a(zw[j], 1u << (8 * b), 0u);      // byte b of zw[j] on the multiplier pipe
                             else
                                 code = b == 3 ? (zw[j] >> 24) : __byte_perm(zw[j], 0u, 0x4440u + b);
                             const uint32_t T = *reinterpret_cast<const uint32_t *>(reinterpret_cast<const char *>(s_tab) + code);
-                            out = xor_if_less(out, rw[b], T, 0xFEu << (8 * b));
+                            if (PACKADD) out = add_if_not_less(out, rw[b], T, 0xFEu << (8 * b));
+                            else out = xor_if_less(out, rw[b], T, 0xFEu << (8 * b));
                         }
                         ow[j] = out;
                     }
@@ -177,10 +218,23 @@ __global__ void __launch_bounds__(BLOCK_THREADS, MINB) half_step_i8(const __grid
             // three row buffers rotate roles (vertical neighbour / current / prefetched) without register moves
             uint4 B0 = ldg128(sbase + (size_t)rh * L + c0), B1 = ldg128(pc), B2 = B1;
             uint32_t e0 = 0, e1 = ldg32(pe), e2 = 0;
-            for (int i = 0;;) {
-                do_row(B1, B0, e1, B2, e2, i + 1 < rows); if (++i == rows) break;
-                do_row(B2, B1, e2, B0, e0, i + 1 < rows); if (++i == rows) break;
-                do_row(B0, B2, e0, B1, e1, i + 1 < rows); if (++i == rows) break;
+            if (AHEAD == 1) {
+                for (int i = 0;;) {
+                    do_row(B1, B0, e1, B2, e2, i + 1 < rows); if (++i == rows) break;
+                    do_row(B2, B1, e2, B0, e0, i + 1 < rows); if (++i == rows) break;
+                    do_row(B0, B2, e0, B1, e1, i + 1 < rows); if (++i == rows) break;
+                }
+            } else {
+                // four buffers: the row loaded while row i is computed is row i + 2
+                uint4 B3 = B1;
+                uint32_t e3 = 0;
+                if (rows > 1) { B2 = ldg128(pc + stride); e2 = ldg32(pe + stride); }
+                for (int i = 0;;) {
+                    do_row(B1, B0, e1, B3, e3, i + 2 < rows); if (++i == rows) break;
+                    do_row(B2, B1, e2, B0, e0, i + 2 < rows); if (++i == rows) break;
+                    do_row(B3, B2, e3, B1, e1, i + 2 < rows); if (++i == rows) break;
+                    do_row(B0, B3, e0, B2, e2, i + 2 < rows); if (++i == rows) break;
+                }
             }
         }
     }

@@ -21,7 +21,7 @@ namespace shaken {
 
 constexpr int WARPS_PER_BLOCK = 8;
 constexpr int BLOCK_THREADS = WARPS_PER_BLOCK * 32;
-constexpr int MAX_ROWS_PER_TASK = 16;   // byte-wide observable counters overflow beyond 31 rows
+constexpr int MAX_ROWS_PER_TASK = 4096;   // int32 observable partials: 2 * 512 * rows per warp stay far below 2^31
 
 enum : int { F_OBS = 1, F_BONDS = 2, F_NOUPDATE = 4 };
 
@@ -58,6 +58,13 @@ __device__ __forceinline__ void warp_add_to(long long *addr, int v)
 __device__ __forceinline__ uint32_t xor_if_less(uint32_t out, uint32_t a, uint32_t b, uint32_t c)
 {
     asm("{\n\t.reg .pred p;\n\tsetp.lo.u32 p, %1, %2;\n\t@p xor.b32 %0, %0, %3;\n\t}" : "+r"(out) : "r"(a), "r"(b), "r"(c));
+    return out;
+}
+
+// out += c if !(a < b) (unsigned): one ISETP and one predicated add (IADD3 costs about half a LOP3 on the ALU port)
+__device__ __forceinline__ uint32_t add_if_not_less(uint32_t out, uint32_t a, uint32_t b, uint32_t c)
+{
+    asm("{\n\t.reg .pred p;\n\tsetp.hs.u32 p, %1, %2;\n\t@p add.u32 %0, %0, %3;\n\t}" : "+r"(out) : "r"(a), "r"(b), "r"(c));
     return out;
 }
 

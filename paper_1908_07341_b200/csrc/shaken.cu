@@ -347,22 +347,47 @@ extern "C" int shaken_init(shaken_ctx *ctx, int mode)
 template <int HALF, int FLAGS>
 static cudaError_t launch_half(const shaken_ctx *ctx, const StepParams &p, int grid)
 {
+    // int8 code paths (results identical).  Automatic choice: launches that also accumulate
+    // observables keep the multiplier pipe free of extra IDP.4A (index bytes go through shared memory), plain
+    // half-steps use the paired lookup (one IDP.4A + one LDS.64 per two sites).
+    constexpr int TUNED = PACK_ADD | PREFETCH2;
+    constexpr int AUTO = ((FLAGS & (F_OBS | F_BONDS)) ? EXTRACT_SMEM : EXTRACT_PAIR) | TUNED;
     if (ctx->packed) half_step_pk<HALF, FLAGS><<<grid, BLOCK_THREADS, 0, ctx->stream>>>(p);
-    else if (ctx->variant == 1) half_step_i8<HALF, FLAGS, EXTRACT_PRMT, 2><<<grid, BLOCK_THREADS, 0, ctx->stream>>>(p);
-    else if (ctx->variant == 4) half_step_i8<HALF, FLAGS, EXTRACT_SMEM, 3><<<grid, BLOCK_THREADS, 0, ctx->stream>>>(p);
-    else if (ctx->variant == 5) half_step_i8<HALF, FLAGS, EXTRACT_SMEM, 4><<<grid, BLOCK_THREADS, 0, ctx->stream>>>(p);
-    else if (ctx->variant == 6) half_step_i8<HALF, FLAGS, EXTRACT_PRMT, 3><<<grid, BLOCK_THREADS, 0, ctx->stream>>>(p);
-    else half_step_i8<HALF, FLAGS, EXTRACT_SMEM, 2><<<grid, BLOCK_THREADS, 0, ctx->stream>>>(p);
+    else switch (ctx->variant) {
+        case 1: half_step_i8<HALF, FLAGS, EXTRACT_PRMT | TUNED, 2><<<grid, BLOCK_THREADS, 0, ctx->stream>>>(p); break;
+        case 2: half_step_i8<HALF, FLAGS, EXTRACT_SMEM, 2><<<grid, BLOCK_THREADS, 0, ctx->stream>>>(p); break;   // round-1 v2 kernel
+        case 4: half_step_i8<HALF, FLAGS, EXTRACT_SMEM | TUNED, 2><<<grid, BLOCK_THREADS, 0, ctx->stream>>>(p); break;
+        case 5: half_step_i8<HALF, FLAGS, EXTRACT_PAIR | TUNED, 2><<<grid, BLOCK_THREADS, 0, ctx->stream>>>(p); break;
+        case 6: half_step_i8<HALF, FLAGS, EXTRACT_IDP | TUNED, 2><<<grid, BLOCK_THREADS, 0, ctx->stream>>>(p); break;
+        default: half_step_i8<HALF, FLAGS, AUTO, 2><<<grid, BLOCK_THREADS, 0, ctx->stream>>>(p); break;
+    }
     return cudaGetLastError();
 }
 
-static int choose_rows_per_task(const shaken_ctx *ctx, int nseg)
+static int choose_rows_per_task(const shaken_ctx *ctx, int nseg, long long grid_cap)
 {
-    // enough tasks to fill the machine a few times over, strips as tall as possible otherwise
-    const long long want = (long long)ctx->num_sms * 2 * WARPS_PER_BLOCK * 4;
-    int R = MAX_ROWS_PER_TASK;
-    while (R > 2 && (long long)ctx->n_chains * nseg * ((ctx->L + R - 1) / R) < want) R >>= 1;
-    return R;
+    // Strip height R.  Tall strips amortise the halo row and the unprefetched loads at a strip's start; the persistent
+    // grid walks block tasks (8 warp strips of one chain) round-robin, so the last wave should be full and so should
+    // the 8 warps of a block task.  Maximise
+    //     fill * warp_use * machine * R / (R + 1.5)
+    // fill = ntasks / (grid * waves), warp_use = strips per chain / (8 * block tasks per chain), machine = grid / cap.
+    int best = 4;
+    double best_score = -1.0;
+    const int Rmax = ctx->L < MAX_ROWS_PER_TASK ? ctx->L : MAX_ROWS_PER_TASK;
+    for (int R = Rmax; R >= 4; --R) {
+        const long long nrb = (ctx->L + R - 1) / R;
+        const long long tpc = nrb * nseg;
+        const long long bpc = (tpc + WARPS_PER_BLOCK - 1) / WARPS_PER_BLOCK;
+        const long long ntasks = (long long)ctx->n_chains * bpc;
+        const long long grid = ntasks < grid_cap ? ntasks : grid_cap;
+        const long long waves = (ntasks + grid - 1) / grid;
+        const double fill = (double)ntasks / (double)(grid * waves);
+        const double warp_use = (double)ctx->L / (double)(nrb * R) * (double)tpc / (double)(bpc * WARPS_PER_BLOCK);
+        const double machine = (double)grid / (double)grid_cap;
+        const double score = fill * warp_use * machine * ((double)R / ((double)R + 1.5));
+        if (score > best_score + 1e-9) { best_score = score; best = R; }
+    }
+    return best;
 }
 
 static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool uniform, int64_t n_steps, int64_t obs_every)
@@ -391,7 +416,9 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
     p.n_chains = ctx->n_chains;
     p.chain0 = ctx->chain0;
     p.nseg = (p.nvec + 31) / 32;
-    p.rows_per_task = choose_rows_per_task(ctx, p.nseg);
+    const int resident = 2;
+    const long long cap = (long long)ctx->num_sms * resident;   // resident 256-thread blocks per SM (launch bounds)
+    p.rows_per_task = choose_rows_per_task(ctx, p.nseg, cap);
     p.nrb = (ctx->L + p.rows_per_task - 1) / p.rows_per_task;
     // block tasks: WARPS_PER_BLOCK consecutive warp strips of one chain
     p.ntasks = (long long)ctx->n_chains * (((long long)p.nrb * p.nseg + WARPS_PER_BLOCK - 1) / WARPS_PER_BLOCK);
@@ -413,7 +440,7 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
     }
 
     // small-lattice path: one CTA per chain keeps both sublattices in shared memory for the whole run
-    if (!ctx->packed && ctx->L <= SMALL_L_MAX && ctx->variant != 3) {
+    if (!ctx->packed && ctx->L <= SMALL_L_MAX && ctx->variant == 0) {
         SmallParams sp;
         memset(&sp, 0, sizeof(sp));
         sp.sigma = (uint8_t *)ctx->d_sigma;
@@ -441,8 +468,6 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
     }
 
     const long long blocks_needed = p.ntasks;
-    const int resident = ctx->variant == 5 ? 4 : (ctx->variant == 4 || ctx->variant == 6) ? 3 : 2;
-    const long long cap = (long long)ctx->num_sms * resident;   // resident 256-thread blocks per SM (launch bounds)
     const int grid = (int)(blocks_needed < cap ? blocks_needed : cap);
     const size_t rec_stride = (size_t)ctx->n_chains * SHAKEN_N_OBS;
 

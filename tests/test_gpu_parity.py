@@ -298,19 +298,38 @@ def test_cfg1_full_length():
 
 @pytest.mark.parametrize("L,n_chains", [(16, 1), (48, 3), (64, 2), (128, 2)])
 def test_small_lattice_path_and_generic_kernels_both_match_oracle(L, n_chains):
-    """L <= 128 runs in the one-CTA-per-chain persistent kernel (kernel_small.cuh); variant 3 forces the generic
-    strip kernels and variant 1 the PRMT extraction.  All must equal the oracle, records included, also when a
-    run is split and obs_every does not divide the split."""
+    """L <= 128 runs in the one-CTA-per-chain persistent kernel (kernel_small.cuh) under variant 0; every other
+    variant forces one of the generic strip kernels (include/shaken.h).  All must equal the oracle, records included,
+    also when a run is split and obs_every does not divide the split."""
     seed = 77 + L
     J = np.linspace(0.2, 0.9, n_chains)
     q = np.linspace(1.5, 0.1, n_chains)
     o = so.Oracle(L, n_chains, seed)
     o.init(0)
     o.run_grid(J, q, 11, 3)
-    for variant in (0, 1, 3):
+    for variant in (0, 1, 2, 3, 4, 5, 6):
         with shaken.Shaken(L, n_chains, seed, max_records=8) as s:
             s.set_variant(variant)
             s.init(0)
             s.run_grid(J, q, 4, 3)
             s.run_grid(J, q, 7, 3)
             assert_same_state(s, o, f"L={L} variant={variant}")
+
+
+@pytest.mark.parametrize("variant", [0, 1, 2, 4, 5, 6])
+def test_every_int8_code_path_matches_oracle_on_a_ragged_lattice(variant):
+    """L = 272: 17 vectors per row (ragged warp strip), several row blocks per chain, three chains with different
+    couplings incl. a saturated table; records on some steps only, so launches with and without fused sums, the
+    deferred bond sums and the closing read-only pass all occur."""
+    L, n, seed = 272, 3, 41
+    J = np.array([0.44, 0.7, 0.05])
+    q = np.array([0.66, 0.7, 20.0])
+    o = so.Oracle(L, n, seed)
+    o.init(0)
+    o.run_grid(J, q, 9, 2)
+    with shaken.Shaken(L, n, seed, max_records=8) as s:
+        s.set_variant(variant)
+        s.init(0)
+        s.run_grid(J, q, 5, 2)
+        s.run_grid(J, q, 4, 2)
+        assert_same_state(s, o, f"variant={variant}")
