@@ -29,9 +29,10 @@ __host__ __device__ constexpr uint32_t smem_code(int ms, int mh, int mv)
     return ((uint32_t)ms << 3) | ((uint32_t)mh << 4) | (mv ? 0xE4u : 0u);
 }
 
-template <int HALF, int FLAGS, int EXTRACT_, int MINB>
-__global__ void __launch_bounds__(BLOCK_THREADS, MINB) half_step_i8(const __grid_constant__ StepParams p)
+template <int HALF, int FLAGS, int EXTRACT_, int MINB, int THREADS = BLOCK_THREADS>
+__global__ void __launch_bounds__(THREADS, MINB) half_step_i8(const __grid_constant__ StepParams p)
 {
+    constexpr int WPB = THREADS / 32;                       // warp strips per block task
     constexpr int EXTRACT = EXTRACT_ & 15;
     constexpr bool PACKADD = (EXTRACT_ & PACK_ADD) != 0;
     constexpr int AHEAD = (EXTRACT_ & PREFETCH2) ? 2 : 1;   // rows between a load and its first use
@@ -41,7 +42,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, MINB) half_step_i8(const __grid
     static_assert(!(BONDS && HALF == 1), "bond sums ride on half-step 0");
 
     __shared__ uint32_t s_tab[64];
-    __shared__ uint32_t s_idx[EXTRACT == EXTRACT_SMEM ? 4 : 1][BLOCK_THREADS];
+    __shared__ uint32_t s_idx[EXTRACT == EXTRACT_SMEM ? 4 : 1][THREADS];
     // EXTRACT_PAIR: thresholds of TWO sites per lookup.  Entry e = c_even + 8 c_odd (c = m_self + 2 m_horizontal +
     // 4 m_vertical) holds {T(c_even), T(c_odd)}, replicated per lane: lane l reads 8 bytes at e * 256 + l * 8, i.e.
     // always banks 2l, 2l+1 -- conflict-free for any mix of indices.  16 KiB per block.
@@ -54,7 +55,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, MINB) half_step_i8(const __grid
     const int R = p.rows_per_task;
     const size_t plane = (size_t)L * (size_t)L;
     const int tpc = p.nrb * p.nseg;                                  // warp tasks per chain
-    const int bpc = (tpc + WARPS_PER_BLOCK - 1) / WARPS_PER_BLOCK;   // block tasks per chain
+    const int bpc = (tpc + WPB - 1) / WPB;                           // block tasks per chain
 
     int cur_chain = -1;
     ChainKeys ck = {0u, 0u};
@@ -79,7 +80,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, MINB) half_step_i8(const __grid
 
     for (long long bt = blockIdx.x; bt < p.ntasks; bt += gridDim.x) {
         const int chain = (int)(bt / bpc);
-        const int lt = (int)(bt % bpc) * WARPS_PER_BLOCK + warp;     // this warp's task inside the chain
+        const int lt = (int)(bt % bpc) * WPB + warp;     // this warp's task inside the chain
         if (chain != cur_chain) {                                    // block-uniform
             if ((OBS || BONDS) && cur_chain >= 0) flush(cur_chain);
             cur_chain = chain;
@@ -87,7 +88,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, MINB) half_step_i8(const __grid
                 ck = make_chain_keys(p.keys, p.chain0 + (uint32_t)chain);
                 __syncthreads();                                     // everyone is done with the old table
                 if (EXTRACT == EXTRACT_PAIR) {
-                    for (int t = threadIdx.x; t < 64 * 32; t += BLOCK_THREADS) {
+                    for (int t = threadIdx.x; t < 64 * 32; t += THREADS) {
                         const int e = t >> 5;
                         uint32_t T2[2];
 #pragma unroll
@@ -155,7 +156,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, MINB) half_step_i8(const __grid
                     } else if (UPDATE) {
                         const uint32_t y = (hw[j] & 0x10101010u) | (vw[j] & ~0x10101010u);
                         zw[j] = ((w[j] & 0x08080808u) | (y & ~0x08080808u)) & 0xFCFCFCFCu;
-                        if (EXTRACT == EXTRACT_SMEM) *reinterpret_cast<volatile uint32_t *>(my_idx + j * BLOCK_THREADS) = zw[j];
+                        if (EXTRACT == EXTRACT_SMEM) *reinterpret_cast<volatile uint32_t *>(my_idx + j * THREADS) = zw[j];
                     }
                 }
 #pragma unroll
@@ -181,7 +182,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, MINB) half_step_i8(const __grid
                             }
                             uint32_t code;
                             if (EXTRACT == EXTRACT_SMEM)
-                                code = reinterpret_cast<volatile const uint8_t *>(my_idx + j * BLOCK_THREADS)[b];
+                                code = reinterpret_cast<volatile const uint8_t *>(my_idx + j * THREADS)[b];
                             else if (EXTRACT == EXTRACT_IDP)
                                 code = __dp4a(zw[j], 1u << (8 * b), 0u);      // byte b of zw[j] on the multiplier pipe
                             else

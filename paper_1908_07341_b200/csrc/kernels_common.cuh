@@ -21,6 +21,7 @@ namespace shaken {
 
 constexpr int WARPS_PER_BLOCK = 8;
 constexpr int BLOCK_THREADS = WARPS_PER_BLOCK * 32;
+constexpr int I8_THREADS = 512;         // int8 half-step: one 512-thread block per SM, up to 128 registers per thread
 constexpr int MAX_ROWS_PER_TASK = 4096;   // int32 observable partials: 2 * 512 * rows per warp stay far below 2^31
 
 enum : int { F_OBS = 1, F_BONDS = 2, F_NOUPDATE = 4 };

@@ -354,17 +354,18 @@ static cudaError_t launch_half(const shaken_ctx *ctx, const StepParams &p, int g
     constexpr int AUTO = ((FLAGS & (F_OBS | F_BONDS)) ? EXTRACT_SMEM : EXTRACT_PAIR) | TUNED;
     if (ctx->packed) half_step_pk<HALF, FLAGS><<<grid, BLOCK_THREADS, 0, ctx->stream>>>(p);
     else switch (ctx->variant) {
-        case 1: half_step_i8<HALF, FLAGS, EXTRACT_PRMT | TUNED, 2><<<grid, BLOCK_THREADS, 0, ctx->stream>>>(p); break;
+        case 1: half_step_i8<HALF, FLAGS, EXTRACT_PRMT | TUNED, 1, I8_THREADS><<<grid, I8_THREADS, 0, ctx->stream>>>(p); break;
         case 2: half_step_i8<HALF, FLAGS, EXTRACT_SMEM, 2><<<grid, BLOCK_THREADS, 0, ctx->stream>>>(p); break;   // round-1 v2 kernel
-        case 4: half_step_i8<HALF, FLAGS, EXTRACT_SMEM | TUNED, 2><<<grid, BLOCK_THREADS, 0, ctx->stream>>>(p); break;
-        case 5: half_step_i8<HALF, FLAGS, EXTRACT_PAIR | TUNED, 2><<<grid, BLOCK_THREADS, 0, ctx->stream>>>(p); break;
-        case 6: half_step_i8<HALF, FLAGS, EXTRACT_IDP | TUNED, 2><<<grid, BLOCK_THREADS, 0, ctx->stream>>>(p); break;
-        default: half_step_i8<HALF, FLAGS, AUTO, 2><<<grid, BLOCK_THREADS, 0, ctx->stream>>>(p); break;
+        case 4: half_step_i8<HALF, FLAGS, EXTRACT_SMEM | TUNED, 1, I8_THREADS><<<grid, I8_THREADS, 0, ctx->stream>>>(p); break;
+        case 5: half_step_i8<HALF, FLAGS, EXTRACT_PAIR | TUNED, 1, I8_THREADS><<<grid, I8_THREADS, 0, ctx->stream>>>(p); break;
+        case 6: half_step_i8<HALF, FLAGS, EXTRACT_IDP | TUNED, 1, I8_THREADS><<<grid, I8_THREADS, 0, ctx->stream>>>(p); break;
+        case 7: half_step_i8<HALF, FLAGS, AUTO, 2><<<grid, BLOCK_THREADS, 0, ctx->stream>>>(p); break;          // 2 x 256 threads
+        default: half_step_i8<HALF, FLAGS, AUTO, 1, I8_THREADS><<<grid, I8_THREADS, 0, ctx->stream>>>(p); break;
     }
     return cudaGetLastError();
 }
 
-static int choose_rows_per_task(const shaken_ctx *ctx, int nseg, long long grid_cap)
+static int choose_rows_per_task(const shaken_ctx *ctx, int nseg, long long grid_cap, int wpb)
 {
     // Strip height R.  Tall strips amortise the halo row and the unprefetched loads at a strip's start; the persistent
     // grid walks block tasks (8 warp strips of one chain) round-robin, so the last wave should be full and so should
@@ -377,12 +378,12 @@ static int choose_rows_per_task(const shaken_ctx *ctx, int nseg, long long grid_
     for (int R = Rmax; R >= 4; --R) {
         const long long nrb = (ctx->L + R - 1) / R;
         const long long tpc = nrb * nseg;
-        const long long bpc = (tpc + WARPS_PER_BLOCK - 1) / WARPS_PER_BLOCK;
+        const long long bpc = (tpc + wpb - 1) / wpb;
         const long long ntasks = (long long)ctx->n_chains * bpc;
         const long long grid = ntasks < grid_cap ? ntasks : grid_cap;
         const long long waves = (ntasks + grid - 1) / grid;
         const double fill = (double)ntasks / (double)(grid * waves);
-        const double warp_use = (double)ctx->L / (double)(nrb * R) * (double)tpc / (double)(bpc * WARPS_PER_BLOCK);
+        const double warp_use = (double)ctx->L / (double)(nrb * R) * (double)tpc / (double)(bpc * wpb);
         const double machine = (double)grid / (double)grid_cap;
         const double score = fill * warp_use * machine * ((double)R / ((double)R + 1.5));
         if (score > best_score + 1e-9) { best_score = score; best = R; }
@@ -416,12 +417,13 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
     p.n_chains = ctx->n_chains;
     p.chain0 = ctx->chain0;
     p.nseg = (p.nvec + 31) / 32;
-    const int resident = 2;
-    const long long cap = (long long)ctx->num_sms * resident;   // resident 256-thread blocks per SM (launch bounds)
-    p.rows_per_task = choose_rows_per_task(ctx, p.nseg, cap);
+    int resident = 2, wpb = WARPS_PER_BLOCK;                  // resident blocks per SM (launch bounds), warps per block
+    if (!ctx->packed && ctx->variant != 2 && ctx->variant != 7) { resident = 1; wpb = I8_THREADS / 32; }
+    const long long cap = (long long)ctx->num_sms * resident;
+    p.rows_per_task = choose_rows_per_task(ctx, p.nseg, cap, wpb);
     p.nrb = (ctx->L + p.rows_per_task - 1) / p.rows_per_task;
     // block tasks: WARPS_PER_BLOCK consecutive warp strips of one chain
-    p.ntasks = (long long)ctx->n_chains * (((long long)p.nrb * p.nseg + WARPS_PER_BLOCK - 1) / WARPS_PER_BLOCK);
+    p.ntasks = (long long)ctx->n_chains * (((long long)p.nrb * p.nseg + wpb - 1) / wpb);
 
     if (uniform) {
         kernel_table(J[0], q[0], p.utab);
