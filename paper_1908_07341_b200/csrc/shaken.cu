@@ -36,6 +36,10 @@ struct shaken_ctx {
     int64_t n_rec = 0;
     uint32_t *d_tab = nullptr;    // [n_chains][8] per-chain tables for shaken_run_grid
     unsigned long long *d_bad = nullptr;
+    uint2 *d_xch = nullptr;       // band path: exchange rows xs, xt ([2][n_bands][L/4] {word, stamp} each)
+    size_t xch_bytes = 0;
+    uint32_t xch_stamp = 0;       // last stamp written into d_xch
+    int coop = -1;                // cooperative launch supported (-1: not queried yet)
     void *d_stage = nullptr;      // staging for packed <-> int8 conversion
     size_t stage_bytes = 0;
 
@@ -141,6 +145,7 @@ extern "C" int shaken_destroy(shaken_ctx *ctx)
     cudaFree(ctx->d_tab);
     cudaFree(ctx->d_bad);
     cudaFree(ctx->d_stage);
+    cudaFree(ctx->d_xch);
     delete ctx;
     return SHAKEN_OK;
 }
@@ -467,6 +472,75 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
         ctx->step += (uint64_t)n_steps;
         ctx->n_rec += n_new;
         return SHAKEN_OK;
+    }
+
+    // band path: mid-size lattices, few chains -- the whole run in one cooperative launch (kernel_band.cuh)
+    if (!ctx->packed && ctx->variant == 0 && ctx->L > SMALL_L_MAX && ctx->L <= BAND_L_MAX && ctx->n_chains <= ctx->num_sms) {
+        if (ctx->coop < 0) {
+            int dev = 0, v = 0;
+            CU(cudaGetDevice(&dev));
+            CU(cudaDeviceGetAttribute(&v, cudaDevAttrCooperativeLaunch, dev));
+            ctx->coop = v;
+        }
+        int bpc = ctx->num_sms / ctx->n_chains;
+        if (bpc > ctx->L) bpc = ctx->L;
+        const int rpb = (ctx->L + bpc - 1) / bpc;
+        bpc = (ctx->L + rpb - 1) / rpb;
+        const int W = ctx->L / 4;
+        const size_t smem = ((size_t)2 * rpb * W + 2 * (size_t)W) * sizeof(uint32_t);   // two band layers, two halo rows
+        const int n_bands = bpc * ctx->n_chains;
+        // worth it only while a half-step is short next to a launch (measured: 2.3x at 512^2, 1.2-1.4x at 1024^2, none at 2048^2)
+        const bool small_job = (double)ctx->n_chains * ctx->L * ctx->L <= 1.1e6;
+        if (ctx->coop && small_job && smem <= 160 * 1024) {
+            const size_t xrow = (size_t)2 * n_bands * W;                 // uint2 elements per exchange array
+            const size_t need = 2 * xrow * sizeof(uint2);
+            if (ctx->xch_bytes < need) {
+                cudaFree(ctx->d_xch);
+                ctx->d_xch = nullptr;
+                ctx->xch_bytes = 0;
+                if (cudaMalloc(&ctx->d_xch, need) != cudaSuccess) {
+                    cudaGetLastError();
+                    return fail(ctx, SHAKEN_ENOMEM, "cudaMalloc of %zu exchange bytes failed", need);
+                }
+                ctx->xch_bytes = need;
+                ctx->xch_stamp = 0xFFFFFFFFu;                            // forces the clearing below
+            }
+            // stamps must be new to the buffer: clear it when the 32-bit stamp space would wrap (or after allocation)
+            if ((uint64_t)ctx->xch_stamp + 2ull * (uint64_t)n_steps + 2ull >= 0xFFFFFFFFull) {
+                if ((uint64_t)n_steps >= 0x7FFFFFF0ull) return fail(ctx, SHAKEN_EINVAL, "shaken_run: n_steps too large for one call");
+                CU(cudaMemsetAsync(ctx->d_xch, 0, ctx->xch_bytes, ctx->stream));
+                ctx->xch_stamp = 0;
+            }
+            BandParams bp;
+            memset(&bp, 0, sizeof(bp));
+            bp.sigma = (uint8_t *)ctx->d_sigma;
+            bp.tau = (uint8_t *)ctx->d_tau;
+            bp.L = ctx->L;
+            bp.n_chains = ctx->n_chains;
+            bp.chain0 = ctx->chain0;
+            bp.t0 = ctx->step;
+            bp.n_steps = n_steps;
+            bp.obs_every = obs_every;
+            bp.rec = ctx->d_rec ? ctx->d_rec + (size_t)ctx->n_rec * ctx->n_chains * SHAKEN_N_OBS : nullptr;
+            bp.gtab = p.gtab;
+            memcpy(bp.utab, p.utab, sizeof(bp.utab));
+            make_step_keys(ctx->seed, 0, bp.keys);
+            bp.bpc = bpc;
+            bp.rows_per_band = rpb;
+            bp.xs = ctx->d_xch;
+            bp.xt = ctx->d_xch + xrow;
+            bp.stamp0 = ctx->xch_stamp;
+            bp.magicW = (uint32_t)(4294967296ull / (uint64_t)W) + 1u;
+            bp.magicV = (uint32_t)(4294967296ull / (uint64_t)(W / 4)) + 1u;
+            ctx->xch_stamp += (uint32_t)(2 * n_steps);
+            CU(cudaFuncSetAttribute(band_run_i8, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            void *args[] = {&bp};
+            CU(cudaLaunchCooperativeKernel((const void *)band_run_i8, dim3(n_bands), dim3(BAND_THREADS), args, smem, ctx->stream));
+            ctx->launches++;
+            ctx->step += (uint64_t)n_steps;
+            ctx->n_rec += n_new;
+            return SHAKEN_OK;
+        }
     }
 
     const long long blocks_needed = p.ntasks;
