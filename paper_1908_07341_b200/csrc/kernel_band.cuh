@@ -1,13 +1,13 @@
-// kernel_band.cuh -- mid-size lattices (128 < L <= 1024, few chains): a half-step is a microsecond of work, so one
+// kernel_band.cuh -- mid-size lattices (128 < L <= 2048, few chains): a half-step is a microsecond of work, so one
 // launch per half-step is mostly launch latency (cfg 2: 4.9 us per launch for 0.8 us of arithmetic).  Here the whole
 // run is ONE cooperative launch.  Every CTA owns a band of rows of one chain and keeps both sublattices of the band in
 // shared memory; per half-step it needs exactly one row from a neighbouring band (eq. (14): the field
 // uses the down row in half 0, the up row in half 1), which the neighbour publishes through a small global buffer in
 // "data + stamp" form: every 8-byte store carries the spin word and the half-step stamp, so a reader that sees the
-// stamp has the data (no fence, no separate flag).  A CTA computes the rows in walking order, so the row its neighbour
-// waits for is in the first trip and is published right after it; one warp collects the row the CTA itself needs
-// next at the end of the half-step.  There is no grid-wide barrier: only neighbouring bands wait for each other, which
-// is why all CTAs must be co-resident -- the cooperative launch guarantees it.
+// stamp has the data (no fence, no separate flag).  A CTA computes its rows in walking order, so the row its neighbour
+// waits for is in the first trip, and each of its vectors is published by the thread that computed it; one warp does
+// no arithmetic and polls for the row the CTA itself needs next.  There is no grid-wide barrier: only neighbouring
+// bands wait for each other, which is why all CTAs must be co-resident -- the cooperative launch guarantees it.
 // Site -> random word mapping, thresholds and rule are those of kernel_i8.cuh; only the schedule differs.
 #pragma once
 #include "kernels_common.cuh"
@@ -62,7 +62,8 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) band_run_i8(const __grid_cons
     const int ncalls = nr * W;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t lane8 = (uint32_t)lane * 8u;
-    const bool duty_warp = warp == BAND_THREADS / 32 - 1;   // polls for the neighbour's row while the other warps compute
+    const bool duty_warp = warp == BAND_THREADS / 32 - 1;
+    constexpr int WORKERS = BAND_THREADS - 32;   // polls for the neighbour's row while the other warps compute
 
     uint32_t *sg = smem;                          // sigma band [nr][W]
     uint32_t *ta = smem + p.rows_per_band * W;    // tau band
@@ -113,7 +114,7 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) band_run_i8(const __grid_cons
     // half 0: tau from sigma, rows ascending.  half 1: sigma from tau, rows walked from the last one down.
     // `half` is a run-time value on purpose: one copy of this code serves both half-steps and every trip.
     const int nvec = W >> 2, nvecs = nr * nvec;   // vectors per row, per band
-    auto update_vector = [&](const int half, const int c) {
+    auto update_vector = [&](const int half, const int c, uint2 *xmine, const uint32_t stamp) {
         const uint32_t *src = half ? ta : sg;
         uint32_t *dst = half ? sg : ta;
         const uint32_t *halo = half ? ht : hs;
@@ -135,6 +136,14 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) band_run_i8(const __grid_cons
             o[j] = update_word(w[j], half ? hr : hl, vw[j], n + (uint32_t)j);
         }
         *reinterpret_cast<uint4 *>(dst + at) = make_uint4(o[0], o[1], o[2], o[3]);
+        // the first row in walking order (first tau row in half 0, last sigma row in half 1) is the one the neighbouring
+        // band waits for: it leaves at once, straight from the thread that computed it ({word, stamp} pairs, 16 bytes
+        // per store), with no barrier on the critical path of the ring
+        if (rr == 0) {
+            uint4 *x = reinterpret_cast<uint4 *>(xmine + 4 * cv);
+            __stcg(x, make_uint4(o[0], stamp, o[1], stamp));
+            __stcg(x + 1, make_uint4(o[2], stamp, o[3], stamp));
+        }
     };
 
     // block-wide sums of up to six int partials into one record (int64 atomics: bands of a chain share the record)
@@ -171,22 +180,20 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) band_run_i8(const __grid_cons
     // fly while the band is computed.  collect (duty warp, after the arithmetic): words whose stamp is not there yet
     // are polled from L2 one round trip at a time.
     auto collect = [&](const uint2 *src, const uint32_t stamp, uint32_t *dst) {
-        for (int i0 = 0; i0 < W; i0 += 256) {     // W <= 512: up to 8 words per lane, re-read together until all are stamped
+        // W <= 512: at most two rounds of 8 words per lane.  The loads are unconditional (indices past the row are
+        // clamped to its last word) and all eight are in flight together; a round is repeated until every word carries
+        // the stamp.  (A version with predicated loads compiled into a loop that was 3.7x slower.)
+        for (int i0 = 0; i0 < W; i0 += 256) {
             uint2 v[8];
-            bool ok = false;
-            while (!ok) {
+            bool ok;
+            do {
                 ok = true;
 #pragma unroll
-                for (int j = 0; j < 8; ++j) {
-                    const int i = i0 + j * 32 + lane;
-                    if (i < W) v[j] = ld_relaxed_v2(src + i);
-                }
+                for (int j = 0; j < 8; ++j) v[j] = ld_relaxed_v2(src + min(i0 + j * 32 + lane, W - 1));
 #pragma unroll
-                for (int j = 0; j < 8; ++j) {
-                    const int i = i0 + j * 32 + lane;
-                    if (i < W && v[j].y != stamp) ok = false;
-                }
-            }
+                for (int j = 0; j < 8; ++j)
+                    if (v[j].y != stamp) ok = false;
+            } while (!ok);
 #pragma unroll
             for (int j = 0; j < 8; ++j) {
                 const int i = i0 + j * 32 + lane;
@@ -214,16 +221,12 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) band_run_i8(const __grid_cons
         const uint32_t stamp = p.stamp0 + (uint32_t)(h + 1);
         uint2 *xmine = (half ? p.xs : p.xt) + ((size_t)par * nb + band) * W;
         const uint2 *xnbr = (half ? p.xs : p.xt) + ((size_t)par * nb + (half ? down : up)) * W;
-        // first trip: the first 512 vectors in walking order, which include the row the neighbour waits for
-        if (tid < nvecs) update_vector(half, tid);
-        __syncthreads();
-        {
-            const uint32_t *row = half ? sg + (nr - 1) * W : ta;
-            for (int i = tid; i < W; i += BAND_THREADS) __stcg(xmine + i, make_uint2(row[i], stamp));
-        }
-#pragma unroll 1
-        for (int c = tid + BAND_THREADS; c < nvecs; c += BAND_THREADS) update_vector(half, c);
+        // The last warp does no arithmetic: it polls for the neighbour's row from the start of the half-step, so the
+        // handshake (one L2 round trip after the neighbour's first vectors are done) hides behind the other 15 warps.
         if (duty_warp) collect(xnbr, stamp, half ? hs : ht);
+        else
+#pragma unroll 1
+            for (int c = tid; c < nvecs; c += WORKERS) update_vector(half, c, xmine, stamp);
         __syncthreads();
 
         // record (M_sigma, M_tau, E_J, E_q now; C_x, C_y at the start of the next half-step 0)

@@ -489,8 +489,9 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
         const int W = ctx->L / 4;
         const size_t smem = ((size_t)2 * rpb * W + 2 * (size_t)W) * sizeof(uint32_t);   // two band layers, two halo rows
         const int n_bands = bpc * ctx->n_chains;
-        // worth it only while a half-step is short next to a launch (measured: 2.3x at 512^2, 1.2-1.4x at 1024^2, none at 2048^2)
-        const bool small_job = (double)ctx->n_chains * ctx->L * ctx->L <= 1.1e6;
+        // worth it while a half-step is short next to a launch; measured against the strip kernels: 3.6x at 512^2, 2.5x at
+        // 1024^2, 2.2x at 2048^2 (the largest band that fits shared memory)
+        const bool small_job = (double)ctx->n_chains * ctx->L * ctx->L <= 4.5e6;
         if (ctx->coop && small_job && smem <= 160 * 1024) {
             const size_t xrow = (size_t)2 * n_bands * W;                 // uint2 elements per exchange array
             const size_t need = 2 * xrow * sizeof(uint2);
