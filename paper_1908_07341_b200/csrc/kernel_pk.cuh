@@ -3,45 +3,52 @@
 //
 // The acceptance needs a 32-bit compare per SITE, so packing saves memory traffic (0.25 B per update), not
 // integer work.  The per-site table index is formed 4 sites at a time in byte-SIMD registers:
-//   Y[k]  = 4 * (bits k, 8+k, 16+k, 24+k of the word)                       (k = 0..7: one shift + one AND)
-//   C[k]  = Y[k] + 2 * (Yv[k] + Yh[k])  = 4 * (c + 2 (v + h)) = 4 * (2 k_plus + c)  per byte,
+//   Y[k]  = 2 * (bits k, 8+k, 16+k, 24+k of the word)                       (k = 0..7: one shift + one AND)
+//   C[k]  = Y[k] + 2 * (Yv[k] + Yh[k])  = 2 * (c + 2 (v + h)) = 2 * (2 k_plus + c) = 2 idx   per byte,
 // where Yv is the previous row's Y (kept in registers) and Yh[k] = Y[k-1] (left, half 0) or Y[k+1] (right,
 // half 1): in this strided grouping the horizontal neighbour of site 8m+k sits in the SAME byte m of the
 // adjacent group, so only k = 0 (k = 7) needs a byte funnel shift and one bit of the neighbouring word.
-// Byte m of C[k] is the byte offset of T[2k+c] for site 8m+k; the eight C words go through a per-thread
-// shared-memory slot and come back one byte at a time (LDS.U8), exactly as in the int8 kernel.
+// Two sites share one lookup: P[j] = C[2j] + 8 C[2j+1] holds in byte m the pair code 2 (idx_a + 8 idx_b) of the
+// consecutive sites a = 8m+2j, b = a+1 (both of the same Philox call), one IDP.4A turns that byte into the byte
+// offset 256 (idx_a + 8 idx_b) + 8 lane, and one LDS.64 fetches {T[idx_a], T[idx_b]} from a lane-replicated table
+// (46 entries x 256 B; lane l always reads banks 2l, 2l+1: conflict-free for any mix of indices).
+// Accepted sites are added into the output word with a predicated IADD (half the ALU-port cost of a LOP3).
 // Observables are population counts of XORed words.
 #pragma once
 #include "kernels_common.cuh"
 
 namespace shaken {
 
-__device__ __forceinline__ void spread4(uint32_t W, uint32_t Y4[8])
+constexpr int PK_THREADS = 512;     // one 512-thread block per SM, up to 128 registers per thread
+constexpr int PK_PAIR_ENTRIES = 46; // idx_a + 8 idx_b, idx in 0..5
+
+__device__ __forceinline__ void spread2(uint32_t W, uint32_t Y2[8])
 {
 #pragma unroll
-    for (int k = 0; k < 8; ++k) Y4[k] = (k <= 2 ? (W << (2 - k)) : (W >> (k - 2))) & 0x04040404u;
+    for (int k = 0; k < 8; ++k) Y2[k] = (k == 0 ? (W << 1) : (W >> (k - 1))) & 0x02020202u;
 }
 
 template <int HALF, int FLAGS>
-__global__ void __launch_bounds__(BLOCK_THREADS, 2) half_step_pk(const __grid_constant__ StepParams p)
+__global__ void __launch_bounds__(PK_THREADS, 1) half_step_pk(const __grid_constant__ StepParams p)
 {
     constexpr bool OBS = (FLAGS & F_OBS) != 0;
     constexpr bool BONDS = (FLAGS & F_BONDS) != 0;
     constexpr bool UPDATE = (FLAGS & F_NOUPDATE) == 0;
+    constexpr int WPB = PK_THREADS / 32;
     static_assert(!(BONDS && HALF == 1), "bond sums ride on half-step 0");
 
-    __shared__ uint32_t s_tab[8];                       // T[2k + c], natural order
-    __shared__ uint32_t s_idx[8][BLOCK_THREADS];        // per-thread staging of the eight C words
+    __shared__ uint2 s_pair[PK_PAIR_ENTRIES][32];
 
     const int lane = threadIdx.x & 31;
     const int warp = threadIdx.x >> 5;
+    const uint32_t lane8 = (uint32_t)lane * 8u;
     const int L = p.L;
     const int L4 = L >> 2;
     const int W = p.nvec;                               // words per row
     const int R = p.rows_per_task;
     const size_t plane = (size_t)L * (size_t)W;
     const int tpc = p.nrb * p.nseg;
-    const int bpc = (tpc + WARPS_PER_BLOCK - 1) / WARPS_PER_BLOCK;
+    const int bpc = (tpc + WPB - 1) / WPB;
 
     int cur_chain = -1;
     ChainKeys ck = {0u, 0u};
@@ -66,14 +73,21 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 2) half_step_pk(const __grid_co
 
     for (long long bt = blockIdx.x; bt < p.ntasks; bt += gridDim.x) {
         const int chain = (int)(bt / bpc);
-        const int lt = (int)(bt % bpc) * WARPS_PER_BLOCK + warp;
+        const int lt = (int)(bt % bpc) * WPB + warp;
         if (chain != cur_chain) {                                    // block-uniform
             if ((OBS || BONDS) && cur_chain >= 0) flush(cur_chain);
             cur_chain = chain;
             if (UPDATE) {
                 ck = make_chain_keys(p.keys, p.chain0 + (uint32_t)chain);
                 __syncthreads();
-                if (threadIdx.x < 8) s_tab[threadIdx.x] = p.gtab ? p.gtab[(size_t)chain * 8 + threadIdx.x] : p.utab[threadIdx.x];
+                for (int t = threadIdx.x; t < PK_PAIR_ENTRIES * 32; t += PK_THREADS) {
+                    const int e = t >> 5, ia = e & 7, ib = e >> 3;
+                    if (ia < 6 && ib < 6) {
+                        const uint32_t Ta = p.gtab ? p.gtab[(size_t)chain * 8 + ia] : p.utab[ia];
+                        const uint32_t Tb = p.gtab ? p.gtab[(size_t)chain * 8 + ib] : p.utab[ib];
+                        s_pair[e][t & 31] = make_uint2(Ta, Tb);
+                    }
+                }
                 __syncthreads();
             }
         }
@@ -98,46 +112,48 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 2) half_step_pk(const __grid_co
             uint32_t *pd = dbase + (size_t)r0 * W + cv;
             uint32_t n = (uint32_t)r0 * (uint32_t)L4 + (uint32_t)cv * 8u;
             const uint32_t nstep = (uint32_t)(dir * L4);
-            uint32_t *const my_idx = &s_idx[0][threadIdx.x];
 
+            // the row in use, and the next two already on their way (prefetch distance 2)
             uint32_t V = __ldg(sbase + (size_t)rh * W + cv);
-            uint32_t S = __ldg(pc);
-            uint32_t e = __ldg(pe);
+            uint32_t S0 = __ldg(pc), E0 = __ldg(pe), S1 = S0, E1 = E0, S2 = S0, E2 = E0;
+            if (rows > 1) { S1 = __ldg(pc + stride); E1 = __ldg(pe + stride); }
             uint32_t Yv[8];
-            if (UPDATE) spread4(V, Yv);
+            if (UPDATE) spread2(V, Yv);
             int a0 = 0, a1 = 0, a2 = 0;     // popcount partials of this task
 
             for (int i = 0; i < rows; ++i) {
-                uint32_t Sn = S, en = e;
-                if (i + 1 < rows) {
-                    Sn = __ldg(pc + stride);
-                    en = __ldg(pe + stride);
+                if (i + 2 < rows) {
+                    S2 = __ldg(pc + 2 * stride);
+                    E2 = __ldg(pe + 2 * stride);
                 }
+                const uint32_t S = S0, e = E0;
                 // horizontal neighbour plane: left (half 0) or right (half 1)
                 const uint32_t Hp = HALF == 0 ? ((S << 1) | (e >> 31)) : ((S >> 1) | (e << 31));
                 uint32_t out = 0;
                 if (UPDATE) {
-                    uint32_t Y[8];
-                    spread4(S, Y);
+                    uint32_t Y[8], C[8], P[4];
+                    spread2(S, Y);
 #pragma unroll
                     for (int k = 0; k < 8; ++k) {
                         uint32_t H;
-                        if (HALF == 0) H = k >= 1 ? Y[k - 1] : ((Y[7] << 8) | ((e >> 31) << 2));
-                        else           H = k <= 6 ? Y[k + 1] : ((Y[0] >> 8) | ((e & 1u) << 26));
-                        const uint32_t C = Y[k] + 2u * (Yv[k] + H);
-                        *reinterpret_cast<volatile uint32_t *>(my_idx + k * BLOCK_THREADS) = C;
+                        if (HALF == 0) H = k >= 1 ? Y[k - 1] : ((Y[7] << 8) | ((e >> 31) << 1));
+                        else           H = k <= 6 ? Y[k + 1] : ((Y[0] >> 8) | ((e & 1u) << 25));
+                        C[k] = Y[k] + 2u * (Yv[k] + H);
                     }
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) P[j] = C[2 * j] + 8u * C[2 * j + 1];
 #pragma unroll
                     for (int q = 0; q < 8; ++q) {
                         uint32_t rw[4];
                         philox_site_words(n + (uint32_t)q, p.keys, ck, rw);
-#pragma unroll
-                        for (int b = 0; b < 4; ++b) {
-                            const int site = 4 * q + b, m = site >> 3, k = site & 7;
-                            const uint32_t code = reinterpret_cast<volatile const uint8_t *>(my_idx + k * BLOCK_THREADS)[m];
-                            const uint32_t T = *reinterpret_cast<const uint32_t *>(reinterpret_cast<const char *>(s_tab) + code);
-                            out = xor_if_less(out, rw[b], T, 1u << site);
-                        }
+                        const int m = q >> 1, j0 = (q & 1) * 2;
+                        const uint32_t o01 = __dp4a(P[j0], 0x80u << (8 * m), lane8), o23 = __dp4a(P[j0 + 1], 0x80u << (8 * m), lane8);
+                        const uint2 t01 = *reinterpret_cast<const uint2 *>(reinterpret_cast<const char *>(s_pair) + o01);
+                        const uint2 t23 = *reinterpret_cast<const uint2 *>(reinterpret_cast<const char *>(s_pair) + o23);
+                        out = add_if_less(out, rw[0], t01.x, 1u << (4 * q));
+                        out = add_if_less(out, rw[1], t01.y, 2u << (4 * q));
+                        out = add_if_less(out, rw[2], t23.x, 4u << (4 * q));
+                        out = add_if_less(out, rw[3], t23.y, 8u << (4 * q));
                     }
                     *pd = out;
 #pragma unroll
@@ -156,7 +172,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 2) half_step_pk(const __grid_co
                         a2 += __popc(S ^ V);
                     }
                 }
-                V = S; S = Sn; e = en;
+                V = S; S0 = S1; E0 = E1; S1 = S2; E1 = E2;
                 pc += stride; pe += stride; pd += stride;
                 n += nstep;
             }

@@ -62,6 +62,13 @@ __device__ __forceinline__ uint32_t xor_if_less(uint32_t out, uint32_t a, uint32
     return out;
 }
 
+// out += c if a < b (unsigned): one ISETP and one predicated add
+__device__ __forceinline__ uint32_t add_if_less(uint32_t out, uint32_t a, uint32_t b, uint32_t c)
+{
+    asm("{\n\t.reg .pred p;\n\tsetp.lo.u32 p, %1, %2;\n\t@p add.u32 %0, %0, %3;\n\t}" : "+r"(out) : "r"(a), "r"(b), "r"(c));
+    return out;
+}
+
 // out += c if !(a < b) (unsigned): one ISETP and one predicated add (IADD3 costs about half a LOP3 on the ALU port)
 __device__ __forceinline__ uint32_t add_if_not_less(uint32_t out, uint32_t a, uint32_t b, uint32_t c)
 {

@@ -357,7 +357,7 @@ static cudaError_t launch_half(const shaken_ctx *ctx, const StepParams &p, int g
     // half-steps use the paired lookup (one IDP.4A + one LDS.64 per two sites).
     constexpr int TUNED = PACK_ADD | PREFETCH2;
     constexpr int AUTO = ((FLAGS & (F_OBS | F_BONDS)) ? EXTRACT_SMEM : EXTRACT_PAIR) | TUNED;
-    if (ctx->packed) half_step_pk<HALF, FLAGS><<<grid, BLOCK_THREADS, 0, ctx->stream>>>(p);
+    if (ctx->packed) half_step_pk<HALF, FLAGS><<<grid, PK_THREADS, 0, ctx->stream>>>(p);
     else switch (ctx->variant) {
         case 1: half_step_i8<HALF, FLAGS, EXTRACT_PRMT | TUNED, 1, I8_THREADS><<<grid, I8_THREADS, 0, ctx->stream>>>(p); break;
         case 2: half_step_i8<HALF, FLAGS, EXTRACT_SMEM, 2><<<grid, BLOCK_THREADS, 0, ctx->stream>>>(p); break;   // round-1 v2 kernel
@@ -423,7 +423,8 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
     p.chain0 = ctx->chain0;
     p.nseg = (p.nvec + 31) / 32;
     int resident = 2, wpb = WARPS_PER_BLOCK;                  // resident blocks per SM (launch bounds), warps per block
-    if (!ctx->packed && ctx->variant != 2 && ctx->variant != 7) { resident = 1; wpb = I8_THREADS / 32; }
+    if (ctx->packed) { resident = 1; wpb = PK_THREADS / 32; }
+    else if (ctx->variant != 2 && ctx->variant != 7) { resident = 1; wpb = I8_THREADS / 32; }
     const long long cap = (long long)ctx->num_sms * resident;
     p.rows_per_task = choose_rows_per_task(ctx, p.nseg, cap, wpb);
     p.nrb = (ctx->L + p.rows_per_task - 1) / p.rows_per_task;
