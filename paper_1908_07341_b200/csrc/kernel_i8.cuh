@@ -21,7 +21,7 @@
 
 namespace shaken {
 
-enum : int { EXTRACT_PRMT = 0, EXTRACT_SMEM = 1, EXTRACT_IDP = 2, EXTRACT_PAIR = 3, PACK_ADD = 16, PREFETCH2 = 32 };
+enum : int { EXTRACT_PRMT = 0, EXTRACT_SMEM = 1, EXTRACT_IDP = 2, EXTRACT_PAIR = 3, PACK_ADD = 16, PREFETCH2 = 32, PER_WARP = 64 };
 
 // byte the EXTRACT_SMEM encoding produces for minus flags (ms, mh, mv)
 __host__ __device__ constexpr uint32_t smem_code(int ms, int mh, int mv)
@@ -36,12 +36,17 @@ __global__ void __launch_bounds__(THREADS, MINB) half_step_i8(const __grid_const
     constexpr int EXTRACT = EXTRACT_ & 15;
     constexpr bool PACKADD = (EXTRACT_ & PACK_ADD) != 0;
     constexpr int AHEAD = (EXTRACT_ & PREFETCH2) ? 2 : 1;   // rows between a load and its first use
+    // PER_WARP: a task is ONE warp strip and every warp walks its own task list with its own threshold table, so warps
+    // of a block may work on different chains and never wait for each other (many small chains: the strips can be
+    // tall and the last wave full at warp granularity).  Otherwise a task is WPB strips of one chain per block.
+    constexpr bool PERWARP = (EXTRACT_ & PER_WARP) != 0;
+    static_assert(!PERWARP || EXTRACT != EXTRACT_PAIR, "the paired table (16 KiB) exists once per block");
     constexpr bool OBS = (FLAGS & F_OBS) != 0;
     constexpr bool BONDS = (FLAGS & F_BONDS) != 0;
     constexpr bool UPDATE = (FLAGS & F_NOUPDATE) == 0;
     static_assert(!(BONDS && HALF == 1), "bond sums ride on half-step 0");
 
-    __shared__ uint32_t s_tab[64];
+    __shared__ uint32_t s_tabs[PERWARP ? WPB : 1][64];
     __shared__ uint32_t s_idx[EXTRACT == EXTRACT_SMEM ? 4 : 1][THREADS];
     // EXTRACT_PAIR: thresholds of TWO sites per lookup.  Entry e = c_even + 8 c_odd (c = m_self + 2 m_horizontal +
     // 4 m_vertical) holds {T(c_even), T(c_odd)}, replicated per lane: lane l reads 8 bytes at e * 256 + l * 8, i.e.
@@ -50,6 +55,7 @@ __global__ void __launch_bounds__(THREADS, MINB) half_step_i8(const __grid_const
 
     const int lane = threadIdx.x & 31;
     const int warp = threadIdx.x >> 5;
+    uint32_t *const s_tab = s_tabs[PERWARP ? warp : 0];
     const int L = p.L;
     const int L4 = L >> 2;
     const int R = p.rows_per_task;
@@ -78,10 +84,26 @@ __global__ void __launch_bounds__(THREADS, MINB) half_step_i8(const __grid_const
         cnt0 = cnt1 = cnt2 = 0;
     };
 
-    for (long long bt = blockIdx.x; bt < p.ntasks; bt += gridDim.x) {
-        const int chain = (int)(bt / bpc);
-        const int lt = (int)(bt % bpc) * WPB + warp;     // this warp's task inside the chain
-        if (chain != cur_chain) {                                    // block-uniform
+    const long long task0 = PERWARP ? (long long)blockIdx.x * WPB + warp : (long long)blockIdx.x;
+    const long long task_step = PERWARP ? (long long)gridDim.x * WPB : (long long)gridDim.x;
+    for (long long bt = task0; bt < p.ntasks; bt += task_step) {
+        const int chain = (int)(bt / (PERWARP ? tpc : bpc));
+        const int lt = PERWARP ? (int)(bt % tpc) : (int)(bt % bpc) * WPB + warp;   // this warp's task inside the chain
+        if (PERWARP && chain != cur_chain) {                          // warp-uniform
+            if ((OBS || BONDS) && cur_chain >= 0) flush(cur_chain);
+            cur_chain = chain;
+            if (UPDATE) {
+                ck = make_chain_keys(p.keys, p.chain0 + (uint32_t)chain);
+                __syncwarp();
+                if (lane < 8) {
+                    const int ms = lane & 1, mh = (lane >> 1) & 1, mv = lane >> 2;
+                    const int idx = 2 * (2 - mh - mv) + (1 - ms);              // T[2k + c]
+                    s_tab[smem_code(ms, mh, mv) >> 2] = p.gtab ? p.gtab[(size_t)chain * 8 + idx] : p.utab[idx];
+                }
+                __syncwarp();
+            }
+        }
+        if (!PERWARP && chain != cur_chain) {                         // block-uniform
             if ((OBS || BONDS) && cur_chain >= 0) flush(cur_chain);
             cur_chain = chain;
             if (UPDATE) {

@@ -49,6 +49,7 @@ struct shaken_ctx {
     bool have_spins = false;
     int num_sms = 0;
     int variant = 0;
+    bool perwarp = false;         // strip kernels: per-warp task lists for this run (many small chains)
     int64_t launches = 0;
     char err[512] = {0};
 };
@@ -365,17 +366,21 @@ static cudaError_t launch_half(const shaken_ctx *ctx, const StepParams &p, int g
         case 5: half_step_i8<HALF, FLAGS, EXTRACT_PAIR | TUNED, 1, I8_THREADS><<<grid, I8_THREADS, 0, ctx->stream>>>(p); break;
         case 6: half_step_i8<HALF, FLAGS, EXTRACT_IDP | TUNED, 1, I8_THREADS><<<grid, I8_THREADS, 0, ctx->stream>>>(p); break;
         case 7: half_step_i8<HALF, FLAGS, AUTO, 2><<<grid, BLOCK_THREADS, 0, ctx->stream>>>(p); break;          // 2 x 256 threads
-        default: half_step_i8<HALF, FLAGS, AUTO, 1, I8_THREADS><<<grid, I8_THREADS, 0, ctx->stream>>>(p); break;
+        case 8: half_step_i8<HALF, FLAGS, EXTRACT_SMEM | TUNED | PER_WARP, 1, I8_THREADS><<<grid, I8_THREADS, 0, ctx->stream>>>(p); break;
+        default:
+            if (ctx->perwarp) half_step_i8<HALF, FLAGS, EXTRACT_SMEM | TUNED | PER_WARP, 1, I8_THREADS><<<grid, I8_THREADS, 0, ctx->stream>>>(p);
+            else half_step_i8<HALF, FLAGS, AUTO, 1, I8_THREADS><<<grid, I8_THREADS, 0, ctx->stream>>>(p);
+            break;
     }
     return cudaGetLastError();
 }
 
-static int choose_rows_per_task(const shaken_ctx *ctx, int nseg, long long grid_cap, int wpb)
+static int choose_rows_per_task(const shaken_ctx *ctx, int nseg, long long grid_cap, int wpb, double *score_out = nullptr)
 {
     // Strip height R.  Tall strips amortise the halo row and the unprefetched loads at a strip's start; the persistent
     // grid walks block tasks (8 warp strips of one chain) round-robin, so the last wave should be full and so should
-    // the 8 warps of a block task.  Maximise
-    //     fill * warp_use * machine * R / (R + 1.5)
+    // the warps of a block task.  Maximise
+    //     fill * warp_use * machine * R / (R + 3)      (halo row + the unprefetched first rows of a strip)
     // fill = ntasks / (grid * waves), warp_use = strips per chain / (8 * block tasks per chain), machine = grid / cap.
     int best = 4;
     double best_score = -1.0;
@@ -390,9 +395,10 @@ static int choose_rows_per_task(const shaken_ctx *ctx, int nseg, long long grid_
         const double fill = (double)ntasks / (double)(grid * waves);
         const double warp_use = (double)ctx->L / (double)(nrb * R) * (double)tpc / (double)(bpc * wpb);
         const double machine = (double)grid / (double)grid_cap;
-        const double score = fill * warp_use * machine * ((double)R / ((double)R + 1.5));
+        const double score = fill * warp_use * machine * ((double)R / ((double)R + 3.0));
         if (score > best_score + 1e-9) { best_score = score; best = R; }
     }
+    if (score_out) *score_out = best_score;
     return best;
 }
 
@@ -426,7 +432,21 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
     if (ctx->packed) { resident = 1; wpb = PK_THREADS / 32; }
     else if (ctx->variant != 2 && ctx->variant != 7) { resident = 1; wpb = I8_THREADS / 32; }
     const long long cap = (long long)ctx->num_sms * resident;
-    p.rows_per_task = choose_rows_per_task(ctx, p.nseg, cap, wpb);
+    double score_block = 0.0;
+    p.rows_per_task = choose_rows_per_task(ctx, p.nseg, cap, wpb, &score_block);
+    // many small chains: per-warp task lists (kernel_i8.cuh PER_WARP) balance at warp granularity with tall strips;
+    // they cannot use the paired lookup, which is worth ~5 % on launches without fused sums
+    ctx->perwarp = false;
+    if (!ctx->packed && (ctx->variant == 8 || (ctx->variant == 0 && ctx->n_chains > 1))) {
+        double score_pw = 0.0;
+        const int Rpw = choose_rows_per_task(ctx, p.nseg, cap * wpb, 1, &score_pw);
+        const bool mostly_plain = obs_every == 0 || obs_every > 4;
+        if (ctx->variant == 8 || score_pw * (mostly_plain ? 0.95 : 1.0) > score_block + 0.02) {
+            ctx->perwarp = true;
+            p.rows_per_task = Rpw;
+            wpb = 1;                                       // p.ntasks counts warp strips
+        }
+    }
     p.nrb = (ctx->L + p.rows_per_task - 1) / p.rows_per_task;
     // block tasks: WARPS_PER_BLOCK consecutive warp strips of one chain
     p.ntasks = (long long)ctx->n_chains * (((long long)p.nrb * p.nseg + wpb - 1) / wpb);
@@ -545,7 +565,7 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
         }
     }
 
-    const long long blocks_needed = p.ntasks;
+    const long long blocks_needed = ctx->perwarp ? (p.ntasks + I8_THREADS / 32 - 1) / (I8_THREADS / 32) : p.ntasks;
     const int grid = (int)(blocks_needed < cap ? blocks_needed : cap);
     const size_t rec_stride = (size_t)ctx->n_chains * SHAKEN_N_OBS;
 
