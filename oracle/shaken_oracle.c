@@ -30,7 +30,8 @@
  * random word), J=0 closed-form contraction tanh(q), exact 2^9-state
  * transition matrix on the 3x3 torus built from eq. (15)-(16), detailed
  * balance w.r.t. pi_s = Z_sigma/Z, the two forms of eq. (5),
- * monotone coupling, observables by brute force.
+ * monotone coupling, observables by brute force; coupling groups and coalescence times
+ * against pairs of uncoupled single-chain runs and the J = 0 closed form.
  * The site->counter mapping itself is a convention: parity unpinned beyond
  * self-consistency (by design).
  */
@@ -132,6 +133,10 @@ typedef struct oracle_ctx {
     int64_t n_records;
     int64_t cap_records;
     int complement;     /* test hook: replace every random word r by 2^32-1-r */
+    int64_t group;      /* coupling: chains c with equal c / group evolve "with the same update function and the same
+                         * sequence of random numbers": all draw the words of chain (c / group) * group */
+    int64_t *coal;      /* [n_chains / group] coalescence time T = min{n : X_n = Y_n} in full steps,
+                         * -1 while the sigma layers of the group still differ */
 } oracle_ctx;
 
 enum { ORACLE_OK = 0, ORACLE_EINVAL = -1, ORACLE_ENOMEM = -2 };
@@ -148,20 +153,48 @@ int oracle_create(oracle_ctx **out, int64_t L, int64_t n_chains, uint64_t seed)
     if (!o->sigma || !o->tau) { free(o->sigma); free(o->tau); free(o); return ORACLE_ENOMEM; }
     memset(o->sigma, 1, n);
     memset(o->tau, 1, n);
+    o->group = 1;
     *out = o;
     return ORACLE_OK;
+}
+
+/* Coupled chains.  group >= 1 must divide n_chains; group = 1 uncouples.  Forgets coalescence times. */
+int oracle_set_coupling(oracle_ctx *o, int64_t group)
+{
+    if (!o || group < 1 || o->n_chains % group != 0) return ORACLE_EINVAL;
+    free(o->coal);
+    o->coal = NULL;
+    o->group = group;
+    if (group > 1) {
+        int64_t ng = o->n_chains / group;
+        o->coal = (int64_t *)malloc((size_t)ng * sizeof(int64_t));
+        if (!o->coal) return ORACLE_ENOMEM;
+        for (int64_t i = 0; i < ng; ++i) o->coal[i] = -1;
+    }
+    return ORACLE_OK;
+}
+
+/* Coalescence times of the groups, -1 = not yet; returns the number of groups written (0 when uncoupled). */
+int64_t oracle_coalescence(const oracle_ctx *o, int64_t *out, int64_t max_groups)
+{
+    if (!o || max_groups < 0) return ORACLE_EINVAL;
+    if (o->group <= 1) return 0;
+    int64_t ng = o->n_chains / o->group, n = ng < max_groups ? ng : max_groups;
+    for (int64_t i = 0; i < n; ++i) out[i] = o->coal[i];
+    return n;
 }
 
 void oracle_destroy(oracle_ctx *o)
 {
     if (!o) return;
-    free(o->sigma); free(o->tau); free(o->records); free(o);
+    free(o->sigma); free(o->tau); free(o->records); free(o->coal); free(o);
 }
 
-/* mode +1: all +1; -1: all -1; 0: iid +-1 from the init stream (spin = +1 iff word < 2^31). */
+/* mode +1: all +1; -1: all -1; 0: iid +-1 from the init stream (spin = +1 iff word < 2^31);
+ * 2 ("sandwich"): the first chain of every coupling group all +1 (sigma^top), the others all -1 (sigma^bot). */
 int oracle_init(oracle_ctx *o, int mode)
 {
-    if (!o || (mode != 1 && mode != -1 && mode != 0)) return ORACLE_EINVAL;
+    if (!o || (mode != 1 && mode != -1 && mode != 0 && mode != 2)) return ORACLE_EINVAL;
     int64_t L = o->L;
     uint64_t nsite = (uint64_t)L * (uint64_t)L;
     for (int64_t ch = 0; ch < o->n_chains; ++ch)
@@ -170,6 +203,8 @@ int oracle_init(oracle_ctx *o, int mode)
             if (mode == 0) {
                 s = init_word(o->seed, (uint32_t)ch, 0u, x) < 0x80000000u ? 1 : -1;
                 t = init_word(o->seed, (uint32_t)ch, 1u, x) < 0x80000000u ? 1 : -1;
+            } else if (mode == 2) {
+                s = t = (int8_t)(ch % o->group == 0 ? 1 : -1);
             } else {
                 s = t = (int8_t)mode;
             }
@@ -178,6 +213,8 @@ int oracle_init(oracle_ctx *o, int mode)
         }
     o->step = 0;
     o->n_records = 0;
+    if (o->coal)
+        for (int64_t i = 0; i < o->n_chains / o->group; ++i) o->coal[i] = -1;
     return ORACLE_OK;
 }
 
@@ -275,10 +312,20 @@ int oracle_run_grid(oracle_ctx *o, const double *J, const double *q, int64_t n_s
     for (int64_t s = 0; s < n_steps; ++s) {
         for (int64_t ch = 0; ch < o->n_chains; ++ch) {
             int8_t *sg = o->sigma + (size_t)ch * nsite, *ta = o->tau + (size_t)ch * nsite;
-            half_step(o, ch, T + 6 * ch, 0, sg, ta, o->step);
-            half_step(o, ch, T + 6 * ch, 1, ta, sg, o->step);
+            int64_t rng_chain = (ch / o->group) * o->group;      /* the same random numbers within a group */
+            half_step(o, rng_chain, T + 6 * ch, 0, sg, ta, o->step);
+            half_step(o, rng_chain, T + 6 * ch, 1, ta, sg, o->step);
         }
         o->step++;
+        if (o->coal)                                             /* T = min{n : X_n = Y_n} on the sigma layer */
+            for (int64_t gi = 0; gi < o->n_chains / o->group; ++gi) {
+                if (o->coal[gi] >= 0) continue;
+                const int8_t *first = o->sigma + (size_t)(gi * o->group) * nsite;
+                int same = 1;
+                for (int64_t m = 1; m < o->group && same; ++m)
+                    same = memcmp(first, first + (size_t)m * nsite, nsite) == 0;
+                if (same) o->coal[gi] = (int64_t)o->step;
+            }
         if (obs_every > 0 && o->step % (uint64_t)obs_every == 0) {
             int rc = push_record(o);
             if (rc) { free(T); return rc; }

@@ -80,6 +80,10 @@ def lib():
         L.oracle_half_step_rows.argtypes = [p, p, C.c_int64, C.c_uint64, C.c_int64, C.c_double, C.c_double,
                                             C.c_uint64, C.c_int, C.c_int64, C.c_int64]
         L.oracle_half_step_rows.restype = C.c_int
+        L.oracle_set_coupling.argtypes = [p, C.c_int64]
+        L.oracle_set_coupling.restype = C.c_int
+        L.oracle_coalescence.argtypes = [p, C.POINTER(C.c_int64), C.c_int64]
+        L.oracle_coalescence.restype = C.c_int64
         _lib = L
     return _lib
 
@@ -160,6 +164,20 @@ class Oracle:
 
     def init(self, mode: int):
         self._ck(lib().oracle_init(self._h, int(mode)), "oracle_init")
+
+    def set_coupling(self, group: int):
+        """Chains c with equal c // group share their random numbers (PAPER.md:232); forgets coalescence times."""
+        self._ck(lib().oracle_set_coupling(self._h, int(group)), "oracle_set_coupling")
+        self.group = int(group)
+
+    def coalescence(self) -> np.ndarray:
+        """Coalescence time of every group in full steps, -1 = not yet."""
+        ng = self.n_chains // getattr(self, "group", 1) if getattr(self, "group", 1) > 1 else 0
+        out = np.full(ng, -1, dtype=np.int64)
+        if ng:
+            got = lib().oracle_coalescence(self._h, out.ctypes.data_as(C.POINTER(C.c_int64)), ng)
+            assert got == ng
+        return out
 
     def set_complement(self, on: bool):
         lib().oracle_set_complement(self._h, int(bool(on)))
