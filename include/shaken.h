@@ -57,6 +57,7 @@ enum {
 #define SHAKEN_INIT_UP 1
 #define SHAKEN_INIT_DOWN (-1)
 #define SHAKEN_INIT_IID 0
+#define SHAKEN_INIT_SANDWICH 2 /* first chain of every coupling group all +1, the others all -1 */
 
 /*
  * shaken_create: allocate a context for n_chains independent L x L tori (batched-chain layout,
@@ -98,7 +99,7 @@ int shaken_reserve_records(shaken_ctx *ctx, int64_t max_records);
 
 /*
  * shaken_init: set sigma and tau of every chain and reset the step counter and the record count to 0.
- *   mode  SHAKEN_INIT_UP: all +1;  SHAKEN_INIT_DOWN: all -1 (the paper's scan start; the
+ *   mode  SHAKEN_INIT_SANDWICH: see shaken_set_coupling;  SHAKEN_INIT_UP: all +1;  SHAKEN_INIT_DOWN: all -1 (the paper's scan start; the
  *         top/bottom chains of :238);  SHAKEN_INIT_IID: iid +-1, spin = +1 iff the init-stream word
  *         Philox(key = seed, counter = (site>>2, chain, which, 0xFFFFFFFF))[site & 3] < 2^31,
  *         which = 0 for sigma, 1 for tau.
@@ -157,6 +158,21 @@ int shaken_set_step(shaken_ctx *ctx, uint64_t step);
  * one big batch (independent units, no exchange: SURVEY 8(e)).  Default 0.  first_chain + n_chains <= 2^32.
  */
 int shaken_set_chain_offset(shaken_ctx *ctx, uint32_t first_chain);
+
+/*
+ * Coupled chains and coalescence times.
+ * shaken_set_coupling: chains c with equal c / group evolve "with the same update function and the same sequence of
+ *   random numbers": all draw the words of the group's first chain (counter word 1 = first_chain + (c / group) * group).
+ *   group >= 1 must divide n_chains; 1 (default) uncouples.  Couplings J, q are still per chain (give the members of a
+ *   group the same values for the paper's experiment).  Forgets coalescence times.  Errors: SHAKEN_EINVAL, SHAKEN_ENOMEM.
+ * While group > 1, after EVERY full step the sigma layers of each group's members are compared on the device; the
+ *   coalescence time T = min{n : X_n = Y_n} of a group is the number of full steps done (global step counter) when they
+ *   were first all equal.  shaken_init resets the times to -1.
+ * shaken_coalescence: copy min(n_chains / group, max_groups) times to out (HOST int64, -1 = not yet); returns the
+ *   count (0 when uncoupled) or a negative error code.  Synchronises the stream.
+ */
+int shaken_set_coupling(shaken_ctx *ctx, int32_t group);
+int64_t shaken_coalescence(shaken_ctx *ctx, int64_t *out, int64_t max_groups);
 
 /* Wait until everything enqueued by this context has finished. */
 int shaken_synchronize(shaken_ctx *ctx);

@@ -93,7 +93,7 @@ __global__ void __launch_bounds__(THREADS, MINB) half_step_i8(const __grid_const
             if ((OBS || BONDS) && cur_chain >= 0) flush(cur_chain);
             cur_chain = chain;
             if (UPDATE) {
-                ck = make_chain_keys(p.keys, p.chain0 + (uint32_t)chain);
+                ck = make_chain_keys(p.keys, rng_chain(p, chain));
                 __syncwarp();
                 if (lane < 8) {
                     const int ms = lane & 1, mh = (lane >> 1) & 1, mv = lane >> 2;
@@ -107,7 +107,7 @@ __global__ void __launch_bounds__(THREADS, MINB) half_step_i8(const __grid_const
             if ((OBS || BONDS) && cur_chain >= 0) flush(cur_chain);
             cur_chain = chain;
             if (UPDATE) {
-                ck = make_chain_keys(p.keys, p.chain0 + (uint32_t)chain);
+                ck = make_chain_keys(p.keys, rng_chain(p, chain));
                 __syncthreads();                                     // everyone is done with the old table
                 if (EXTRACT == EXTRACT_PAIR) {
                     for (int t = threadIdx.x; t < 64 * 32; t += THREADS) {

@@ -78,7 +78,7 @@ __global__ void __launch_bounds__(PK_THREADS, 1) half_step_pk(const __grid_const
             if ((OBS || BONDS) && cur_chain >= 0) flush(cur_chain);
             cur_chain = chain;
             if (UPDATE) {
-                ck = make_chain_keys(p.keys, p.chain0 + (uint32_t)chain);
+                ck = make_chain_keys(p.keys, rng_chain(p, chain));
                 __syncthreads();
                 for (int t = threadIdx.x; t < PK_PAIR_ENTRIES * 32; t += PK_THREADS) {
                     const int e = t >> 5, ia = e & 7, ib = e >> 3;

@@ -117,6 +117,40 @@ __global__ void validate_bytes(const uint8_t *bytes, long long n_vec, unsigned l
     if (nbad) atomicAdd(bad, (unsigned long long)nbad);
 }
 
+// "sandwich" start: the first chain of every coupling group all +1, the others all -1, both layers.
+// vec_per_chain 16-byte vectors per chain; plus / minus are the byte patterns of the layout (int8: 0x01 / 0xFF, packed: 0xFF / 0x00).
+__global__ void init_sandwich(uint4 *sigma, uint4 *tau, long long n_vec, long long vec_per_chain, int group, uint32_t plus, uint32_t minus)
+{
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n_vec; i += (long long)gridDim.x * blockDim.x) {
+        const long long chain = i / vec_per_chain;
+        const uint32_t w = (chain % group == 0) ? plus : minus;
+        sigma[i] = make_uint4(w, w, w, w);
+        tau[i] = make_uint4(w, w, w, w);
+    }
+}
+
+// Coalescence (T = min{n : X_n = Y_n}).  compare: every member of a not yet coalesced group against the
+// group's first chain, 16 bytes at a time; any difference stamps diff[group] with the step index (all writers store the
+// same value).  finalize: a group whose stamp is not this step's has coalesced now.
+__global__ void coalesce_compare(const uint4 *sigma, long long vec_per_chain, int group, long long n_groups, const long long *coal,
+                                 unsigned long long *diff, unsigned long long stamp)
+{
+    const long long per_group = (long long)(group - 1) * vec_per_chain, total = n_groups * per_group;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
+        const long long gi = i / per_group, rest = i - gi * per_group;
+        if (coal[gi] >= 0) continue;
+        const long long m = 1 + rest / vec_per_chain, v = rest % vec_per_chain;
+        const uint4 a = sigma[(gi * group) * vec_per_chain + v], b = sigma[(gi * group + m) * vec_per_chain + v];
+        if (a.x != b.x || a.y != b.y || a.z != b.z || a.w != b.w) diff[gi] = stamp;
+    }
+}
+
+__global__ void coalesce_finalize(long long *coal, const unsigned long long *diff, long long n_groups, unsigned long long stamp)
+{
+    for (long long gi = (long long)blockIdx.x * blockDim.x + threadIdx.x; gi < n_groups; gi += (long long)gridDim.x * blockDim.x)
+        if (coal[gi] < 0 && diff[gi] != stamp) coal[gi] = (long long)stamp;
+}
+
 __global__ void philox_hook(const uint32_t *ctr, const uint32_t *key, uint32_t *out, long long n)
 {
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {

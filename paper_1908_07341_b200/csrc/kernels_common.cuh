@@ -32,7 +32,9 @@ struct StepParams {
     int L;                  // lattice side
     int nvec;               // vectors per row: L/16 (int8) or L/32 (packed)
     int n_chains;
-    uint32_t chain0;        // global index of chain 0 of this context (Philox counter word 1 = chain0 + chain)
+    uint32_t chain0;        // global index of chain 0 of this context (Philox counter word 1 = chain0 + rng chain)
+    int group;              // coupling group size (>= 1): chains c with equal c / group draw the words of chain
+                            // (c / group) * group, i.e. evolve with the same random numbers
     int rows_per_task;
     int nseg;               // warp-wide strips per row = ceil(nvec / 32)
     int nrb;                // row blocks = ceil(L / rows_per_task)
@@ -43,6 +45,9 @@ struct StepParams {
     long long *rec_prev;    // [n_chains][6] record whose C_x, C_y are still owed (F_BONDS) or nullptr
     StepKeys keys;
 };
+
+// counter word 1 of a chain: its own global index, or that of the first chain of its coupling group
+__device__ __forceinline__ uint32_t rng_chain(const StepParams &p, int chain) { return p.chain0 + (uint32_t)((chain / p.group) * p.group); }
 
 __device__ __forceinline__ uint4 ldg128(const void *p) { return __ldg(reinterpret_cast<const uint4 *>(p)); }
 __device__ __forceinline__ uint32_t ldg32(const void *p) { return __ldg(reinterpret_cast<const uint32_t *>(p)); }

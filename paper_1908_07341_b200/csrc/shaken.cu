@@ -49,6 +49,8 @@ struct shaken_ctx {
     bool have_spins = false;
     int num_sms = 0;
     int variant = 0;
+    int group = 1;                // coupling group size (shaken_set_coupling)
+    long long *d_coal = nullptr;  // [n_chains / group] coalescence times, -1 = not yet; followed by the difference stamps
     bool perwarp = false;         // strip kernels: per-warp task lists for this run (many small chains)
     int64_t launches = 0;
     char err[512] = {0};
@@ -147,6 +149,7 @@ extern "C" int shaken_destroy(shaken_ctx *ctx)
     cudaFree(ctx->d_bad);
     cudaFree(ctx->d_stage);
     cudaFree(ctx->d_xch);
+    cudaFree(ctx->d_coal);
     delete ctx;
     return SHAKEN_OK;
 }
@@ -276,6 +279,10 @@ extern "C" int shaken_set_step(shaken_ctx *ctx, uint64_t step)
 {
     if (!ctx) return SHAKEN_EINVAL;
     ctx->step = step;
+    if (ctx->d_coal) {   // difference stamps are step indices: forget them (coalescence times already found stay)
+        const size_t ng = (size_t)(ctx->n_chains / ctx->group);
+        CU(cudaMemsetAsync(ctx->d_coal + ng, 0, ng * sizeof(long long), ctx->stream));
+    }
     return SHAKEN_OK;
 }
 
@@ -304,6 +311,57 @@ extern "C" int shaken_set_variant(shaken_ctx *ctx, int variant)
     return SHAKEN_OK;
 }
 
+// ---------------------------------------------------------------------------------------------------
+// coupled chains and coalescence times
+// ---------------------------------------------------------------------------------------------------
+static int reset_coalescence(shaken_ctx *ctx)
+{
+    if (!ctx->d_coal) return SHAKEN_OK;
+    const size_t ng = (size_t)(ctx->n_chains / ctx->group);
+    CU(cudaMemsetAsync(ctx->d_coal, 0xFF, ng * sizeof(long long), ctx->stream));          // -1
+    CU(cudaMemsetAsync(ctx->d_coal + ng, 0, ng * sizeof(long long), ctx->stream));        // stamps
+    return SHAKEN_OK;
+}
+
+extern "C" int shaken_set_coupling(shaken_ctx *ctx, int32_t group)
+{
+    if (!ctx) return fail(nullptr, SHAKEN_EINVAL, "shaken_set_coupling: ctx is NULL");
+    if (group < 1 || ctx->n_chains % group != 0)
+        return fail(ctx, SHAKEN_EINVAL, "shaken_set_coupling: group=%d must be >= 1 and divide n_chains=%d", group, ctx->n_chains);
+    if (ctx->d_coal) {
+        CU(cudaStreamSynchronize(ctx->stream));
+        cudaFree(ctx->d_coal);
+        ctx->d_coal = nullptr;
+    }
+    ctx->group = group;
+    if (group > 1) {
+        int rc = ensure_device(ctx);
+        if (rc) return rc;
+        const size_t ng = (size_t)(ctx->n_chains / group);
+        if (cudaMalloc(&ctx->d_coal, 2 * ng * sizeof(long long)) != cudaSuccess) {
+            cudaGetLastError();
+            ctx->group = 1;
+            return fail(ctx, SHAKEN_ENOMEM, "cudaMalloc of the coalescence times failed");
+        }
+        return reset_coalescence(ctx);
+    }
+    return SHAKEN_OK;
+}
+
+extern "C" int64_t shaken_coalescence(shaken_ctx *ctx, int64_t *out, int64_t max_groups)
+{
+    if (!ctx || max_groups < 0) return fail(ctx, SHAKEN_EINVAL, "shaken_coalescence: bad argument");
+    if (ctx->group <= 1) return 0;
+    const int64_t ng = ctx->n_chains / ctx->group, n = ng < max_groups ? ng : max_groups;
+    if (n > 0) {
+        if (!out) return fail(ctx, SHAKEN_EINVAL, "shaken_coalescence: out is NULL");
+        cudaError_t e = cudaMemcpyAsync(out, ctx->d_coal, (size_t)n * sizeof(int64_t), cudaMemcpyDeviceToHost, ctx->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+        if (e != cudaSuccess) return fail(ctx, SHAKEN_ECUDA, "shaken_coalescence: %s", cudaGetErrorString(e));
+    }
+    return n;
+}
+
 static int grid_for(const shaken_ctx *ctx, long long work_items, int per_thread_items = 1)
 {
     long long blocks = (work_items + (long long)256 * per_thread_items - 1) / ((long long)256 * per_thread_items);
@@ -319,8 +377,8 @@ static int grid_for(const shaken_ctx *ctx, long long work_items, int per_thread_
 extern "C" int shaken_init(shaken_ctx *ctx, int mode)
 {
     if (!ctx) return fail(nullptr, SHAKEN_EINVAL, "shaken_init: ctx is NULL");
-    if (mode != SHAKEN_INIT_UP && mode != SHAKEN_INIT_DOWN && mode != SHAKEN_INIT_IID)
-        return fail(ctx, SHAKEN_EINVAL, "shaken_init: mode %d is not +1, -1 or 0", mode);
+    if (mode != SHAKEN_INIT_UP && mode != SHAKEN_INIT_DOWN && mode != SHAKEN_INIT_IID && mode != SHAKEN_INIT_SANDWICH)
+        return fail(ctx, SHAKEN_EINVAL, "shaken_init: mode %d is not +1, -1, 0 or 2", mode);
     int rc = ensure_spins(ctx);
     if (rc) return rc;
     const size_t nb = shaken_spin_bytes(ctx);
@@ -336,6 +394,12 @@ extern "C" int shaken_init(shaken_ctx *ctx, int mode)
         }
         ctx->launches++;
         CU(cudaGetLastError());
+    } else if (mode == SHAKEN_INIT_SANDWICH) {
+        const long long n_vec = (long long)(nb / 16), vpc = n_vec / ctx->n_chains;
+        const uint32_t plus = ctx->packed ? 0xFFFFFFFFu : 0x01010101u, minus = ctx->packed ? 0u : 0xFFFFFFFFu;
+        init_sandwich<<<grid_for(ctx, n_vec), 256, 0, ctx->stream>>>((uint4 *)ctx->d_sigma, (uint4 *)ctx->d_tau, n_vec, vpc, ctx->group, plus, minus);
+        ctx->launches++;
+        CU(cudaGetLastError());
     } else {
         const int up = mode == SHAKEN_INIT_UP;
         const int byte = ctx->packed ? (up ? 0xFF : 0x00) : (up ? 0x01 : 0xFF);
@@ -344,6 +408,8 @@ extern "C" int shaken_init(shaken_ctx *ctx, int mode)
     }
     ctx->have_spins = true;
     ctx->step = 0;
+    int rcc = reset_coalescence(ctx);
+    if (rcc) return rcc;
     return shaken_clear_records(ctx);
 }
 
@@ -427,6 +493,7 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
     p.nvec = ctx->packed ? ctx->L / 32 : ctx->L / 16;
     p.n_chains = ctx->n_chains;
     p.chain0 = ctx->chain0;
+    p.group = ctx->group;
     p.nseg = (p.nvec + 31) / 32;
     int resident = 2, wpb = WARPS_PER_BLOCK;                  // resident blocks per SM (launch bounds), warps per block
     if (ctx->packed) { resident = 1; wpb = PK_THREADS / 32; }
@@ -468,7 +535,7 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
     }
 
     // small-lattice path: one CTA per chain keeps both sublattices in shared memory for the whole run
-    if (!ctx->packed && ctx->L <= SMALL_L_MAX && ctx->variant == 0) {
+    if (!ctx->packed && ctx->L <= SMALL_L_MAX && ctx->variant == 0 && ctx->group == 1) {
         SmallParams sp;
         memset(&sp, 0, sizeof(sp));
         sp.sigma = (uint8_t *)ctx->d_sigma;
@@ -496,7 +563,7 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
     }
 
     // band path: mid-size lattices, few chains -- the whole run in one cooperative launch (kernel_band.cuh)
-    if (!ctx->packed && ctx->variant == 0 && ctx->L > SMALL_L_MAX && ctx->L <= BAND_L_MAX && ctx->n_chains <= ctx->num_sms) {
+    if (!ctx->packed && ctx->variant == 0 && ctx->group == 1 && ctx->L > SMALL_L_MAX && ctx->L <= BAND_L_MAX && ctx->n_chains <= ctx->num_sms) {
         if (ctx->coop < 0) {
             int dev = 0, v = 0;
             CU(cudaGetDevice(&dev));
@@ -597,6 +664,16 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
         if (e != cudaSuccess) return fail(ctx, SHAKEN_ECUDA, "half-step 1 launch: %s", cudaGetErrorString(e));
         ctx->launches += 2;
         ctx->step = t + 1;
+        if (ctx->group > 1) {
+            // sigma of every member against the first chain of its group, after every full step
+            const long long ng = ctx->n_chains / ctx->group;
+            const long long vpc = (long long)(shaken_spin_bytes(ctx) / 16) / ctx->n_chains;
+            unsigned long long *diff = reinterpret_cast<unsigned long long *>(ctx->d_coal + ng);
+            coalesce_compare<<<grid_for(ctx, ng * (ctx->group - 1) * vpc), 256, 0, ctx->stream>>>((const uint4 *)ctx->d_sigma, vpc, ctx->group, ng, ctx->d_coal, diff, (unsigned long long)ctx->step);
+            coalesce_finalize<<<grid_for(ctx, ng), 256, 0, ctx->stream>>>(ctx->d_coal, diff, ng, (unsigned long long)ctx->step);
+            CU(cudaGetLastError());
+            ctx->launches += 2;
+        }
         if (rec) {
             pending = cur;
             ctx->n_rec++;

@@ -20,7 +20,7 @@ LIB_PATH = os.path.join(_HERE, "libshaken.so")
 
 OK, EINVAL, ENOMEM, ECUDA, ESTATE, ENOSPC = 0, -1, -2, -3, -4, -5
 INT8, PACKED = 0, 1
-INIT_UP, INIT_DOWN, INIT_IID = 1, -1, 0
+INIT_UP, INIT_DOWN, INIT_IID, INIT_SANDWICH = 1, -1, 0, 2
 N_OBS = 6
 OBS_NAMES = ("M_sigma", "M_tau", "E_J", "E_q", "C_x", "C_y")
 
@@ -44,6 +44,8 @@ SIGNATURES = {
     "shaken_get_step": (C.c_int, [_p, C.POINTER(C.c_uint64)]),
     "shaken_set_step": (C.c_int, [_p, C.c_uint64]),
     "shaken_set_chain_offset": (C.c_int, [_p, C.c_uint32]),
+    "shaken_set_coupling": (C.c_int, [_p, C.c_int32]),
+    "shaken_coalescence": (C.c_int64, [_p, _p, C.c_int64]),
     "shaken_synchronize": (C.c_int, [_p]),
     "shaken_thresholds": (C.c_int, [C.c_double, C.c_double, C.POINTER(C.c_uint32)]),
     "shaken_philox_words": (C.c_int, [_p, _p, _p, C.c_int64]),
@@ -236,6 +238,18 @@ class Shaken:
 
     def set_chain_offset(self, first_chain: int):
         self._ck(self._lib.shaken_set_chain_offset(self._h, int(first_chain)))
+
+    def set_coupling(self, group: int):
+        self._ck(self._lib.shaken_set_coupling(self._h, int(group)))
+        self.group = int(group)
+
+    def coalescence(self) -> np.ndarray:
+        """Coalescence time of every coupling group in full steps, -1 = not yet (empty when uncoupled)."""
+        g = getattr(self, "group", 1)
+        ng = self.n_chains // g if g > 1 else 0
+        out = np.full(ng, -1, dtype=np.int64)
+        got = self._ck(self._lib.shaken_coalescence(self._h, out.ctypes.data, ng))
+        return out[:got]
 
     def synchronize(self):
         self._ck(self._lib.shaken_synchronize(self._h))

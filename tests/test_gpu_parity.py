@@ -333,3 +333,54 @@ def test_every_int8_code_path_matches_oracle_on_a_ragged_lattice(variant):
         s.run_grid(J, q, 5, 2)
         s.run_grid(J, q, 4, 2)
         assert_same_state(s, o, f"variant={variant}")
+
+
+# ----------------------------------------------------------------------------- coupled chains, coalescence
+@pytest.mark.parametrize("packed", [False, True])
+def test_coupled_chains_and_coalescence_times_match_oracle(packed):
+    """groups of chains that share their random numbers, sandwich start (top all +1, bottom all -1),
+    coalescence time = first full step after which the sigma layers of a group agree.  Spins, records and the times
+    must equal the oracle's bit for bit; the 32 x 32 torus is the paper's own size."""
+    L, g, n_groups, seed, steps = 32, 2, 6, 13, 120
+    J = np.repeat([0.2, 0.3, 0.44, 0.44, 0.6, 0.3], g)
+    q = np.repeat([0.3, 1.0, 0.5, 2.0, 0.3, 0.1], g)
+    o = so.Oracle(L, g * n_groups, seed)
+    o.set_coupling(g)
+    o.init(2)
+    with shaken.Shaken(L, g * n_groups, seed, packed=packed, max_records=steps) as s:
+        s.set_coupling(g)
+        s.init(shaken.INIT_SANDWICH)
+        assert np.array_equal(s.get_spins(0), o.get_spins(0)) and np.array_equal(s.get_spins(1), o.get_spins(1))
+        for chunk in (1, 40, 79):                     # the times must not depend on how the run is split
+            o.run_grid(J, q, chunk, 10)
+            s.run_grid(J, q, chunk, 10)
+            assert np.array_equal(s.coalescence(), o.coalescence()), chunk
+        assert_same_state(s, o, f"coupled packed={packed}")
+        coal = s.coalescence()
+        assert coal.shape == (n_groups,) and np.any(coal > 0)
+        sig = s.get_spins(0)
+        for gi in range(n_groups):
+            top, bot = sig[g * gi], sig[g * gi + 1]
+            assert np.all(top >= bot)                  # ordering preserved (PAPER.md:238)
+            assert (coal[gi] > 0) == bool(np.array_equal(top, bot))
+        s.init(shaken.INIT_SANDWICH)
+        assert np.all(s.coalescence() == -1)
+
+
+def test_coupling_group_of_three_with_chain_offset_and_bookkeeping():
+    L, g, seed = 48, 3, 5
+    o_big = so.Oracle(L, 2 * g, seed)
+    o_big.set_coupling(g)
+    o_big.init(2)
+    o_big.run(0.25, 0.4, 60, 0)
+    with shaken.Shaken(L, g, seed) as s:               # second group alone: chains 3..5 of the batch
+        s.set_chain_offset(g)
+        s.set_coupling(g)
+        s.init(shaken.INIT_SANDWICH)
+        s.run(0.25, 0.4, 60, 0)
+        assert np.array_equal(s.get_spins(0), o_big.get_spins(0)[g:])
+        assert np.array_equal(s.coalescence(), o_big.coalescence()[1:])
+        with pytest.raises(shaken.ShakenError):
+            s.set_coupling(2)                          # must divide n_chains
+        s.set_coupling(1)
+        assert s.coalescence().size == 0
