@@ -535,13 +535,16 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
     }
 
     // small-lattice path: one CTA per chain keeps both sublattices in shared memory for the whole run
-    if (!ctx->packed && ctx->L <= SMALL_L_MAX && ctx->variant == 0 && ctx->group == 1) {
+    if (!ctx->packed && ctx->L <= SMALL_L_MAX && ctx->variant == 0 && ctx->group <= SMALL_GROUP_MAX &&
+        (size_t)2 * ctx->group * ctx->L * ctx->L <= 200 * 1024) {
         SmallParams sp;
         memset(&sp, 0, sizeof(sp));
         sp.sigma = (uint8_t *)ctx->d_sigma;
         sp.tau = (uint8_t *)ctx->d_tau;
         sp.L = ctx->L;
         sp.n_chains = ctx->n_chains;
+        sp.group = ctx->group;
+        sp.coal = ctx->group > 1 ? ctx->d_coal : nullptr;
         sp.chain0 = ctx->chain0;
         sp.t0 = ctx->step;
         sp.n_steps = n_steps;
@@ -552,9 +555,9 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
         make_step_keys(ctx->seed, 0, sp.keys);
         const int ncalls = ctx->L * ctx->L / 4;
         int threads = ncalls < SMALL_THREADS ? ((ncalls + 31) / 32) * 32 : SMALL_THREADS;
-        const size_t smem = (size_t)2 * ctx->L * ctx->L;
+        const size_t smem = (size_t)2 * ctx->group * ctx->L * ctx->L;
         if (smem > 48 * 1024) CU(cudaFuncSetAttribute(small_run_i8, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        small_run_i8<<<ctx->n_chains, threads, smem, ctx->stream>>>(sp);
+        small_run_i8<<<ctx->n_chains / ctx->group, threads, smem, ctx->stream>>>(sp);
         CU(cudaGetLastError());
         ctx->launches++;
         ctx->step += (uint64_t)n_steps;

@@ -336,8 +336,8 @@ def test_every_int8_code_path_matches_oracle_on_a_ragged_lattice(variant):
 
 
 # ----------------------------------------------------------------------------- coupled chains, coalescence
-@pytest.mark.parametrize("packed", [False, True])
-def test_coupled_chains_and_coalescence_times_match_oracle(packed):
+@pytest.mark.parametrize("packed,variant", [(False, 0), (False, 3), (True, 0)])
+def test_coupled_chains_and_coalescence_times_match_oracle(packed, variant):
     """groups of chains that share their random numbers, sandwich start (top all +1, bottom all -1),
     coalescence time = first full step after which the sigma layers of a group agree.  Spins, records and the times
     must equal the oracle's bit for bit; the 32 x 32 torus is the paper's own size."""
@@ -348,6 +348,7 @@ def test_coupled_chains_and_coalescence_times_match_oracle(packed):
     o.set_coupling(g)
     o.init(2)
     with shaken.Shaken(L, g * n_groups, seed, packed=packed, max_records=steps) as s:
+        s.set_variant(variant)                         # 0: one CTA per group (kernel_small.cuh); 3: strip kernels + compare
         s.set_coupling(g)
         s.init(shaken.INIT_SANDWICH)
         assert np.array_equal(s.get_spins(0), o.get_spins(0)) and np.array_equal(s.get_spins(1), o.get_spins(1))
