@@ -253,3 +253,32 @@ def derived_stats(M, n_sites: int) -> dict:
 def energy(J: float, q: float, E_J: int, E_q: int) -> float:
     """H(sigma, tau) of eq. (5): -(J*E_J + q*E_q)."""
     return -(float(J) * float(int(E_J)) + float(q) * float(int(E_q)))
+
+
+# ---------------------------------------------------------------------- exact sampling (PAPER.md:240, :276)
+def propp_wilson(o: "Oracle", J, q, base: int = 1 << 40, max_doublings: int = 40):
+    """Coupling from the past (Propp & Wilson 1996, the paper's ref. [13]; "two copies of the Markov
+    chain ... run with the same update function and the same sequence of random numbers", :276 "samples are drawn
+    using the Propp-Wilson algorithm"), written out step by step for a context whose coupling groups are pairs.
+
+    Time runs over the NEGATIVE integers: the update from time s to s+1 always uses the random numbers of the full-step
+    index ``base + s`` (counter-based generator: a fixed function of the index), whatever the starting time.  For
+    T = 1, 2, 4, ...: start sigma^top (all +1) and sigma^bot (all -1) at time -T, run T steps to time 0; because the
+    dynamics preserves the ordering (:238), once top and bottom agree at time 0 every start would have ended there and
+    that configuration is an exact draw from the stationary measure.  All pairs are run with the same T until the last
+    one has coalesced (a pair that coalesced from -T ends in the same state from any earlier start).
+
+    Returns (samples [n_pairs, L, L] int8 = sigma at time 0, T used)."""
+    if getattr(o, "group", 1) != 2:
+        raise ValueError("propp_wilson needs coupling groups of two (top, bottom)")
+    Ja = np.ascontiguousarray(J, dtype=np.float64)
+    qa = np.ascontiguousarray(q, dtype=np.float64)
+    T = 1
+    for _ in range(max_doublings):
+        o.init(2)                       # top all +1, bottom all -1; also resets the step counter ...
+        o.step = base - T               # ... so the starting time -T is set afterwards
+        o.run_grid(Ja, qa, T, 0)
+        if np.all(o.coalescence() >= 0):
+            return o.get_spins(0)[0::2].copy(), T
+        T *= 2
+    raise RuntimeError("no coalescence within the allowed number of doublings")
