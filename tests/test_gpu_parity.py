@@ -385,3 +385,23 @@ def test_coupling_group_of_three_with_chain_offset_and_bookkeeping():
             s.set_coupling(2)                          # must divide n_chains
         s.set_coupling(1)
         assert s.coalescence().size == 0
+
+
+def test_propp_wilson_driver_draws_the_oracles_samples():
+    """coupling from the past on the GPU (paper_1908_07341_b200/sampling.py) against the oracle's
+    own driver (oracle/shaken_oracle.py: propp_wilson, pinned on the 3 x 3 torus): same look-back T, same samples."""
+    from paper_1908_07341_b200 import sampling
+
+    L, n_pairs, seed = 16, 24, 31
+    qs = np.repeat(np.linspace(0.3, 1.5, n_pairs), 2)
+    Js = np.repeat(np.linspace(0.15, 0.35, n_pairs), 2)
+    o = so.Oracle(L, 2 * n_pairs, seed)
+    o.set_coupling(2)
+    want, T_want = so.propp_wilson(o, Js, qs, base=1 << 33)
+    for packed in (False,):
+        with shaken.Shaken(L, 2 * n_pairs, seed, packed=packed) as s:
+            s.set_coupling(2)
+            got, T = sampling.propp_wilson(s, Js, qs, base=1 << 33)
+            assert T == T_want and np.array_equal(got, want)
+            with pytest.raises(ValueError):
+                sampling.propp_wilson(s, Js + np.tile([0.0, 0.1], n_pairs), qs)
