@@ -380,5 +380,32 @@ int oracle_set_spins(oracle_ctx *o, int which, const int8_t *host)
     return ORACLE_OK;
 }
 
+/* Diagonal spin-spin correlations of the sigma layer (Table 1), as translation-averaged integer sums
+ * over the torus.  With x = (i, j) -> column i, row j:
+ *   SW-NE  pi(sigma_{0,0} sigma_{l,l}):  out[..][0] = sum_{r,c} sigma[r][c]   * sigma[r+l][c+l]
+ *   NW-SE  pi(sigma_{0,l} sigma_{l,0}):  out[..][1] = sum_{r,c} sigma[r+l][c] * sigma[r][c+l]        (indices mod L)
+ * out layout [chain][n_ell][2]. */
+int oracle_diag_correlations(const oracle_ctx *o, const int64_t *ells, int64_t n_ell, int64_t *out)
+{
+    if (!o || !ells || !out || n_ell < 0) return ORACLE_EINVAL;
+    int64_t L = o->L;
+    size_t nsite = (size_t)L * (size_t)L;
+    for (int64_t ch = 0; ch < o->n_chains; ++ch) {
+        const int8_t *sg = o->sigma + (size_t)ch * nsite;
+        for (int64_t e = 0; e < n_ell; ++e) {
+            int64_t l = ells[e], swne = 0, nwse = 0;
+            for (int64_t r = 0; r < L; ++r)
+                for (int64_t c = 0; c < L; ++c) {
+                    int64_t r2 = wrap(r + l, L), c2 = wrap(c + l, L);
+                    swne += (int64_t)sg[r * L + c] * (int64_t)sg[r2 * L + c2];
+                    nwse += (int64_t)sg[r2 * L + c] * (int64_t)sg[r * L + c2];
+                }
+            out[((size_t)ch * (size_t)n_ell + (size_t)e) * 2 + 0] = swne;
+            out[((size_t)ch * (size_t)n_ell + (size_t)e) * 2 + 1] = nwse;
+        }
+    }
+    return ORACLE_OK;
+}
+
 uint64_t oracle_get_step(const oracle_ctx *o) { return o ? o->step : 0; }
 int oracle_set_step(oracle_ctx *o, uint64_t step) { if (!o) return ORACLE_EINVAL; o->step = step; return ORACLE_OK; }

@@ -80,6 +80,8 @@ def lib():
         L.oracle_half_step_rows.argtypes = [p, p, C.c_int64, C.c_uint64, C.c_int64, C.c_double, C.c_double,
                                             C.c_uint64, C.c_int, C.c_int64, C.c_int64]
         L.oracle_half_step_rows.restype = C.c_int
+        L.oracle_diag_correlations.argtypes = [p, C.POINTER(C.c_int64), C.c_int64, C.POINTER(C.c_int64)]
+        L.oracle_diag_correlations.restype = C.c_int
         L.oracle_set_coupling.argtypes = [p, C.c_int64]
         L.oracle_set_coupling.restype = C.c_int
         L.oracle_coalescence.argtypes = [p, C.POINTER(C.c_int64), C.c_int64]
@@ -164,6 +166,14 @@ class Oracle:
 
     def init(self, mode: int):
         self._ck(lib().oracle_init(self._h, int(mode)), "oracle_init")
+
+    def diag_correlations(self, ells) -> np.ndarray:
+        """[chain][ell][2] int64: translation-summed SW-NE and NW-SE diagonal products of sigma."""
+        e = np.ascontiguousarray(ells, dtype=np.int64)
+        out = np.zeros((self.n_chains, e.size, 2), dtype=np.int64)
+        self._ck(lib().oracle_diag_correlations(self._h, e.ctypes.data_as(C.POINTER(C.c_int64)), e.size,
+                                                out.ctypes.data_as(C.POINTER(C.c_int64))), "oracle_diag_correlations")
+        return out
 
     def set_coupling(self, group: int):
         """Chains c with equal c // group share their random numbers (PAPER.md:232); forgets coalescence times."""
