@@ -174,6 +174,16 @@ int shaken_set_chain_offset(shaken_ctx *ctx, uint32_t first_chain);
 int shaken_set_coupling(shaken_ctx *ctx, int32_t group);
 int64_t shaken_coalescence(shaken_ctx *ctx, int64_t *out, int64_t max_groups);
 
+/*
+ * shaken_diag_correlations: diagonal spin-spin correlations of the CURRENT sigma layer (Table 1; SURVEY
+ * 8(f) rank 2) as translation-summed integers over the torus (divide by L*L for the paper's pi(sigma_{0,0} sigma_{l,l})):
+ *   ells  HOST [n_ell] distances l >= 0 (taken mod L; the paper uses 1, 2, 4, 8, 16 on a 32 x 32 box)
+ *   out   HOST [n_chains][n_ell][2] int64:  [0] SW-NE  sum_{r,c} sigma[r][c] sigma[r+l][c+l]
+ *                                           [1] NW-SE  sum_{r,c} sigma[r+l][c] sigma[r][c+l]
+ * Both layouts.  Synchronises the stream.  Errors: SHAKEN_EINVAL, SHAKEN_ESTATE, SHAKEN_ENOMEM, SHAKEN_ECUDA.
+ */
+int shaken_diag_correlations(shaken_ctx *ctx, const int32_t *ells, int32_t n_ell, int64_t *out);
+
 /* Wait until everything enqueued by this context has finished. */
 int shaken_synchronize(shaken_ctx *ctx);
 

@@ -151,6 +151,46 @@ __global__ void coalesce_finalize(long long *coal, const unsigned long long *dif
         if (coal[gi] < 0 && diff[gi] != stamp) coal[gi] = (long long)stamp;
 }
 
+// Diagonal correlation sums of the sigma layer (Table 1), translation-summed over the torus:
+//   out[chain][e][0] = sum sigma[r][c] sigma[r+l][c+l]  (SW-NE),  out[chain][e][1] = sum sigma[r+l][c] sigma[r][c+l]  (NW-SE).
+// One thread per 32-bit word of row r; the partner word, l columns to the right, is a funnel shift of two aligned
+// words (int8: by 8 (l mod 4) bits, products by IDP.4A; packed: by l mod 32 bits, products by popcount of the XOR).
+// grid = (blocks per chain, n_chains); one int64 atomic per warp and sum.
+template <bool PACKED>
+__global__ void diag_corr(const uint32_t *sigma, int L, int ell, long long *out, int n_ell, int e)
+{
+    const int SPW = PACKED ? 32 : 4;                    // sites per word
+    const int W = L / SPW;
+    const int chain = blockIdx.y;
+    const uint32_t *sg = sigma + (size_t)chain * L * W;
+    const int wsh = ell / SPW, sh = (ell % SPW) * (PACKED ? 1 : 8);
+    long long swne = 0, nwse = 0;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < L * W; i += gridDim.x * blockDim.x) {
+        const int r = i / W, cw = i - r * W;
+        const int r2 = r + ell >= L ? r + ell - L : r + ell;
+        const int w0 = (cw + wsh) % W, w1 = w0 + 1 == W ? 0 : w0 + 1;
+        const uint32_t a = sg[r * W + cw], a2 = sg[r2 * W + cw];
+        const uint32_t b2 = __funnelshift_r(sg[r2 * W + w0], sg[r2 * W + w1], sh);   // sites (r+l, c+l ..)
+        const uint32_t b = __funnelshift_r(sg[r * W + w0], sg[r * W + w1], sh);      // sites (r, c+l ..)
+        if (PACKED) {
+            swne += 32 - 2 * __popc(a ^ b2);
+            nwse += 32 - 2 * __popc(a2 ^ b);
+        } else {
+            swne += __dp4a((int)a, (int)b2, 0);
+            nwse += __dp4a((int)a2, (int)b, 0);
+        }
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        swne += __shfl_down_sync(0xFFFFFFFFu, swne, o);
+        nwse += __shfl_down_sync(0xFFFFFFFFu, nwse, o);
+    }
+    if ((threadIdx.x & 31) == 0) {
+        long long *dst = out + ((size_t)chain * n_ell + e) * 2;
+        atomicAdd(reinterpret_cast<unsigned long long *>(dst), (unsigned long long)swne);
+        atomicAdd(reinterpret_cast<unsigned long long *>(dst + 1), (unsigned long long)nwse);
+    }
+}
+
 __global__ void philox_hook(const uint32_t *ctr, const uint32_t *key, uint32_t *out, long long n)
 {
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {

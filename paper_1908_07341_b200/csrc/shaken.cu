@@ -803,6 +803,43 @@ extern "C" int shaken_set_spins(shaken_ctx *ctx, int which, const int8_t *host)
 }
 
 // ---------------------------------------------------------------------------------------------------
+// diagonal correlations
+// ---------------------------------------------------------------------------------------------------
+extern "C" int shaken_diag_correlations(shaken_ctx *ctx, const int32_t *ells, int32_t n_ell, int64_t *out)
+{
+    if (!ctx || !ells || !out || n_ell < 1) return fail(ctx, SHAKEN_EINVAL, "shaken_diag_correlations: bad argument");
+    if (!ctx->have_spins || !ctx->d_sigma) return fail(ctx, SHAKEN_ESTATE, "shaken_diag_correlations: no spins yet");
+    for (int e = 0; e < n_ell; ++e)
+        if (ells[e] < 0) return fail(ctx, SHAKEN_EINVAL, "shaken_diag_correlations: negative distance");
+    int rc = ensure_device(ctx);
+    if (rc) return rc;
+    const size_t n = (size_t)ctx->n_chains * (size_t)n_ell * 2;
+    long long *d = nullptr;
+    if (cudaMalloc(&d, n * sizeof(long long)) != cudaSuccess) {
+        cudaGetLastError();
+        return fail(ctx, SHAKEN_ENOMEM, "cudaMalloc of %zu correlation sums failed", n);
+    }
+    cudaError_t err = cudaMemsetAsync(d, 0, n * sizeof(long long), ctx->stream);
+    const int W = ctx->packed ? ctx->L / 32 : ctx->L / 4;
+    long long bpc = ((long long)ctx->L * W + 255) / 256;
+    const long long cap = (long long)ctx->num_sms * 8 / ctx->n_chains + 1;
+    if (bpc > cap) bpc = cap;
+    const dim3 grid((unsigned)bpc, (unsigned)ctx->n_chains);
+    for (int e = 0; e < n_ell && err == cudaSuccess; ++e) {
+        const int l = ells[e] % ctx->L;
+        if (ctx->packed) diag_corr<true><<<grid, 256, 0, ctx->stream>>>((const uint32_t *)ctx->d_sigma, ctx->L, l, d, n_ell, e);
+        else diag_corr<false><<<grid, 256, 0, ctx->stream>>>((const uint32_t *)ctx->d_sigma, ctx->L, l, d, n_ell, e);
+        ctx->launches++;
+        err = cudaGetLastError();
+    }
+    if (err == cudaSuccess) err = cudaMemcpyAsync(out, d, n * sizeof(long long), cudaMemcpyDeviceToHost, ctx->stream);
+    if (err == cudaSuccess) err = cudaStreamSynchronize(ctx->stream);
+    cudaFree(d);
+    if (err != cudaSuccess) return fail(ctx, SHAKEN_ECUDA, "shaken_diag_correlations: %s", cudaGetErrorString(err));
+    return SHAKEN_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------
 // test hook
 // ---------------------------------------------------------------------------------------------------
 extern "C" int shaken_philox_words(const uint32_t *ctr, const uint32_t *key, uint32_t *out, int64_t n)

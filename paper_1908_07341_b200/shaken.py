@@ -46,6 +46,7 @@ SIGNATURES = {
     "shaken_set_chain_offset": (C.c_int, [_p, C.c_uint32]),
     "shaken_set_coupling": (C.c_int, [_p, C.c_int32]),
     "shaken_coalescence": (C.c_int64, [_p, _p, C.c_int64]),
+    "shaken_diag_correlations": (C.c_int, [_p, _p, C.c_int32, _p]),
     "shaken_synchronize": (C.c_int, [_p]),
     "shaken_thresholds": (C.c_int, [C.c_double, C.c_double, C.POINTER(C.c_uint32)]),
     "shaken_philox_words": (C.c_int, [_p, _p, _p, C.c_int64]),
@@ -250,6 +251,13 @@ class Shaken:
         out = np.full(ng, -1, dtype=np.int64)
         got = self._ck(self._lib.shaken_coalescence(self._h, out.ctypes.data, ng))
         return out[:got]
+
+    def diag_correlations(self, ells) -> np.ndarray:
+        """[chain][ell][2] int64: translation-summed SW-NE and NW-SE diagonal products of the current sigma."""
+        e = np.ascontiguousarray(ells, dtype=np.int32)
+        out = np.zeros((self.n_chains, e.size, 2), dtype=np.int64)
+        self._ck(self._lib.shaken_diag_correlations(self._h, e.ctypes.data, e.size, out.ctypes.data))
+        return out
 
     def synchronize(self):
         self._ck(self._lib.shaken_synchronize(self._h))

@@ -405,3 +405,20 @@ def test_propp_wilson_driver_draws_the_oracles_samples():
             assert T == T_want and np.array_equal(got, want)
             with pytest.raises(ValueError):
                 sampling.propp_wilson(s, Js + np.tile([0.0, 0.1], n_pairs), qs)
+
+
+@pytest.mark.parametrize("L,packed", [(32, False), (32, True), (176, False), (160, True)])
+def test_diagonal_correlation_sums_match_oracle(L, packed):
+    """SURVEY 8(f) rank 2 (Table 1: 32 x 32 box, l = 1, 2, 4, 8, 16): SW-NE and NW-SE sums of the
+    sigma layer after a few steps, for distances that are and are not multiples of the word width, incl. l >= L."""
+    n, seed = 3, 17
+    ells = [0, 1, 2, 3, 4, 5, 8, 16, 31, 33, L - 1, L, L + 7]
+    o = so.Oracle(L, n, seed)
+    o.init(0)
+    o.run_grid([0.3, 0.44, 0.6], [0.2, 1.0, 0.5], 5, 0)
+    with shaken.Shaken(L, n, seed, packed=packed) as s:
+        s.init(0)
+        s.run_grid([0.3, 0.44, 0.6], [0.2, 1.0, 0.5], 5, 0)
+        assert np.array_equal(s.diag_correlations(ells), o.diag_correlations(ells))
+        with pytest.raises(shaken.ShakenError):
+            s.diag_correlations([-1])
