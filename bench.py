@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- one JSON line for BASELINE.json's metric: spin site-updates/ns of the shaken-dynamics hot path.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg4|cfg1|cfg2|cfg3|cfg5] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg4|cfg1|cfg2|cfg3|cfg5|paper<L>] [--impl reference]
 
 A *step* is one full shaken step over the whole workload: half-step 0 (eq. 15) and half-step 1 (eq. 16) of
 every site of every chain, with the observable sums fused in as the workload prescribes.  Default workload:
@@ -58,6 +58,8 @@ def parse_args():
 def workload(name: str):
     from paper_1908_07341_b200 import workloads
 
+    if name.startswith("paper"):        # the paper's own benchmark point at lattice side L: --workload paper2048
+        return workloads.paper_benchmark_point(int(name[5:]))
     idx = {"cfg1": 1, "cfg2": 2, "cfg3": 3, "cfg4": 4, "cfg5": 5}[name]
     return workloads.config(idx)
 
