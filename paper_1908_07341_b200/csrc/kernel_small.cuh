@@ -34,20 +34,28 @@ struct SmallParams {
     StepKeys keys;           // only k0[], k1[] are used (functions of the seed)
 };
 
-__global__ void __launch_bounds__(SMALL_THREADS, 1) small_run_i8(const __grid_constant__ SmallParams p)
+// dynamic shared memory of small_run_i8: G members x (sigma words, tau words), then G paired threshold tables
+__host__ __device__ inline size_t small_smem_bytes(int L, int G) { return (size_t)G * ((size_t)2 * L * L + 64 * 32 * sizeof(uint2)); }
+
+// MAXT: the largest block this instance is launched with (256 for L <= 64: no register cap on the four interleaved
+// Philox calls; 1024 for L = 128)
+template <int MAXT>
+__global__ void __launch_bounds__(MAXT, 1) small_run_i8(const __grid_constant__ SmallParams p)
 {
     extern __shared__ __align__(16) uint32_t smem[];
     const int L = p.L;
     const int W = L >> 2;                         // 32-bit words (= Philox calls) per row
     const int ncalls = L * W;                     // per sublattice
+    const int nvec = L >> 4, nvecs = L * nvec;    // 16-byte vectors per row / per sublattice
     const int G = p.group;
-    __shared__ uint32_t s_tab[SMALL_GROUP_MAX][64];
+    uint2 *s_pair = reinterpret_cast<uint2 *>(smem + 2 * G * ncalls);   // [G][64][32], see kernel_i8.cuh EXTRACT_PAIR
     __shared__ int s_red[32][6];
 
     const int gi = blockIdx.x, chain_first = gi * G;
     const int tid = threadIdx.x;
     const int lane = tid & 31, warp = tid >> 5;
     const int nwarps = blockDim.x >> 5;
+    const uint32_t lane8 = (uint32_t)lane * 8u;
     const size_t plane = (size_t)L * L;
     // member m: sigma words at smem + 2 m ncalls, tau words right behind
     for (int m = 0; m < G; ++m) {
@@ -55,13 +63,18 @@ __global__ void __launch_bounds__(SMALL_THREADS, 1) small_run_i8(const __grid_co
         const uint32_t *gt = reinterpret_cast<const uint32_t *>(p.tau + (size_t)(chain_first + m) * plane);
         uint32_t *sg = smem + 2 * m * ncalls, *ta = sg + ncalls;
         for (int i = tid; i < ncalls; i += blockDim.x) { sg[i] = gs[i]; ta[i] = gt[i]; }
-    }
-    if (tid < 8 * G) {
-        const int m = tid >> 3, t = tid & 7;
-        const int ms = t & 1, mh = (t >> 1) & 1, mv = t >> 2;
-        const int idx = 2 * (2 - mh - mv) + (1 - ms);
-        s_tab[m][(((uint32_t)ms << 3) | ((uint32_t)mh << 4) | (mv ? 0xE4u : 0u)) >> 2] =
-            p.gtab ? p.gtab[(size_t)(chain_first + m) * 8 + idx] : p.utab[idx];
+        for (int t = tid; t < 64 * 32; t += blockDim.x) {
+            const int e = t >> 5;
+            uint32_t T2[2];
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const int c = h ? (e >> 3) : (e & 7);
+                const int ms = c & 1, mh = (c >> 1) & 1, mv = c >> 2;
+                const int idx = 2 * (2 - mh - mv) + (1 - ms);          // T[2k + c]
+                T2[h] = p.gtab ? p.gtab[(size_t)(chain_first + m) * 8 + idx] : p.utab[idx];
+            }
+            s_pair[(size_t)m * 64 * 32 + t] = make_uint2(T2[0], T2[1]);
+        }
     }
     __syncthreads();
 
@@ -75,28 +88,43 @@ __global__ void __launch_bounds__(SMALL_THREADS, 1) small_run_i8(const __grid_co
             ChainKeys ck;
             // one sequence of random numbers for the whole group: the words of its first chain
             device_half_step_keys(p.keys, 2ull * t + (unsigned)half, p.chain0 + (uint32_t)chain_first, xa2, xb0, ck);
-            for (int c = tid; c < ncalls; c += blockDim.x) {
-                const int r = c / W, cw = c - r * W;
-                uint32_t rw[4];
-                philox_site_words((uint32_t)c, p.keys, xa2, xb0, ck, rw);
-                const int cv = half == 0 ? (r == 0 ? L - 1 : r - 1) * W + cw : (r == L - 1 ? 0 : r + 1) * W + cw;
-                const int ce = half == 0 ? r * W + (cw == 0 ? W - 1 : cw - 1) : r * W + (cw == W - 1 ? 0 : cw + 1);
+            // one 16-byte vector (4 words, 4 interleaved Philox calls) per thread per trip, as in kernel_i8.cuh
+#pragma unroll 1
+            for (int c = tid; c < nvecs; c += blockDim.x) {
+                const int r = c / nvec, cv = c - r * nvec;
+                const int at = r * W + 4 * cv;
+                uint32_t rw[4][4];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) philox_site_words((uint32_t)(at + j), p.keys, xa2, xb0, ck, rw[j]);
+                const int av = half == 0 ? (r == 0 ? L - 1 : r - 1) * W + 4 * cv : (r == L - 1 ? 0 : r + 1) * W + 4 * cv;
+                const int ae = half == 0 ? r * W + (cv == 0 ? W - 1 : 4 * cv - 1) : r * W + (cv == nvec - 1 ? 0 : 4 * cv + 4);
 #pragma unroll 1
                 for (int m = 0; m < G; ++m) {
                     const uint32_t *src = smem + 2 * m * ncalls + (half ? ncalls : 0);
                     uint32_t *dst = smem + 2 * m * ncalls + (half ? 0 : ncalls);
-                    const uint32_t sw = src[c], vw = src[cv], e = src[ce];
-                    const uint32_t hw = half == 0 ? __funnelshift_l(e, sw, 8) : __funnelshift_r(sw, e, 8);
-                    const uint32_t y = (hw & 0x10101010u) | (vw & ~0x10101010u);
-                    const uint32_t z = ((sw & 0x08080808u) | (y & ~0x08080808u)) & 0xFCFCFCFCu;
-                    uint32_t out = 0xFFFFFFFFu;
+                    const char *tab = reinterpret_cast<const char *>(s_pair + (size_t)m * 64 * 32);
+                    const uint4 s4 = *reinterpret_cast<const uint4 *>(src + at);
+                    const uint4 v4 = *reinterpret_cast<const uint4 *>(src + av);
+                    const uint32_t e = src[ae];
+                    const uint32_t w[4] = {s4.x, s4.y, s4.z, s4.w}, vw[4] = {v4.x, v4.y, v4.z, v4.w};
+                    uint32_t o[4];
 #pragma unroll
-                    for (int b = 0; b < 4; ++b) {
-                        const uint32_t code = b == 3 ? (z >> 24) : __byte_perm(z, 0u, 0x4440u + b);
-                        const uint32_t T = *reinterpret_cast<const uint32_t *>(reinterpret_cast<const char *>(s_tab[m]) + code);
-                        out = xor_if_less(out, rw[b], T, 0xFEu << (8 * b));
+                    for (int j = 0; j < 4; ++j) {
+                        const uint32_t hw = half == 0 ? __funnelshift_l(j == 0 ? e : w[j - 1], w[j], 8)
+                                                      : __funnelshift_r(w[j], j == 3 ? e : w[j + 1], 8);
+                        const uint32_t y = (hw & 0x40044004u) | (vw[j] & ~0x40044004u);
+                        const uint32_t z = ((w[j] & 0x20022002u) | (y & ~0x20022002u)) & 0xE00EE00Eu;
+                        const uint32_t o01 = __dp4a(z, 0x00004080u, lane8), o23 = __dp4a(z, 0x40800000u, lane8);
+                        const uint2 t01 = *reinterpret_cast<const uint2 *>(tab + o01);
+                        const uint2 t23 = *reinterpret_cast<const uint2 *>(tab + o23);
+                        uint32_t out = 0x01010101u;
+                        out = add_if_not_less(out, rw[j][0], t01.x, 0xFEu);
+                        out = add_if_not_less(out, rw[j][1], t01.y, 0xFEu << 8);
+                        out = add_if_not_less(out, rw[j][2], t23.x, 0xFEu << 16);
+                        out = add_if_not_less(out, rw[j][3], t23.y, 0xFEu << 24);
+                        o[j] = out;
                     }
-                    dst[c] = out;
+                    *reinterpret_cast<uint4 *>(dst + at) = make_uint4(o[0], o[1], o[2], o[3]);
                 }
             }
             __syncthreads();
@@ -136,10 +164,12 @@ __global__ void __launch_bounds__(SMALL_THREADS, 1) small_run_i8(const __grid_co
                     if (lane == 0) s_red[warp][k] = w;
                 }
                 __syncthreads();
-                if (tid < 6) {
-                    long long tot = 0;
-                    for (int w = 0; w < nwarps; ++w) tot += s_red[w][tid];
-                    p.rec[((size_t)nrec * p.n_chains + chain_first + m) * 6 + tid] = tot;
+                if (warp == 0) {                       // second level: one warp sums the per-warp partials (|sum| <= 2 L^2)
+#pragma unroll
+                    for (int k = 0; k < 6; ++k) {
+                        const int tot = __reduce_add_sync(0xFFFFFFFFu, lane < nwarps ? s_red[lane][k] : 0);
+                        if (lane == 0) p.rec[((size_t)nrec * p.n_chains + chain_first + m) * 6 + k] = (long long)tot;
+                    }
                 }
                 __syncthreads();
             }

@@ -536,7 +536,7 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
 
     // small-lattice path: one CTA per chain keeps both sublattices in shared memory for the whole run
     if (!ctx->packed && ctx->L <= SMALL_L_MAX && ctx->variant == 0 && ctx->group <= SMALL_GROUP_MAX &&
-        (size_t)2 * ctx->group * ctx->L * ctx->L <= 200 * 1024) {
+        small_smem_bytes(ctx->L, ctx->group) <= 200 * 1024) {
         SmallParams sp;
         memset(&sp, 0, sizeof(sp));
         sp.sigma = (uint8_t *)ctx->d_sigma;
@@ -553,11 +553,16 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
         sp.gtab = p.gtab;
         memcpy(sp.utab, p.utab, sizeof(sp.utab));
         make_step_keys(ctx->seed, 0, sp.keys);
-        const int ncalls = ctx->L * ctx->L / 4;
-        int threads = ncalls < SMALL_THREADS ? ((ncalls + 31) / 32) * 32 : SMALL_THREADS;
-        const size_t smem = (size_t)2 * ctx->group * ctx->L * ctx->L;
-        if (smem > 48 * 1024) CU(cudaFuncSetAttribute(small_run_i8, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        small_run_i8<<<ctx->n_chains / ctx->group, threads, smem, ctx->stream>>>(sp);
+        const int nvecs = ctx->L * ctx->L / 16;             // one 16-byte vector per thread per trip
+        int threads = nvecs < SMALL_THREADS ? ((nvecs + 31) / 32) * 32 : SMALL_THREADS;
+        const size_t smem = small_smem_bytes(ctx->L, ctx->group);
+        if (threads <= 256) {
+            if (smem > 40 * 1024) CU(cudaFuncSetAttribute(small_run_i8<256>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            small_run_i8<256><<<ctx->n_chains / ctx->group, threads, smem, ctx->stream>>>(sp);
+        } else {
+            if (smem > 40 * 1024) CU(cudaFuncSetAttribute(small_run_i8<1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            small_run_i8<1024><<<ctx->n_chains / ctx->group, threads, smem, ctx->stream>>>(sp);
+        }
         CU(cudaGetLastError());
         ctx->launches++;
         ctx->step += (uint64_t)n_steps;
