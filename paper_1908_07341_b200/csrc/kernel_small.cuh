@@ -13,8 +13,8 @@
 
 namespace shaken {
 
-constexpr int SMALL_L_MAX = 128;
-constexpr int SMALL_THREADS = 1024;
+constexpr int SMALL_L_MAX = 128;        // always the one-CTA-per-chain path
+constexpr int SMALL_L_BATCH_MAX = 288;  // ... and up to here for batches that fill the machine (2 L^2 + 16 KiB <= 200 KiB)
 constexpr int SMALL_GROUP_MAX = 8;   // coupled chains of one group share a CTA (and every Philox call)
 
 struct SmallParams {
@@ -37,8 +37,8 @@ struct SmallParams {
 // dynamic shared memory of small_run_i8: G members x (sigma words, tau words), then G paired threshold tables
 __host__ __device__ inline size_t small_smem_bytes(int L, int G) { return (size_t)G * ((size_t)2 * L * L + 64 * 32 * sizeof(uint2)); }
 
-// MAXT: the largest block this instance is launched with (256 for L <= 64: no register cap on the four interleaved
-// Philox calls; 1024 for L = 128)
+// MAXT: the largest block this instance is launched with (256 for L <= 64, 512 above: up to 128 registers for the four
+// interleaved Philox calls)
 template <int MAXT>
 __global__ void __launch_bounds__(MAXT, 1) small_run_i8(const __grid_constant__ SmallParams p)
 {

@@ -535,8 +535,12 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
     }
 
     // small-lattice path: one CTA per chain keeps both sublattices in shared memory for the whole run
-    if (!ctx->packed && ctx->L <= SMALL_L_MAX && ctx->variant == 0 && ctx->group <= SMALL_GROUP_MAX &&
-        small_smem_bytes(ctx->L, ctx->group) <= 200 * 1024) {
+    // (also mid-size chains, L <= 288, when there are enough of them to fill the machine: the strip kernels would leave
+    // most lanes of a warp idle on rows narrower than 512 spins, and the band path is for few chains)
+    const bool small_path = !ctx->packed && ctx->variant == 0 && ctx->group <= SMALL_GROUP_MAX &&
+                            small_smem_bytes(ctx->L, ctx->group) <= 200 * 1024 &&
+                            (ctx->L <= SMALL_L_MAX || (ctx->L <= SMALL_L_BATCH_MAX && 2 * (ctx->n_chains / ctx->group) >= ctx->num_sms));
+    if (small_path) {
         SmallParams sp;
         memset(&sp, 0, sizeof(sp));
         sp.sigma = (uint8_t *)ctx->d_sigma;
@@ -554,14 +558,14 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
         memcpy(sp.utab, p.utab, sizeof(sp.utab));
         make_step_keys(ctx->seed, 0, sp.keys);
         const int nvecs = ctx->L * ctx->L / 16;             // one 16-byte vector per thread per trip
-        int threads = nvecs < SMALL_THREADS ? ((nvecs + 31) / 32) * 32 : SMALL_THREADS;
+        const int threads = nvecs <= 256 ? ((nvecs + 31) / 32) * 32 : 512;
         const size_t smem = small_smem_bytes(ctx->L, ctx->group);
         if (threads <= 256) {
             if (smem > 40 * 1024) CU(cudaFuncSetAttribute(small_run_i8<256>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
             small_run_i8<256><<<ctx->n_chains / ctx->group, threads, smem, ctx->stream>>>(sp);
         } else {
-            if (smem > 40 * 1024) CU(cudaFuncSetAttribute(small_run_i8<1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-            small_run_i8<1024><<<ctx->n_chains / ctx->group, threads, smem, ctx->stream>>>(sp);
+            if (smem > 40 * 1024) CU(cudaFuncSetAttribute(small_run_i8<512>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            small_run_i8<512><<<ctx->n_chains / ctx->group, threads, smem, ctx->stream>>>(sp);
         }
         CU(cudaGetLastError());
         ctx->launches++;
@@ -571,7 +575,7 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
     }
 
     // band path: mid-size lattices, few chains -- the whole run in one cooperative launch (kernel_band.cuh)
-    if (!ctx->packed && ctx->variant == 0 && ctx->group == 1 && ctx->L > SMALL_L_MAX && ctx->L <= BAND_L_MAX && ctx->n_chains <= ctx->num_sms) {
+    if (!ctx->packed && ctx->variant == 0 && ctx->group == 1 && ctx->L > SMALL_L_MAX && ctx->L <= BAND_L_MAX && ctx->n_chains <= ctx->num_sms) {   // (small_path returned above)
         if (ctx->coop < 0) {
             int dev = 0, v = 0;
             CU(cudaGetDevice(&dev));
@@ -632,11 +636,19 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
             ctx->xch_stamp += (uint32_t)(2 * n_steps);
             CU(cudaFuncSetAttribute(band_run_i8, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
             void *args[] = {&bp};
-            CU(cudaLaunchCooperativeKernel((const void *)band_run_i8, dim3(n_bands), dim3(BAND_THREADS), args, smem, ctx->stream));
-            ctx->launches++;
-            ctx->step += (uint64_t)n_steps;
-            ctx->n_rec += n_new;
-            return SHAKEN_OK;
+            // the bands wait for one another, so they must all be resident: a cooperative launch either guarantees
+            // that or fails up front (a smaller or shared GPU) -- then the strip kernels below do the job
+            const cudaError_t le = cudaLaunchCooperativeKernel((const void *)band_run_i8, dim3(n_bands), dim3(BAND_THREADS), args, smem, ctx->stream);
+            if (le == cudaSuccess) {
+                ctx->launches++;
+                ctx->step += (uint64_t)n_steps;
+                ctx->n_rec += n_new;
+                return SHAKEN_OK;
+            }
+            cudaGetLastError();
+            ctx->xch_stamp -= (uint32_t)(2 * n_steps);
+            if (le != cudaErrorCooperativeLaunchTooLarge && le != cudaErrorLaunchOutOfResources && le != cudaErrorNotSupported)
+                return fail(ctx, SHAKEN_ECUDA, "band kernel launch: %s", cudaGetErrorString(le));
         }
     }
 

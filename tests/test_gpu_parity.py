@@ -422,3 +422,21 @@ def test_diagonal_correlation_sums_match_oracle(L, packed):
         assert np.array_equal(s.diag_correlations(ells), o.diag_correlations(ells))
         with pytest.raises(shaken.ShakenError):
             s.diag_correlations([-1])
+
+
+def test_batch_of_mid_size_chains_runs_in_the_one_cta_per_chain_path():
+    """128 < L <= 288 with enough chains to fill the machine (the paper's (q,J) scan uses 200 x 200): one
+    CTA per chain, whole run in one launch, rows of 13 vectors (not a power of two) walked by 512 threads."""
+    L, n, seed = 208, 80, 3
+    J = np.linspace(0.1, 0.9, n)
+    q = np.linspace(2.0, 0.1, n)
+    o = so.Oracle(L, n, seed)
+    o.init(-1)                                         # the paper's scan starts from all -1 (PAPER.md:200)
+    o.run_grid(J, q, 5, 2)
+    with shaken.Shaken(L, n, seed, max_records=4) as s:
+        s.init(-1)
+        l0 = s.launch_count
+        s.run_grid(J, q, 3, 2)
+        s.run_grid(J, q, 2, 2)
+        assert s.launch_count - l0 == 2                # one launch per shaken_run call
+        assert_same_state(s, o, "L=208 batch")
