@@ -144,19 +144,27 @@ __global__ void __launch_bounds__(MAXT, 1) small_run_i8(const __grid_constant__ 
             for (int m = 0; m < G; ++m) {
                 const uint32_t *sg = smem + 2 * m * ncalls, *ta = sg + ncalls;
                 int v[6] = {0, 0, 0, 0, 0, 0};
-                for (int c = tid; c < ncalls; c += blockDim.x) {
-                    const int r = c / W, cw = c - r * W;
-                    const int up = (r == L - 1 ? 0 : r + 1) * W + cw;
-                    const int rt = r * W + (cw == W - 1 ? 0 : cw + 1);
-                    const uint32_t s0 = sg[c], t0w = ta[c];
-                    const int sr = (int)__funnelshift_r(s0, sg[rt], 8), tr = (int)__funnelshift_r(t0w, ta[rt], 8);
-                    v[0] = __dp4a((int)s0, 0x01010101, v[0]);
-                    v[1] = __dp4a((int)t0w, 0x01010101, v[1]);
-                    v[2] = __dp4a((int)s0, (int)ta[up], v[2]);
-                    v[2] = __dp4a((int)s0, tr, v[2]);
-                    v[3] = __dp4a((int)s0, (int)t0w, v[3]);
-                    v[4] = __dp4a((int)s0, sr, v[4]);
-                    v[5] = __dp4a((int)s0, (int)sg[up], v[5]);
+                for (int c = tid; c < nvecs; c += blockDim.x) {       // one 16-byte vector of each layer per trip
+                    const int r = c / nvec, cv = c - r * nvec;
+                    const int at = r * W + 4 * cv;
+                    const int up = (r == L - 1 ? 0 : r + 1) * W + 4 * cv;
+                    const int rt = r * W + (cv == nvec - 1 ? 0 : 4 * cv + 4);
+                    const uint4 s4 = *reinterpret_cast<const uint4 *>(sg + at), t4 = *reinterpret_cast<const uint4 *>(ta + at);
+                    const uint4 su4 = *reinterpret_cast<const uint4 *>(sg + up), tu4 = *reinterpret_cast<const uint4 *>(ta + up);
+                    const uint32_t sw[5] = {s4.x, s4.y, s4.z, s4.w, sg[rt]}, tw[5] = {t4.x, t4.y, t4.z, t4.w, ta[rt]};
+                    const uint32_t su[4] = {su4.x, su4.y, su4.z, su4.w}, tu[4] = {tu4.x, tu4.y, tu4.z, tu4.w};
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) {
+                        const int s0 = (int)sw[j], t0w = (int)tw[j];
+                        const int sr = (int)__funnelshift_r(sw[j], sw[j + 1], 8), tr = (int)__funnelshift_r(tw[j], tw[j + 1], 8);
+                        v[0] = __dp4a(s0, 0x01010101, v[0]);
+                        v[1] = __dp4a(t0w, 0x01010101, v[1]);
+                        v[2] = __dp4a(s0, (int)tu[j], v[2]);
+                        v[2] = __dp4a(s0, tr, v[2]);
+                        v[3] = __dp4a(s0, t0w, v[3]);
+                        v[4] = __dp4a(s0, sr, v[4]);
+                        v[5] = __dp4a(s0, (int)su[j], v[5]);
+                    }
                 }
 #pragma unroll
                 for (int k = 0; k < 6; ++k) {
