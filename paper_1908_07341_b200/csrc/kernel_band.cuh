@@ -4,9 +4,9 @@
 // shared memory; per half-step it needs exactly one row from a neighbouring band (eq. (14): the field
 // uses the down row in half 0, the up row in half 1), which the neighbour publishes through a small global buffer in
 // "data + stamp" form: every 8-byte store carries the spin word and the half-step stamp, so a reader that sees the
-// stamp has the data (no fence, no separate flag).  A CTA computes its rows in walking order, so the row its neighbour
-// waits for is in the first trip, and each of its vectors is published by the thread that computed it; one warp does
-// no arithmetic and polls for the row the CTA itself needs next.  There is no grid-wide barrier: only neighbouring
+// stamp has the data (no fence, no separate flag).  A CTA computes the row its neighbour waits for first, one word per
+// thread, and every word is published by the thread that computed it; one warp does no arithmetic and polls for the
+// row the CTA itself needs next.  There is no grid-wide barrier: only neighbouring
 // bands wait for each other, which is why all CTAs must be co-resident -- the cooperative launch guarantees it.
 // Site -> random word mapping, thresholds and rule are those of kernel_i8.cuh; only the schedule differs.
 #pragma once
@@ -136,14 +136,28 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) band_run_i8(const __grid_cons
             o[j] = update_word(w[j], half ? hr : hl, vw[j], n + (uint32_t)j);
         }
         *reinterpret_cast<uint4 *>(dst + at) = make_uint4(o[0], o[1], o[2], o[3]);
-        // the first row in walking order (first tau row in half 0, last sigma row in half 1) is the one the neighbouring
-        // band waits for: it leaves at once, straight from the thread that computed it ({word, stamp} pairs, 16 bytes
-        // per store), with no barrier on the critical path of the ring
-        if (rr == 0) {
+        if (rr == 0) {                            // (tall bands only, see below) a vector of the row the neighbour waits for
             uint4 *x = reinterpret_cast<uint4 *>(xmine + 4 * cv);
             __stcg(x, make_uint4(o[0], stamp, o[1], stamp));
             __stcg(x + 1, make_uint4(o[2], stamp, o[3], stamp));
         }
+    };
+
+    // The first row in walking order (first tau row in half 0, last sigma row in half 1) is the one the neighbouring band
+    // waits for and the only one that reads the incoming row: it is done one WORD per thread (a single Philox call, the
+    // shortest latency there is), ahead of the vectors, and each word leaves at once for the neighbour as a
+    // {word, stamp} pair -- no barrier on the critical path of the ring.
+    auto boundary_word = [&](const int half, const int cw, uint2 *xmine, const uint32_t stamp) {
+        const uint32_t *src = half ? ta : sg;
+        uint32_t *dst = half ? sg : ta;
+        const uint32_t *halo = half ? ht : hs;
+        const int r = half ? nr - 1 : 0, at = r * W + cw;
+        const uint32_t sw = src[at];
+        const uint32_t e = src[r * W + (half ? (cw == W - 1 ? 0 : cw + 1) : (cw == 0 ? W - 1 : cw - 1))];
+        const uint32_t hw = half ? __funnelshift_r(sw, e, 8) : __funnelshift_l(e, sw, 8);
+        const uint32_t out = update_word(sw, hw, halo[cw], (uint32_t)(r0 + r) * (uint32_t)W + (uint32_t)cw);
+        dst[at] = out;
+        __stcg(xmine + cw, make_uint2(out, stamp));
     };
 
     // block-wide sums of up to six int partials into one record (int64 atomics: bands of a chain share the record)
@@ -224,9 +238,17 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) band_run_i8(const __grid_cons
         // The last warp does no arithmetic: it polls for the neighbour's row from the start of the half-step, so the
         // handshake (one L2 round trip after the neighbour's first vectors are done) hides behind the other 15 warps.
         if (duty_warp) collect(xnbr, stamp, half ? hs : ht);
-        else
+        else if (nvecs <= 3 * WORKERS) {
+            // short bands: the hand-over is the critical path, so the neighbour's row goes first, word by word
+#pragma unroll 1
+            for (int cw = tid; cw < W; cw += WORKERS) boundary_word(half, cw, xmine, stamp);
+#pragma unroll 1
+            for (int c = nvec + tid; c < nvecs; c += WORKERS) update_vector(half, c, xmine, stamp);   // rows 1 .. nr-1
+        } else {
+            // tall bands: several trips of vectors hide the hand-over anyway; the row is part of the first trip
 #pragma unroll 1
             for (int c = tid; c < nvecs; c += WORKERS) update_vector(half, c, xmine, stamp);
+        }
         __syncthreads();
 
         // record (M_sigma, M_tau, E_J, E_q now; C_x, C_y at the start of the next half-step 0)
