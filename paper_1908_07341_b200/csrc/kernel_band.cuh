@@ -189,10 +189,8 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) band_run_i8(const __grid_cons
         reduce_to(dst, v, 4, 2);
     };
 
-    // Exchange.  publish: every thread below W stores one {word, stamp}.  prefetch (duty warp, right after its own
-    // publish -- the neighbour publishes at about the same time): asynchronous 16-byte copies L2 -> shared memory that
-    // fly while the band is computed.  collect (duty warp, after the arithmetic): words whose stamp is not there yet
-    // are polled from L2 one round trip at a time.
+    // Receiving side of the exchange (polling warp only): copy the neighbour's published row into shared memory as soon
+    // as every word carries this half-step's stamp.
     auto collect = [&](const uint2 *src, const uint32_t stamp, uint32_t *dst) {
         // W <= 512: at most two rounds of 8 words per lane.  The loads are unconditional (indices past the row are
         // clamped to its last word) and all eight are in flight together; a round is repeated until every word carries
