@@ -161,8 +161,8 @@ __global__ void __launch_bounds__(THREADS, MINB) half_step_i8(const __grid_const
             // one row: cq = this row, vq = vertical neighbour row, e = edge word; loads the next row into (nq, en)
             auto do_row = [&](const uint4 &cq, const uint4 &vq, const uint32_t e, uint4 &nq, uint32_t &en, const bool more) {
                 if (more) {
-                    nq = ldg128(pc + AHEAD * stride);
-                    en = ldg32(pe + AHEAD * stride);
+                    nq = ldg128(pc);                                  // pc, pe run AHEAD rows in front of the row in use
+                    en = ldg32(pe);
                 }
                 const uint32_t w[4] = {cq.x, cq.y, cq.z, cq.w};
                 const uint32_t vw[4] = {vq.x, vq.y, vq.z, vq.w};
@@ -241,6 +241,7 @@ __global__ void __launch_bounds__(THREADS, MINB) half_step_i8(const __grid_const
             // three row buffers rotate roles (vertical neighbour / current / prefetched) without register moves
             uint4 B0 = ldg128(sbase + (size_t)rh * L + c0), B1 = ldg128(pc), B2 = B1;
             uint32_t e0 = 0, e1 = ldg32(pe), e2 = 0;
+            pc += stride; pe += stride;
             if (AHEAD == 1) {
                 for (int i = 0;;) {
                     do_row(B1, B0, e1, B2, e2, i + 1 < rows); if (++i == rows) break;
@@ -251,7 +252,8 @@ __global__ void __launch_bounds__(THREADS, MINB) half_step_i8(const __grid_const
                 // four buffers: the row loaded while row i is computed is row i + 2
                 uint4 B3 = B1;
                 uint32_t e3 = 0;
-                if (rows > 1) { B2 = ldg128(pc + stride); e2 = ldg32(pe + stride); }
+                if (rows > 1) { B2 = ldg128(pc); e2 = ldg32(pe); }
+                pc += stride; pe += stride;
                 for (int i = 0;;) {
                     do_row(B1, B0, e1, B3, e3, i + 2 < rows); if (++i == rows) break;
                     do_row(B2, B1, e2, B0, e0, i + 2 < rows); if (++i == rows) break;
