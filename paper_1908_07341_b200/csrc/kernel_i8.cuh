@@ -21,7 +21,7 @@
 
 namespace shaken {
 
-enum : int { EXTRACT_PRMT = 0, EXTRACT_SMEM = 1, EXTRACT_IDP = 2, EXTRACT_PAIR = 3, PACK_ADD = 16, PREFETCH2 = 32, PER_WARP = 64 };
+enum : int { EXTRACT_PRMT = 0, EXTRACT_SMEM = 1, EXTRACT_IDP = 2, EXTRACT_PAIR = 3, PACK_ADD = 16, PREFETCH2 = 32, PER_WARP = 64, OBS_MMA = 128 };
 
 // byte the EXTRACT_SMEM encoding produces for minus flags (ms, mh, mv)
 __host__ __device__ constexpr uint32_t smem_code(int ms, int mh, int mv)
@@ -40,6 +40,12 @@ __global__ void __launch_bounds__(THREADS, MINB) half_step_i8(const __grid_const
     // of a block may work on different chains and never wait for each other (many small chains: the strips can be
     // tall and the last wave full at warp granularity).  Otherwise a task is WPB strips of one chain per block.
     constexpr bool PERWARP = (EXTRACT_ & PER_WARP) != 0;
+    // OBS_MMA: the observable sums are spin-product dot products, i.e. a (small) dense contraction: they go to the tensor
+    // cores (int8 mma.sync, otherwise idle) instead of IDP.4A, which shares the multiplier pipe with Philox's IMAD.WIDE --
+    // the one pipe this kernel is short of.  With A rows = two operand vectors of a lane group and B column g = the
+    // common factor of the same lane group, the DIAGONAL C[g][g], C[g+8][g] holds the two wanted dot products; the
+    // off-diagonal entries (products across lane groups) are ignored.  Needs all 32 lanes in the row loop.
+    constexpr bool OBSMMA = (EXTRACT_ & OBS_MMA) != 0 && (FLAGS & (F_OBS | F_BONDS)) != 0;
     static_assert(!PERWARP || EXTRACT != EXTRACT_PAIR, "the paired table (16 KiB) exists once per block");
     constexpr bool OBS = (FLAGS & F_OBS) != 0;
     constexpr bool BONDS = (FLAGS & F_BONDS) != 0;
@@ -66,8 +72,20 @@ __global__ void __launch_bounds__(THREADS, MINB) half_step_i8(const __grid_const
     int cur_chain = -1;
     ChainKeys ck = {0u, 0u};
     int cnt0 = 0, cnt1 = 0, cnt2 = 0;   // half 1: M_sigma, E_J, E_q ; half 0: M_tau, C_x, C_y
+    int acc1[4] = {0, 0, 0, 0}, acc2[4] = {0, 0, 0, 0};   // OBS_MMA accumulators (see do_row)
 
     auto flush = [&](int chain) {
+        if (OBSMMA) {
+            // lane (g, t) holds C[g][2t], C[g][2t+1], C[g+8][2t], C[g+8][2t+1]: the diagonal sits at t = g / 2
+            const int g = lane >> 2, t = lane & 3;
+            const bool diag = t == (g >> 1), odd = g & 1;
+            const int d1a = odd ? acc1[1] : acc1[0], d1b = odd ? acc1[3] : acc1[2];
+            const int d2a = odd ? acc2[1] : acc2[0], d2b = odd ? acc2[3] : acc2[2];
+            if (HALF == 1) { cnt2 = diag ? d1a : 0; cnt1 = diag ? d1b + d2a : 0; cnt0 = diag ? d2b : 0; }
+            else           { cnt1 = diag ? d1a : 0; cnt2 = diag ? d1b : 0; cnt0 = diag ? d2a : 0; }
+#pragma unroll
+            for (int i = 0; i < 4; ++i) acc1[i] = acc2[i] = 0;
+        }
         if (HALF == 1) {
             if (OBS) {
                 warp_add_to(p.rec_cur + (size_t)chain * 6 + 0, cnt0);
@@ -133,8 +151,10 @@ __global__ void __launch_bounds__(THREADS, MINB) half_step_i8(const __grid_const
         }
         const int seg = lt % p.nseg;
         const int rb = lt / p.nseg;
-        const int cv = seg * 32 + lane;
-        if (lt < tpc && cv < p.nvec) {
+        const int cvl = seg * 32 + lane;
+        const bool live = cvl < p.nvec;                  // OBS_MMA keeps dead lanes of a ragged strip in the loop (mma.sync
+        const int cv = OBSMMA ? min(cvl, p.nvec - 1) : cvl;   // is warp-wide): they recompute the last vector and contribute 0
+        if (lt < tpc && (OBSMMA || live)) {
             const int c0 = cv * 16;
             const int r_first = rb * R;
             const int r_last = min(L, r_first + R) - 1;
@@ -218,6 +238,7 @@ __global__ void __launch_bounds__(THREADS, MINB) half_step_i8(const __grid_const
                     // observables: spins are signed bytes +-1, so a sum of spin products over 4 sites is ONE
                     // signed 8-bit dot product (IDP.4A) accumulated in int32 -- exact, no masks, no flushes
                     const int s = (int)w[j], v = (int)vw[j], hh = (int)hw[j], o = (int)out;
+                    if (OBSMMA) continue;
                     if (HALF == 1) {
                         if (OBS) {
                             cnt0 = __dp4a(o, 0x01010101, cnt0);   // M_sigma  = sum sigma'_x
@@ -233,7 +254,29 @@ __global__ void __launch_bounds__(THREADS, MINB) half_step_i8(const __grid_const
                         }
                     }
                 }
-                if (UPDATE) *reinterpret_cast<uint4 *>(pd) = make_uint4(ow[0], ow[1], ow[2], ow[3]);
+                if (OBSMMA) {
+                    // words (0,1) then (2,3) of the 16-byte vector: a0/a2 = first operand vector (rows g), a1/a3 = second
+                    // operand vector (rows g+8), b0/b1 = common factor (column g); dead lanes contribute zeros
+                    const uint32_t ONES = 0x01010101u;
+                    if (HALF == 1) {
+                        const uint32_t o0 = live ? ow[0] : 0u, o1 = live ? ow[1] : 0u, o2 = live ? ow[2] : 0u, o3 = live ? ow[3] : 0u;
+                        mma_s8(acc1, w[0], vw[0], w[1], vw[1], o0, o1);       // rows g: tau_x (E_q),  rows g+8: tau_up (E_J)
+                        mma_s8(acc1, w[2], vw[2], w[3], vw[3], o2, o3);
+                        mma_s8(acc2, hw[0], ONES, hw[1], ONES, o0, o1);       // rows g: tau_right (E_J), rows g+8: 1 (M_sigma)
+                        mma_s8(acc2, hw[2], ONES, hw[3], ONES, o2, o3);
+                    } else {
+                        if (BONDS) {
+                            const uint32_t s0 = live ? w[0] : 0u, s1 = live ? w[1] : 0u, s2 = live ? w[2] : 0u, s3 = live ? w[3] : 0u;
+                            mma_s8(acc1, hw[0], vw[0], hw[1], vw[1], s0, s1);  // rows g: sigma_left (C_x), rows g+8: sigma_down (C_y)
+                            mma_s8(acc1, hw[2], vw[2], hw[3], vw[3], s2, s3);
+                        }
+                        if (OBS) {
+                            mma_s8(acc2, ONES, 0u, ONES, 0u, live ? ow[0] : 0u, live ? ow[1] : 0u);   // rows g: 1 (M_tau)
+                            mma_s8(acc2, ONES, 0u, ONES, 0u, live ? ow[2] : 0u, live ? ow[3] : 0u);
+                        }
+                    }
+                }
+                if (UPDATE && (!OBSMMA || live)) *reinterpret_cast<uint4 *>(pd) = make_uint4(ow[0], ow[1], ow[2], ow[3]);
                 pc += stride; pe += stride; pd += stride;
                 n += nstep;
             };

@@ -432,6 +432,7 @@ static cudaError_t launch_half(const shaken_ctx *ctx, const StepParams &p, int g
         case 5: half_step_i8<HALF, FLAGS, EXTRACT_PAIR | TUNED, 1, I8_THREADS><<<grid, I8_THREADS, 0, ctx->stream>>>(p); break;
         case 6: half_step_i8<HALF, FLAGS, EXTRACT_IDP | TUNED, 1, I8_THREADS><<<grid, I8_THREADS, 0, ctx->stream>>>(p); break;
         case 7: half_step_i8<HALF, FLAGS, AUTO, 2><<<grid, BLOCK_THREADS, 0, ctx->stream>>>(p); break;          // 2 x 256 threads
+        case 9: half_step_i8<HALF, FLAGS, EXTRACT_PAIR | TUNED | OBS_MMA, 1, I8_THREADS><<<grid, I8_THREADS, 0, ctx->stream>>>(p); break;
         case 8: half_step_i8<HALF, FLAGS, EXTRACT_SMEM | TUNED | PER_WARP, 1, I8_THREADS><<<grid, I8_THREADS, 0, ctx->stream>>>(p); break;
         default:
             if (ctx->perwarp) half_step_i8<HALF, FLAGS, EXTRACT_SMEM | TUNED | PER_WARP, 1, I8_THREADS><<<grid, I8_THREADS, 0, ctx->stream>>>(p);

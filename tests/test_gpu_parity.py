@@ -307,7 +307,7 @@ def test_small_lattice_path_and_generic_kernels_both_match_oracle(L, n_chains):
     o = so.Oracle(L, n_chains, seed)
     o.init(0)
     o.run_grid(J, q, 11, 3)
-    for variant in (0, 1, 2, 3, 4, 5, 6, 7, 8):
+    for variant in (0, 1, 2, 3, 4, 5, 6, 7, 8, 9):
         with shaken.Shaken(L, n_chains, seed, max_records=8) as s:
             s.set_variant(variant)
             s.init(0)
@@ -316,7 +316,7 @@ def test_small_lattice_path_and_generic_kernels_both_match_oracle(L, n_chains):
             assert_same_state(s, o, f"L={L} variant={variant}")
 
 
-@pytest.mark.parametrize("variant", [0, 1, 2, 4, 5, 6, 7, 8])
+@pytest.mark.parametrize("variant", [0, 1, 2, 4, 5, 6, 7, 8, 9])
 def test_every_int8_code_path_matches_oracle_on_a_ragged_lattice(variant):
     """L = 272: 17 vectors per row (ragged warp strip), several row blocks per chain, three chains with different
     couplings incl. a saturated table; records on some steps only, so launches with and without fused sums, the
