@@ -110,3 +110,29 @@ def test_cfg5_packed_32768_sampled_rows_and_brute_force_sums():
             assert np.array_equal(so.half_step_rows(sigma_k, w.seed, 0, J, q, t, 0, r0, n), tau_new[r0:r0 + n]), ("half0", r0)
             assert np.array_equal(so.half_step_rows(tau_new, w.seed, 0, J, q, t, 1, r0, n), sigma_new[r0:r0 + n]), ("half1", r0)
         assert np.array_equal(s.observables()[-1, 0], so.measure(sigma_new, tau_new))
+
+
+@pytest.mark.parametrize("packed", [False, True])
+def test_maximum_lattice_side_65536_sampled_rows(packed):
+    """Edge case: the largest L the library accepts (4.3e9 sites per layer; site indices reach 2^32, Philox counter word
+    0 reaches 2^30).  One recorded step from an iid start, checked on sampled row bands against the oracle (across strip
+    and wrap boundaries) and on the magnetisation sums by brute force."""
+    L, seed, J, q = 65536, 9, 0.44, 0.66
+    with shaken.Shaken(L, 1, seed, packed=packed, max_records=2) as s:
+        s.init(0)
+        sigma0 = s.get_spins(0)[0].copy()
+        for r in (0, 40000, L - 1):                       # init stream at the far end of the index range
+            n = (r * L) // 4 + (L // 4 - 1)
+            want = np.where(so.philox4x32_10((n, 0, 0, 0xFFFFFFFF), (seed, 0)) < 2**31, 1, -1)
+            assert np.array_equal(sigma0[r, L - 4:], want)
+        s.run(J, q, 1, 1)
+        tau1 = s.get_spins(1)[0]
+        for r0, n in [(0, 2), (L - 2, 2), (33333, 1), (221, 3)]:
+            assert np.array_equal(so.half_step_rows(sigma0, seed, 0, J, q, 0, 0, r0, n), tau1[r0:r0 + n]), ("half0", r0)
+        del sigma0
+        sigma1 = s.get_spins(0)[0]
+        for r0, n in [(0, 2), (L - 2, 2), (50001, 1)]:
+            assert np.array_equal(so.half_step_rows(tau1, seed, 0, J, q, 0, 1, r0, n), sigma1[r0:r0 + n]), ("half1", r0)
+        rec = s.observables()[-1, 0]
+        assert rec[0] == int(sigma1.sum(dtype=np.int64)) and rec[1] == int(tau1.sum(dtype=np.int64))
+        assert rec[3] == int((sigma1.astype(np.int16) * tau1).sum(dtype=np.int64))          # E_q
