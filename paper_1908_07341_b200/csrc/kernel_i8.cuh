@@ -102,6 +102,8 @@ __global__ void __launch_bounds__(THREADS, MINB) half_step_i8(const __grid_const
         cnt0 = cnt1 = cnt2 = 0;
     };
 
+    let_next_kernel_launch();
+    wait_for_previous_kernel();
     const long long task0 = PERWARP ? (long long)blockIdx.x * WPB + warp : (long long)blockIdx.x;
     const long long task_step = PERWARP ? (long long)gridDim.x * WPB : (long long)gridDim.x;
     for (long long bt = task0; bt < p.ntasks; bt += task_step) {

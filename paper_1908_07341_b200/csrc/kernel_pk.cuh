@@ -71,6 +71,8 @@ __global__ void __launch_bounds__(PK_THREADS, 1) half_step_pk(const __grid_const
         cnt0 = cnt1 = cnt2 = 0;
     };
 
+    let_next_kernel_launch();
+    wait_for_previous_kernel();
     for (long long bt = blockIdx.x; bt < p.ntasks; bt += gridDim.x) {
         const int chain = (int)(bt / bpc);
         const int lt = (int)(bt % bpc) * WPB + warp;

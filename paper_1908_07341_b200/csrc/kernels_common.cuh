@@ -69,6 +69,13 @@ __device__ __forceinline__ void mma_s8(int (&c)[4], uint32_t a0, uint32_t a1, ui
         : "+r"(c[0]), "+r"(c[1]), "+r"(c[2]), "+r"(c[3]) : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
 }
 
+// Programmatic dependent launch: the half-step kernels of a run are launched back to back with
+// cudaLaunchAttributeProgrammaticStreamSerialization, so the launch of kernel n+1 is processed while kernel n still runs;
+// kernel n+1 must not touch memory before kernel n has completed and flushed, which is what this waits for (a no-op
+// for a kernel launched the ordinary way).
+__device__ __forceinline__ void wait_for_previous_kernel() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void let_next_kernel_launch() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 // out ^= c if a < b (unsigned): one ISETP and one predicated LOP3
 __device__ __forceinline__ uint32_t xor_if_less(uint32_t out, uint32_t a, uint32_t b, uint32_t c)
 {

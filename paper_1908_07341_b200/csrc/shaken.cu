@@ -416,6 +416,23 @@ extern "C" int shaken_init(shaken_ctx *ctx, int mode)
 // ---------------------------------------------------------------------------------------------------
 // (a3)-(a8) the step loop
 // ---------------------------------------------------------------------------------------------------
+// launch with programmatic stream serialization (see kernels_common.cuh: wait_for_previous_kernel)
+template <typename K>
+static void launch_pdl(K kernel, int grid, int threads, cudaStream_t stream, const StepParams &p)
+{
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof(cfg));
+    cfg.gridDim = dim3((unsigned)grid);
+    cfg.blockDim = dim3((unsigned)threads);
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    cudaLaunchKernelEx(&cfg, kernel, p);
+}
+
 template <int HALF, int FLAGS>
 static cudaError_t launch_half(const shaken_ctx *ctx, const StepParams &p, int grid)
 {
@@ -424,19 +441,19 @@ static cudaError_t launch_half(const shaken_ctx *ctx, const StepParams &p, int g
     // half-steps use the paired lookup (one IDP.4A + one LDS.64 per two sites).
     constexpr int TUNED = PACK_ADD | PREFETCH2;
     constexpr int AUTO = ((FLAGS & (F_OBS | F_BONDS)) ? EXTRACT_SMEM : EXTRACT_PAIR) | TUNED;
-    if (ctx->packed) half_step_pk<HALF, FLAGS><<<grid, PK_THREADS, 0, ctx->stream>>>(p);
+    if (ctx->packed) launch_pdl(half_step_pk<HALF, FLAGS>, grid, PK_THREADS, ctx->stream, p);
     else switch (ctx->variant) {
-        case 1: half_step_i8<HALF, FLAGS, EXTRACT_PRMT | TUNED, 1, I8_THREADS><<<grid, I8_THREADS, 0, ctx->stream>>>(p); break;
-        case 2: half_step_i8<HALF, FLAGS, EXTRACT_SMEM, 2><<<grid, BLOCK_THREADS, 0, ctx->stream>>>(p); break;   // round-1 v2 kernel
-        case 4: half_step_i8<HALF, FLAGS, EXTRACT_SMEM | TUNED, 1, I8_THREADS><<<grid, I8_THREADS, 0, ctx->stream>>>(p); break;
-        case 5: half_step_i8<HALF, FLAGS, EXTRACT_PAIR | TUNED, 1, I8_THREADS><<<grid, I8_THREADS, 0, ctx->stream>>>(p); break;
-        case 6: half_step_i8<HALF, FLAGS, EXTRACT_IDP | TUNED, 1, I8_THREADS><<<grid, I8_THREADS, 0, ctx->stream>>>(p); break;
-        case 7: half_step_i8<HALF, FLAGS, AUTO, 2><<<grid, BLOCK_THREADS, 0, ctx->stream>>>(p); break;          // 2 x 256 threads
-        case 9: half_step_i8<HALF, FLAGS, EXTRACT_PAIR | TUNED | OBS_MMA, 1, I8_THREADS><<<grid, I8_THREADS, 0, ctx->stream>>>(p); break;
-        case 8: half_step_i8<HALF, FLAGS, EXTRACT_SMEM | TUNED | PER_WARP, 1, I8_THREADS><<<grid, I8_THREADS, 0, ctx->stream>>>(p); break;
+        case 1: launch_pdl(half_step_i8<HALF, FLAGS, EXTRACT_PRMT | TUNED, 1, I8_THREADS>, grid, I8_THREADS, ctx->stream, p); break;
+        case 2: launch_pdl(half_step_i8<HALF, FLAGS, EXTRACT_SMEM, 2>, grid, BLOCK_THREADS, ctx->stream, p); break;   // round-1 v2 kernel
+        case 4: launch_pdl(half_step_i8<HALF, FLAGS, EXTRACT_SMEM | TUNED, 1, I8_THREADS>, grid, I8_THREADS, ctx->stream, p); break;
+        case 5: launch_pdl(half_step_i8<HALF, FLAGS, EXTRACT_PAIR | TUNED, 1, I8_THREADS>, grid, I8_THREADS, ctx->stream, p); break;
+        case 6: launch_pdl(half_step_i8<HALF, FLAGS, EXTRACT_IDP | TUNED, 1, I8_THREADS>, grid, I8_THREADS, ctx->stream, p); break;
+        case 7: launch_pdl(half_step_i8<HALF, FLAGS, AUTO, 2>, grid, BLOCK_THREADS, ctx->stream, p); break;          // 2 x 256 threads
+        case 9: launch_pdl(half_step_i8<HALF, FLAGS, EXTRACT_PAIR | TUNED | OBS_MMA, 1, I8_THREADS>, grid, I8_THREADS, ctx->stream, p); break;
+        case 8: launch_pdl(half_step_i8<HALF, FLAGS, EXTRACT_SMEM | TUNED | PER_WARP, 1, I8_THREADS>, grid, I8_THREADS, ctx->stream, p); break;
         default:
-            if (ctx->perwarp) half_step_i8<HALF, FLAGS, EXTRACT_SMEM | TUNED | PER_WARP, 1, I8_THREADS><<<grid, I8_THREADS, 0, ctx->stream>>>(p);
-            else half_step_i8<HALF, FLAGS, AUTO, 1, I8_THREADS><<<grid, I8_THREADS, 0, ctx->stream>>>(p);
+            if (ctx->perwarp) launch_pdl(half_step_i8<HALF, FLAGS, EXTRACT_SMEM | TUNED | PER_WARP, 1, I8_THREADS>, grid, I8_THREADS, ctx->stream, p);
+            else launch_pdl(half_step_i8<HALF, FLAGS, AUTO, 1, I8_THREADS>, grid, I8_THREADS, ctx->stream, p);
             break;
     }
     return cudaGetLastError();
