@@ -347,6 +347,99 @@ int oracle_run(oracle_ctx *o, double J, double q, int64_t n_steps, int64_t obs_e
     return rc;
 }
 
+/* ------------------------------------------------------------------ */
+/* Alternate parallel heat bath on the SQUARE lattice:  */
+/* "a parallel version of the heat bath dynamics that updates,         */
+/* alternatively, the spins on the odd and the even sites of the       */
+/* lattice", whose equilibrium measure is the Gibbs measure of the     */
+/* square-lattice Ising model with coupling J.  One spin field (the    */
+/* sigma array; tau is not touched), L even.  Site (r, c) has colour   */
+/* (r + c) & 1; half-step `half` of full step t redraws every site of  */
+/* colour `half` by heat bath on h = J * (sum of its four neighbours): */
+/* +1 iff rnd < A[k], k = number of +1 neighbours, h = J (2k - 4).     */
+/* The sites of one colour, numbered m = 0, 1, ... in row-major order  */
+/* (m = (r L + c) >> 1), draw the words the shaken half-step g = 2t +  */
+/* half gives sites 0, 1, ...: word m & 3 of counter (m >> 2, chain,   */
+/* g lo, g hi).                                                        */
+/* ------------------------------------------------------------------ */
+void oracle_alt_thresholds(double J, uint32_t A[5])
+{
+    for (int k = 0; k < 5; ++k) A[k] = oracle_threshold((double)(2 * k - 4) * J);
+}
+
+/* Rows r0 .. r0+nrows-1 of the lattice after one half-step; src (L x L) is the lattice before it. */
+static void alt_half_step_rows(int64_t L, uint64_t seed, int complement, int64_t ch, const uint32_t A[5], int half,
+                               const int8_t *src, int8_t *dst_rows, uint64_t t, int64_t r0, int64_t nrows)
+{
+    uint64_t g = 2u * t + (uint64_t)half;
+    for (int64_t r = r0; r < r0 + nrows; ++r)
+        for (int64_t c = 0; c < L; ++c) {
+            int8_t out = src[r * L + c];
+            if (((r + c) & 1) == half) {
+                int k = (src[wrap(r + 1, L) * L + c] == 1) + (src[wrap(r - 1, L) * L + c] == 1) +
+                        (src[r * L + wrap(c + 1, L)] == 1) + (src[r * L + wrap(c - 1, L)] == 1);
+                uint32_t rw = rnd_word(seed, (uint32_t)ch, g, (uint64_t)(r * L + c) >> 1);
+                if (complement) rw = ~rw;
+                out = rw < A[k] ? 1 : -1;
+            }
+            dst_rows[(r - r0) * L + c] = out;
+        }
+}
+
+int oracle_alt_half_step_rows(const int8_t *src, int8_t *dst_rows, int64_t L, uint64_t seed, int64_t chain,
+                              double J, uint64_t t, int half, int64_t r0, int64_t nrows)
+{
+    if (!src || !dst_rows || L < 2 || (L & 1) || (half != 0 && half != 1) || r0 < 0 || nrows < 0 || r0 + nrows > L)
+        return ORACLE_EINVAL;
+    uint32_t A[5];
+    oracle_alt_thresholds(J, A);
+    alt_half_step_rows(L, seed, 0, chain, A, half, src, dst_rows, t, r0, nrows);
+    return ORACLE_OK;
+}
+
+/* n_steps full steps (even sites, then odd sites) of every chain with per-chain coupling J[ch].  Coupling groups and
+ * coalescence times as in oracle_run_grid.  A record after a step holds (M, 0, 0, 0, C_x, C_y) of the sigma array:
+ * H(sigma) = -J (C_x + C_y). */
+int oracle_run_alternate(oracle_ctx *o, const double *J, int64_t n_steps, int64_t obs_every)
+{
+    if (!o || !J || n_steps < 0 || obs_every < 0 || (o->L & 1)) return ORACLE_EINVAL;
+    for (int64_t ch = 0; ch < o->n_chains; ++ch)
+        if (!isfinite(J[ch])) return ORACLE_EINVAL;
+    size_t nsite = (size_t)o->L * (size_t)o->L;
+    int8_t *tmp = (int8_t *)malloc(nsite);
+    if (!tmp) return ORACLE_ENOMEM;
+    for (int64_t s = 0; s < n_steps; ++s) {
+        for (int64_t ch = 0; ch < o->n_chains; ++ch) {
+            int8_t *sg = o->sigma + (size_t)ch * nsite;
+            int64_t rng_chain = (ch / o->group) * o->group;
+            uint32_t A[5];
+            oracle_alt_thresholds(J[ch], A);
+            for (int half = 0; half < 2; ++half) {
+                alt_half_step_rows(o->L, o->seed, o->complement, rng_chain, A, half, sg, tmp, o->step, 0, o->L);
+                memcpy(sg, tmp, nsite);
+            }
+        }
+        o->step++;
+        if (o->coal)
+            for (int64_t gi = 0; gi < o->n_chains / o->group; ++gi) {
+                if (o->coal[gi] >= 0) continue;
+                const int8_t *first = o->sigma + (size_t)(gi * o->group) * nsite;
+                int same = 1;
+                for (int64_t m = 1; m < o->group && same; ++m)
+                    same = memcmp(first, first + (size_t)m * nsite, nsite) == 0;
+                if (same) o->coal[gi] = (int64_t)o->step;
+            }
+        if (obs_every > 0 && o->step % (uint64_t)obs_every == 0) {
+            int rc = push_record(o);
+            if (rc) { free(tmp); return rc; }
+            int64_t *rec = o->records + (size_t)(o->n_records - 1) * (size_t)o->n_chains * 6;
+            for (int64_t ch = 0; ch < o->n_chains; ++ch) rec[ch * 6 + 1] = rec[ch * 6 + 2] = rec[ch * 6 + 3] = 0;
+        }
+    }
+    free(tmp);
+    return ORACLE_OK;
+}
+
 /* Copy min(n_records, max_records) records, layout [record][chain][6]; returns the count. */
 int64_t oracle_observables(const oracle_ctx *o, int64_t *out, int64_t max_records)
 {

@@ -82,6 +82,13 @@ def lib():
         L.oracle_half_step_rows.restype = C.c_int
         L.oracle_diag_correlations.argtypes = [p, C.POINTER(C.c_int64), C.c_int64, C.POINTER(C.c_int64)]
         L.oracle_diag_correlations.restype = C.c_int
+        L.oracle_alt_thresholds.argtypes = [C.c_double, C.POINTER(C.c_uint32)]
+        L.oracle_alt_thresholds.restype = None
+        L.oracle_alt_half_step_rows.argtypes = [p, p, C.c_int64, C.c_uint64, C.c_int64, C.c_double, C.c_uint64, C.c_int,
+                                                C.c_int64, C.c_int64]
+        L.oracle_alt_half_step_rows.restype = C.c_int
+        L.oracle_run_alternate.argtypes = [p, C.POINTER(C.c_double), C.c_int64, C.c_int64]
+        L.oracle_run_alternate.restype = C.c_int
         L.oracle_set_coupling.argtypes = [p, C.c_int64]
         L.oracle_set_coupling.restype = C.c_int
         L.oracle_coalescence.argtypes = [p, C.POINTER(C.c_int64), C.c_int64]
@@ -132,6 +139,28 @@ def half_step_rows(src: np.ndarray, seed: int, chain: int, J: float, q: float, t
                                      float(J), float(q), int(t), int(half), int(r0), int(nrows))
     if rc:
         raise OracleError(f"oracle_half_step_rows failed: {rc}")
+    return out
+
+
+def alt_thresholds(J: float) -> np.ndarray:
+    """A[k], k = number of +1 among the four neighbours: alternate heat bath on the square lattice."""
+    t = (C.c_uint32 * 5)()
+    lib().oracle_alt_thresholds(float(J), t)
+    return np.array(list(t), dtype=np.uint32)
+
+
+def alt_half_step_rows(src: np.ndarray, seed: int, chain: int, J: float, t: int, half: int, r0: int,
+                       nrows: int) -> np.ndarray:
+    """Rows r0 .. r0+nrows-1 of the lattice after half-step ``half`` (0: even sites, 1: odd sites) of full step t of
+    the alternate dynamics, from the full L x L lattice ``src`` before it."""
+    s = np.ascontiguousarray(src, dtype=np.int8)
+    L = s.shape[-1]
+    assert s.shape == (L, L)
+    out = np.empty((nrows, L), dtype=np.int8)
+    rc = lib().oracle_alt_half_step_rows(s.ctypes.data, out.ctypes.data, L, int(seed) & 0xFFFFFFFFFFFFFFFF, int(chain),
+                                         float(J), int(t), int(half), int(r0), int(nrows))
+    if rc:
+        raise OracleError(f"oracle_alt_half_step_rows failed: {rc}")
     return out
 
 
@@ -209,6 +238,12 @@ class Oracle:
             ),
             "oracle_run_grid",
         )
+
+    def run_alternate(self, J, n_steps: int, obs_every: int = 0):
+        """Alternate (even sites, then odd sites) heat bath on the sigma array, coupling J (scalar or per chain)."""
+        Ja = np.ascontiguousarray(np.broadcast_to(np.asarray(J, dtype=np.float64), (self.n_chains,)))
+        self._ck(lib().oracle_run_alternate(self._h, Ja.ctypes.data_as(C.POINTER(C.c_double)), int(n_steps),
+                                            int(obs_every)), "oracle_run_alternate")
 
     def observables(self) -> np.ndarray:
         n = int(lib().oracle_num_records(self._h))
