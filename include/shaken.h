@@ -121,6 +121,24 @@ int shaken_run(shaken_ctx *ctx, double J, double q, int64_t n_steps, int64_t obs
 int shaken_run_grid(shaken_ctx *ctx, const double *J, const double *q, int64_t n_steps, int64_t obs_every);
 
 /*
+ * Alternate parallel heat bath on the SQUARE lattice ("a parallel version of the heat bath dynamics that
+ * updates, alternatively, the spins on the odd and the even sites of the lattice", the square-lattice equivalent of
+ * eq. (15)-(16); its equilibrium measure is the Gibbs measure of the square-lattice Ising model with coupling J).
+ * It runs on the context's sigma array alone, in place; tau is not touched.  Site (r, c) has colour (r + c) & 1.  Full
+ * step t = half-step 0 (every site of colour 0 redrawn), then half-step 1 (colour 1):
+ *     s'_x = +1  iff  rnd(x) < A[k],   k = number of +1 among the four nearest neighbours,   h = J (2k - 4),
+ *     A[k] = shaken_alt_thresholds(J)[k]  (same integer scale and mirror rule as shaken_thresholds),
+ *     rnd(x) = Philox4x32-10(key = seed, counter = (m >> 2, chain, g lo, g hi))[m & 3],  m = (r L + c) >> 1,  g = 2t + half
+ * (m numbers the sites of one colour in row-major order).  The step counter, coupling groups, coalescence times
+ * (compared on sigma) and the chain offset work as for shaken_run.  A record appended after a step holds
+ * (M, 0, 0, 0, C_x, C_y) of the sigma array: H(sigma) = -J (C_x + C_y).
+ * shaken_run_alternate_grid: J is a HOST array of n_chains doubles.  Errors as shaken_run.
+ */
+int shaken_alt_thresholds(double J, uint32_t out[5]);
+int shaken_run_alternate(shaken_ctx *ctx, double J, int64_t n_steps, int64_t obs_every);
+int shaken_run_alternate_grid(shaken_ctx *ctx, const double *J, int64_t n_steps, int64_t obs_every);
+
+/*
  * shaken_observables: wait for the stream, then copy min(n_records, max_records) records to
  *   out  HOST, layout [record][chain][6] int64 =
  *        M_sigma = sum_x sigma_x, M_tau = sum_x tau_x                      (eq. (17))

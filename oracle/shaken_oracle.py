@@ -301,7 +301,7 @@ def energy(J: float, q: float, E_J: int, E_q: int) -> float:
 
 
 # ---------------------------------------------------------------------- exact sampling
-def propp_wilson(o: "Oracle", J, q, base: int = 1 << 40, max_doublings: int = 40):
+def propp_wilson(o: "Oracle", J, q=None, base: int = 1 << 40, max_doublings: int = 40):
     """Coupling from the past (Propp & Wilson 1996, the paper's ref. [13]; "two copies of the Markov
     chain ... run with the same update function and the same sequence of random numbers", :276 "samples are drawn
     using the Propp-Wilson algorithm"), written out step by step for a context whose coupling groups are pairs.
@@ -313,16 +313,22 @@ def propp_wilson(o: "Oracle", J, q, base: int = 1 << 40, max_doublings: int = 40
     that configuration is an exact draw from the stationary measure.  All pairs are run with the same T until the last
     one has coalesced (a pair that coalesced from -T ends in the same state from any earlier start).
 
+    q = None: the alternate heat bath on the square lattice (run_alternate) in place of the shaken dynamics; :276 draws
+    the samples of that reference dynamics the same way.
+
     Returns (samples [n_pairs, L, L] int8 = sigma at time 0, T used)."""
     if getattr(o, "group", 1) != 2:
         raise ValueError("propp_wilson needs coupling groups of two (top, bottom)")
     Ja = np.ascontiguousarray(J, dtype=np.float64)
-    qa = np.ascontiguousarray(q, dtype=np.float64)
+    qa = None if q is None else np.ascontiguousarray(q, dtype=np.float64)
     T = 1
     for _ in range(max_doublings):
         o.init(2)                       # top all +1, bottom all -1; also resets the step counter ...
         o.step = base - T               # ... so the starting time -T is set afterwards
-        o.run_grid(Ja, qa, T, 0)
+        if qa is None:
+            o.run_alternate(Ja, T, 0)
+        else:
+            o.run_grid(Ja, qa, T, 0)
         if np.all(o.coalescence() >= 0):
             return o.get_spins(0)[0::2].copy(), T
         T *= 2

@@ -744,6 +744,113 @@ extern "C" int shaken_run_grid(shaken_ctx *ctx, const double *J, const double *q
 }
 
 // ---------------------------------------------------------------------------------------------------
+// alternate (even sites / odd sites) parallel heat bath on the square lattice
+// ---------------------------------------------------------------------------------------------------
+extern "C" int shaken_alt_thresholds(double J, uint32_t out[5])
+{
+    if (!out || !isfinite(J)) return fail(nullptr, SHAKEN_EINVAL, "shaken_alt_thresholds: bad argument");
+    for (int k = 0; k < 5; ++k) out[k] = threshold_of_field((double)(2 * k - 4) * J);   // h = J * (sum of 4 neighbours)
+    return SHAKEN_OK;
+}
+
+static int run_alt_impl(shaken_ctx *ctx, const double *J, bool uniform, int64_t n_steps, int64_t obs_every)
+{
+    if (n_steps < 0 || obs_every < 0) return fail(ctx, SHAKEN_EINVAL, "shaken_run_alternate: negative count");
+    const int nJ = uniform ? 1 : ctx->n_chains;
+    for (int i = 0; i < nJ; ++i)
+        if (!isfinite(J[i])) return fail(ctx, SHAKEN_EINVAL, "shaken_run_alternate: non-finite coupling for chain %d", i);
+    if (!ctx->have_spins || !ctx->d_sigma) return fail(ctx, SHAKEN_ESTATE, "shaken_run_alternate: no spins yet (call shaken_init or shaken_set_spins)");
+    int rc = ensure_device(ctx);
+    if (rc) return rc;
+    if (n_steps == 0) return SHAKEN_OK;
+    int64_t n_new = 0;
+    if (obs_every > 0) n_new = (int64_t)((ctx->step + (uint64_t)n_steps) / (uint64_t)obs_every - ctx->step / (uint64_t)obs_every);
+    if (n_new > 0) {
+        rc = grow_records(ctx, ctx->n_rec + n_new);
+        if (rc) return rc;
+    }
+
+    AltParams p;
+    memset(&p, 0, sizeof(p));
+    p.sigma = ctx->d_sigma;
+    p.L = ctx->L;
+    p.nvec = ctx->packed ? ctx->L / 32 : ctx->L / 16;
+    p.n_chains = ctx->n_chains;
+    p.chain0 = ctx->chain0;
+    p.group = ctx->group;
+    int R = 512 / p.nvec;                                        // about 16 vectors per lane and task
+    if (R < 1) R = 1;
+    if (R > ctx->L) R = ctx->L;
+    p.rows_per_task = R;
+    p.nrb = (ctx->L + R - 1) / R;
+    p.ntasks = (long long)ctx->n_chains * p.nrb;
+    if (uniform) {
+        shaken_alt_thresholds(J[0], p.utab);
+        p.gtab = nullptr;
+    } else {
+        if (!ctx->d_tab && cudaMalloc(&ctx->d_tab, (size_t)ctx->n_chains * 8 * sizeof(uint32_t)) != cudaSuccess) {
+            cudaGetLastError();
+            return fail(ctx, SHAKEN_ENOMEM, "cudaMalloc of the threshold tables failed");
+        }
+        std::vector<uint32_t> h((size_t)ctx->n_chains * 8, 0u);
+        for (int i = 0; i < ctx->n_chains; ++i) shaken_alt_thresholds(J[i], &h[(size_t)i * 8]);
+        CU(cudaMemcpyAsync(ctx->d_tab, h.data(), h.size() * sizeof(uint32_t), cudaMemcpyHostToDevice, ctx->stream));
+        CU(cudaStreamSynchronize(ctx->stream));
+        p.gtab = ctx->d_tab;
+    }
+    const int wpb = ALT_THREADS / 32;
+    long long blocks = (p.ntasks + wpb - 1) / wpb;
+    const long long cap = (long long)ctx->num_sms * 8;
+    const int grid = (int)(blocks < cap ? blocks : cap);
+    const size_t rec_stride = (size_t)ctx->n_chains * SHAKEN_N_OBS;
+
+    for (int64_t s = 0; s < n_steps; ++s) {
+        const uint64_t t = ctx->step;
+        const bool rec = obs_every > 0 && (t + 1) % (uint64_t)obs_every == 0;
+        p.rec = nullptr;
+        make_step_keys(ctx->seed, 2 * t, p.keys);
+        if (ctx->packed) alt_half<0, false, true><<<grid, ALT_THREADS, 0, ctx->stream>>>(p);
+        else alt_half<0, false, false><<<grid, ALT_THREADS, 0, ctx->stream>>>(p);
+        make_step_keys(ctx->seed, 2 * t + 1, p.keys);
+        if (rec) {
+            p.rec = ctx->d_rec + (size_t)ctx->n_rec * rec_stride;
+            if (ctx->packed) alt_half<1, true, true><<<grid, ALT_THREADS, 0, ctx->stream>>>(p);
+            else alt_half<1, true, false><<<grid, ALT_THREADS, 0, ctx->stream>>>(p);
+            ctx->n_rec++;
+        } else {
+            if (ctx->packed) alt_half<1, false, true><<<grid, ALT_THREADS, 0, ctx->stream>>>(p);
+            else alt_half<1, false, false><<<grid, ALT_THREADS, 0, ctx->stream>>>(p);
+        }
+        CU(cudaGetLastError());
+        ctx->launches += 2;
+        ctx->step = t + 1;
+        if (ctx->group > 1) {
+            const long long ng = ctx->n_chains / ctx->group;
+            const long long vpc = (long long)(shaken_spin_bytes(ctx) / 16) / ctx->n_chains;
+            unsigned long long *diff = reinterpret_cast<unsigned long long *>(ctx->d_coal + ng);
+            coalesce_compare<<<grid_for(ctx, ng * (ctx->group - 1) * vpc), 256, 0, ctx->stream>>>((const uint4 *)ctx->d_sigma, vpc, ctx->group, ng, ctx->d_coal, diff, (unsigned long long)ctx->step);
+            coalesce_finalize<<<grid_for(ctx, ng), 256, 0, ctx->stream>>>(ctx->d_coal, diff, ng, (unsigned long long)ctx->step);
+            CU(cudaGetLastError());
+            ctx->launches += 2;
+        }
+    }
+    return SHAKEN_OK;
+}
+
+extern "C" int shaken_run_alternate(shaken_ctx *ctx, double J, int64_t n_steps, int64_t obs_every)
+{
+    if (!ctx) return fail(nullptr, SHAKEN_EINVAL, "shaken_run_alternate: ctx is NULL");
+    return run_alt_impl(ctx, &J, true, n_steps, obs_every);
+}
+
+extern "C" int shaken_run_alternate_grid(shaken_ctx *ctx, const double *J, int64_t n_steps, int64_t obs_every)
+{
+    if (!ctx) return fail(nullptr, SHAKEN_EINVAL, "shaken_run_alternate_grid: ctx is NULL");
+    if (!J) return fail(ctx, SHAKEN_EINVAL, "shaken_run_alternate_grid: J is NULL");
+    return run_alt_impl(ctx, J, false, n_steps, obs_every);
+}
+
+// ---------------------------------------------------------------------------------------------------
 // (a9) records and state I/O
 // ---------------------------------------------------------------------------------------------------
 extern "C" int64_t shaken_observables(shaken_ctx *ctx, int64_t *out, int64_t max_records)

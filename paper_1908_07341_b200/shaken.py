@@ -36,6 +36,9 @@ SIGNATURES = {
     "shaken_init": (C.c_int, [_p, C.c_int]),
     "shaken_run": (C.c_int, [_p, C.c_double, C.c_double, C.c_int64, C.c_int64]),
     "shaken_run_grid": (C.c_int, [_p, _p, _p, C.c_int64, C.c_int64]),
+    "shaken_alt_thresholds": (C.c_int, [C.c_double, C.POINTER(C.c_uint32)]),
+    "shaken_run_alternate": (C.c_int, [_p, C.c_double, C.c_int64, C.c_int64]),
+    "shaken_run_alternate_grid": (C.c_int, [_p, _p, C.c_int64, C.c_int64]),
     "shaken_observables": (C.c_int64, [_p, _p, C.c_int64]),
     "shaken_num_records": (C.c_int64, [_p]),
     "shaken_clear_records": (C.c_int, [_p]),
@@ -85,6 +88,15 @@ def lib():
 
 def version() -> str:
     return lib().shaken_version().decode()
+
+
+def alt_thresholds(J: float) -> np.ndarray:
+    """Host-side integer acceptance table A[k] of the alternate dynamics (shaken_alt_thresholds)."""
+    t = (C.c_uint32 * 5)()
+    rc = lib().shaken_alt_thresholds(float(J), t)
+    if rc:
+        raise ShakenError(rc, lib().shaken_last_error(None).decode())
+    return np.array(list(t), dtype=np.uint32)
 
 
 def thresholds(J: float, q: float) -> np.ndarray:
@@ -187,6 +199,16 @@ class Shaken:
         if Ja.shape != (self.n_chains,) or qa.shape != (self.n_chains,):
             raise ValueError("J and q must have one entry per chain")
         self._ck(self._lib.shaken_run_grid(self._h, Ja.ctypes.data, qa.ctypes.data, int(n_steps), int(obs_every)))
+
+    def run_alternate(self, J, n_steps: int, obs_every: int = 0):
+        """Alternate (even sites, then odd sites) heat bath on sigma (shaken_run_alternate[_grid]); J scalar or per chain."""
+        if np.ndim(J) == 0:
+            self._ck(self._lib.shaken_run_alternate(self._h, float(J), int(n_steps), int(obs_every)))
+            return
+        Ja = np.ascontiguousarray(J, dtype=np.float64)
+        if Ja.shape != (self.n_chains,):
+            raise ValueError("J must have one entry per chain")
+        self._ck(self._lib.shaken_run_alternate_grid(self._h, Ja.ctypes.data, int(n_steps), int(obs_every)))
 
     def observables(self, max_records: Optional[int] = None, out: Optional[np.ndarray] = None) -> np.ndarray:
         n = int(self._ck(self._lib.shaken_num_records(self._h)))
