@@ -17,6 +17,8 @@
 // into half-step 1: every bond joins a site redrawn there to a passive one, so  C_x = sum_{x odd} s_x (left + right),
 // C_y = sum_{x odd} s_x (up + down)  and M is the sum of the stored vectors.
 #pragma once
+#include <type_traits>
+
 #include "kernels_common.cuh"
 
 namespace shaken {
@@ -39,6 +41,48 @@ struct AltParams {
     StepKeys keys;
 };
 
+// One int8 vector (16 sites, the 8 of parity PC redrawn).  c = {word left of the vector, its four words, word right of
+// it}; fu, fd = minus-flags of the rows above and below.  A minus-flag word has 4 in every byte whose spin is -1
+// (0xFF & 0x04) and 0 where it is +1, so the four flag words of a site's neighbours add up, without carries, to
+// 4 * (number of -1 neighbours): the byte offset of its threshold in `tab` (which is stored in that order).
+// Sums: a1 += sum of redrawn spins, ah += sum of redrawn spin * 4 * (minus among left, right), av likewise for up, down.
+__device__ __forceinline__ uint32_t minus4(uint32_t x) { return x & 0x04040404u; }
+
+template <int PC, bool OBS>
+__device__ __forceinline__ uint4 alt_vector_i8(const uint32_t (&c)[6], const uint32_t (&fu)[4], const uint32_t (&fd)[4],
+                                               const uint32_t (&rnd)[8], const uint32_t *tab, int &accM, int &a1, int &ah, int &av)
+{
+    constexpr uint32_t active = 0x00FF00FFu << (8 * PC);
+    uint32_t fc[6], out[4];
+#pragma unroll
+    for (int j = 0; j < 6; ++j) fc[j] = minus4(c[j]);
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const uint32_t fl = __funnelshift_l(fc[j], fc[j + 1], 8);         // byte b: flag of the spin left of column b
+        const uint32_t fr = __funnelshift_r(fc[j + 1], fc[j + 2], 8);     // byte b: flag of the spin right of column b
+        const uint32_t hs = fl + fr, vs = fu[j] + fd[j], nm = hs + vs;
+        uint32_t o = c[j + 1] | active;                                   // redrawn bytes start as -1 (0xFF)
+#pragma unroll
+        for (int i = 0; i < 2; ++i) {
+            constexpr uint32_t FE = 0xFEu;
+            const int b = PC + 2 * i;
+            const uint32_t off = __byte_perm(nm, 0u, 0x4440u | (uint32_t)b);
+            const uint32_t T = *reinterpret_cast<const uint32_t *>(reinterpret_cast<const char *>(tab) + off);
+            o = xor_if_less(o, rnd[2 * j + i], T, FE << (8 * b));         // 0xFF ^ 0xFE = +1
+        }
+        out[j] = o;
+        if constexpr (OBS) {
+            const uint32_t oa = o & active;
+            accM = __dp4a((int)o, 0x01010101, accM);
+            a1 = __dp4a((int)oa, 0x01010101, a1);
+            ah = __dp4a((int)oa, (int)hs, ah);
+            av = __dp4a((int)oa, (int)vs, av);
+        }
+    }
+    return make_uint4(out[0], out[1], out[2], out[3]);
+}
+
+// generic form: lanes stride over the (row, vector) pairs of a block of rows -- any L, also rows much narrower than a warp
 template <int HALF, bool OBS, bool PACKED>
 __global__ void __launch_bounds__(ALT_THREADS) alt_half(const __grid_constant__ AltParams p)
 {
@@ -46,6 +90,7 @@ __global__ void __launch_bounds__(ALT_THREADS) alt_half(const __grid_constant__ 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int L = p.L, nvec = p.nvec;
     const int wpr = PACKED ? nvec : 4 * nvec;                      // 32-bit words per row
+    const uint32_t magic = (uint32_t)(4294967296ull / (uint32_t)nvec) + 1u;   // it / nvec = umulhi(it, magic) for it * nvec < 2^32
     uint32_t *tab = s_tab[warp];
 
     for (long long task = (long long)blockIdx.x * (ALT_THREADS / 32) + warp; task < p.ntasks;
@@ -53,14 +98,16 @@ __global__ void __launch_bounds__(ALT_THREADS) alt_half(const __grid_constant__ 
         const int chain = (int)(task / p.nrb), rb = (int)(task - (long long)chain * p.nrb);
         const int r_begin = rb * p.rows_per_task, r_end = min(L, r_begin + p.rows_per_task);
         __syncwarp();
-        if (lane < 8) tab[lane] = p.gtab ? p.gtab[(size_t)chain * 8 + lane] : p.utab[lane];
+        // int8: entry i = A[4 - i], addressed by 4 * (number of -1 neighbours); packed: entry k = A[k]
+        if (lane < 5) tab[lane] = p.gtab ? p.gtab[(size_t)chain * 8 + (PACKED ? lane : 4 - lane)] : p.utab[PACKED ? lane : 4 - lane];
         __syncwarp();
         const ChainKeys ck = make_chain_keys(p.keys, p.chain0 + (uint32_t)((chain / p.group) * p.group));
         uint32_t *base = reinterpret_cast<uint32_t *>(p.sigma) + (size_t)chain * L * wpr;
-        int accM = 0, accX = 0, accY = 0;
+        int accM = 0, accX = 0, accY = 0, a1 = 0;
         const int items = (r_end - r_begin) * nvec;
         for (int it = lane; it < items; it += 32) {
-            const int r = r_begin + it / nvec, v = it - (it / nvec) * nvec;
+            const int dr = nvec == 1 ? it : (int)__umulhi((uint32_t)it, magic);
+            const int r = r_begin + dr, v = it - dr * nvec;
             uint32_t *row = base + (size_t)r * wpr;
             const uint32_t *up = base + (size_t)(r + 1 == L ? 0 : r + 1) * wpr;
             const uint32_t *dn = base + (size_t)(r == 0 ? L - 1 : r - 1) * wpr;
@@ -72,35 +119,16 @@ __global__ void __launch_bounds__(ALT_THREADS) alt_half(const __grid_constant__ 
                 const uint32_t prev = row[v == 0 ? wpr - 1 : 4 * v - 1];        // holds the spin left of the vector
                 const uint32_t next = row[v + 1 == nvec ? 0 : 4 * v + 4];       // holds the spin right of it
                 const uint32_t c[6] = {prev, c4.x, c4.y, c4.z, c4.w, next};
-                const uint32_t u[4] = {u4.x, u4.y, u4.z, u4.w}, d[4] = {d4.x, d4.y, d4.z, d4.w};
+                const uint32_t fu[4] = {minus4(u4.x), minus4(u4.y), minus4(u4.z), minus4(u4.w)};
+                const uint32_t fd[4] = {minus4(d4.x), minus4(d4.y), minus4(d4.z), minus4(d4.w)};
                 uint32_t rnd[8];
                 const uint32_t n0 = (uint32_t)r * (uint32_t)(L >> 3) + 2u * (uint32_t)v;
                 philox_site_words(n0, p.keys, ck, rnd);
                 philox_site_words(n0 + 1u, p.keys, ck, rnd + 4);
-                const uint32_t active = 0x00FF00FFu << (8 * pc);
-                uint32_t out[4];
-#pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    const uint32_t lw = __funnelshift_l(c[j], c[j + 1], 8);     // byte b = spin left of column b
-                    const uint32_t rw = __funnelshift_r(c[j + 1], c[j + 2], 8); // byte b = spin right of column b
-                    const uint32_t hsum = __vadd4(lw, rw), vsum = __vadd4(u[j], d[j]);
-                    // k = (sum of the four +-1 neighbours + 4) / 2, per byte
-                    const uint32_t kq = (__vadd4(__vadd4(hsum, vsum), 0x04040404u) >> 1) & 0x07070707u;
-                    uint32_t o = c[j + 1] & ~active;
-#pragma unroll
-                    for (int i = 0; i < 2; ++i) {
-                        const int sh = 8 * (pc + 2 * i);
-                        const uint32_t T = tab[(kq >> sh) & 7u];
-                        o |= (rnd[2 * j + i] < T ? 0x01u : 0xFFu) << sh;
-                    }
-                    out[j] = o;
-                    if constexpr (OBS) {
-                        accM = __dp4a((int)o, 0x01010101, accM);
-                        accX = __dp4a((int)(o & active), (int)hsum, accX);
-                        accY = __dp4a((int)(o & active), (int)vsum, accY);
-                    }
-                }
-                *reinterpret_cast<uint4 *>(row + 4 * v) = make_uint4(out[0], out[1], out[2], out[3]);
+                uint4 o;
+                if (pc) o = alt_vector_i8<1, OBS>(c, fu, fd, rnd, tab, accM, a1, accX, accY);
+                else o = alt_vector_i8<0, OBS>(c, fu, fd, rnd, tab, accM, a1, accX, accY);
+                *reinterpret_cast<uint4 *>(row + 4 * v) = o;
             } else {
                 const uint32_t c = row[v], a = up[v], b = dn[v];
                 const uint32_t prev = row[v == 0 ? nvec - 1 : v - 1], next = row[v + 1 == nvec ? 0 : v + 1];
@@ -133,10 +161,127 @@ __global__ void __launch_bounds__(ALT_THREADS) alt_half(const __grid_constant__ 
             }
         }
         if constexpr (OBS) {
+            if constexpr (!PACKED) {
+                // s * (l + r) = s * (2 - 2 * minus) per site: ah, av hold 4 * minus, so they are multiples of 4
+                accX = 2 * a1 - accX / 2;
+                accY = 2 * a1 - accY / 2;
+            }
             long long *rec = p.rec + (size_t)chain * 6;
             warp_add_to(rec + 0, accM);
             warp_add_to(rec + 4, accX);
             warp_add_to(rec + 5, accY);
+        }
+    }
+}
+
+// Strip form for wide int8 rows (nvec >= 32): a warp owns a strip 32 vectors wide and rows_per_task (even) rows high and
+// walks it row by row; every row is loaded once, the minus-flags of the rows above and below stay in registers (the flags
+// of a row's PASSIVE bytes do not change when the row is redrawn, and only those are read by its neighbours), and the
+// column parity of the redrawn sites is a compile-time constant of each of the two unrolled row bodies.
+// p.ntasks = n_chains * nrb * nseg with nseg = ceil(nvec / 32); rows_per_task and the first row of every task are even.
+struct AltRow {
+    uint4 c;
+    uint32_t prev, next;
+};
+
+// row = pointer to the lane's own vector of that row; off_prev / off_next = word offsets (relative to it) of the words
+// that hold the spins left and right of the vector (torus wrap included)
+__device__ __forceinline__ AltRow alt_load_row(const uint32_t *row, int off_prev, int off_next)
+{
+    AltRow x;
+    x.c = *reinterpret_cast<const uint4 *>(row);
+    x.prev = row[off_prev];
+    x.next = row[off_next];
+    return x;
+}
+
+__device__ __forceinline__ void minus4(const uint4 &x, uint32_t (&f)[4])
+{
+    f[0] = minus4(x.x); f[1] = minus4(x.y); f[2] = minus4(x.z); f[3] = minus4(x.w);
+}
+
+template <int HALF, bool OBS>
+__global__ void __launch_bounds__(ALT_THREADS, 2) alt_strip_i8(const __grid_constant__ AltParams p)
+{
+    __shared__ uint32_t s_tab[ALT_THREADS / 32][8];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int L = p.L, nvec = p.nvec, wpr = 4 * nvec;
+    const int nseg = (nvec + 31) >> 5;
+    uint32_t *tab = s_tab[warp];
+
+    for (long long task = (long long)blockIdx.x * (ALT_THREADS / 32) + warp; task < p.ntasks;
+         task += (long long)gridDim.x * (ALT_THREADS / 32)) {
+        const int per_chain = p.nrb * nseg;
+        const int chain = (int)(task / per_chain), rest = (int)(task - (long long)chain * per_chain);
+        const int rb = rest / nseg, seg = rest - rb * nseg;
+        const int r_begin = rb * p.rows_per_task, r_end = min(L, r_begin + p.rows_per_task);
+        __syncwarp();
+        if (lane < 5) tab[lane] = p.gtab ? p.gtab[(size_t)chain * 8 + 4 - lane] : p.utab[4 - lane];
+        __syncwarp();
+        const ChainKeys ck = make_chain_keys(p.keys, p.chain0 + (uint32_t)((chain / p.group) * p.group));
+        const bool live = seg * 32 + lane < nvec;
+        const int v = live ? seg * 32 + lane : nvec - 1;          // idle lanes of a ragged last strip repeat the last vector
+        uint32_t *col = reinterpret_cast<uint32_t *>(p.sigma) + (size_t)chain * L * wpr + 4 * v;   // the lane's vector of row 0
+        const int off_prev = v == 0 ? wpr - 1 : -1, off_next = v + 1 == nvec ? 4 - wpr : 4;
+        int accM = 0, a1 = 0, ah = 0, av = 0;
+
+        // rows held: r0 = row r, r1 = row r + 1, r2 = row r + 2 (the "up" of row r + 1, and the next iteration's row r);
+        // fd = minus-flags of row r - 1
+        uint32_t fd[4];
+        minus4(*reinterpret_cast<const uint4 *>(col + (size_t)(r_begin == 0 ? L - 1 : r_begin - 1) * wpr), fd);
+        uint32_t *row = col + (size_t)r_begin * wpr;             // row r
+        AltRow r0 = alt_load_row(row, off_prev, off_next);
+        AltRow r1 = alt_load_row(row + wpr, off_prev, off_next); // L even and r_begin even: rows r + 1 exists
+        const uint32_t *pa = r_begin + 2 >= L ? col : row + 2 * wpr;   // row r + 2 (mod L)
+        AltRow r2 = alt_load_row(pa, off_prev, off_next);
+        uint32_t n0 = (uint32_t)r_begin * (uint32_t)(L >> 3) + 2u * (uint32_t)v;
+        const uint32_t dn = (uint32_t)(L >> 3);
+
+        for (int r = r_begin; r < r_end; r += 2) {
+            // fetch rows r + 3 and r + 4 before computing rows r and r + 1 (not past the strip's upper halo row r_end)
+            AltRow a3, a4;
+            const bool more = r + 2 < r_end;
+            if (more) {
+                a3 = alt_load_row(pa + wpr, off_prev, off_next);               // r + 3 <= r_end - 1 < L: no wrap
+                const uint32_t *p4 = r + 4 >= L ? col : pa + 2 * wpr;
+                a4 = alt_load_row(p4, off_prev, off_next);
+                pa = p4;
+            }
+            uint32_t rnd0[8], rnd1[8];
+            philox_site_words(n0, p.keys, ck, rnd0);
+            philox_site_words(n0 + 1u, p.keys, ck, rnd0 + 4);
+            philox_site_words(n0 + dn, p.keys, ck, rnd1);
+            philox_site_words(n0 + dn + 1u, p.keys, ck, rnd1 + 4);
+            n0 += 2u * dn;
+            int m = 0, b1 = 0, bh = 0, bv = 0;
+            uint32_t f1[4], f2[4], f0[4];
+            minus4(r1.c, f1);
+            minus4(r2.c, f2);
+            minus4(r0.c, f0);
+            const uint32_t c0[6] = {r0.prev, r0.c.x, r0.c.y, r0.c.z, r0.c.w, r0.next};
+            const uint32_t c1[6] = {r1.prev, r1.c.x, r1.c.y, r1.c.z, r1.c.w, r1.next};
+            // even row r: redrawn columns have parity HALF; odd row r + 1: parity 1 - HALF
+            const uint4 o0 = alt_vector_i8<HALF, OBS>(c0, f1, fd, rnd0, tab, m, b1, bh, bv);
+            const uint4 o1 = alt_vector_i8<1 - HALF, OBS>(c1, f2, f0, rnd1, tab, m, b1, bh, bv);
+            if (live) {
+                *reinterpret_cast<uint4 *>(row) = o0;
+                *reinterpret_cast<uint4 *>(row + wpr) = o1;
+                if constexpr (OBS) { accM += m; a1 += b1; ah += bh; av += bv; }
+            }
+            row += 2 * wpr;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) fd[j] = f1[j];           // flags of the OLD row r + 1: its passive bytes are what row r + 2 reads
+            if (more) {
+                r0 = r2;
+                r1 = a3;
+                r2 = a4;
+            }
+        }
+        if constexpr (OBS) {
+            long long *rec = p.rec + (size_t)chain * 6;
+            warp_add_to(rec + 0, accM);
+            warp_add_to(rec + 4, 2 * a1 - ah / 2);
+            warp_add_to(rec + 5, 2 * a1 - av / 2);
         }
     }
 }

@@ -778,12 +778,30 @@ static int run_alt_impl(shaken_ctx *ctx, const double *J, bool uniform, int64_t 
     p.n_chains = ctx->n_chains;
     p.chain0 = ctx->chain0;
     p.group = ctx->group;
-    int R = 512 / p.nvec;                                        // about 16 vectors per lane and task
-    if (R < 1) R = 1;
-    if (R > ctx->L) R = ctx->L;
+    const bool strips = !ctx->packed && p.nvec >= 32;            // wide int8 rows: alt_strip_i8 walks column strips
+    int R;
+    if (strips) {
+        const int nseg = (p.nvec + 31) / 32;
+        // strip height: balance over the resident warps (2 blocks of 8 warps per SM) against the two halo rows per strip
+        const double warps = (double)ctx->num_sms * 2 * (ALT_THREADS / 32);
+        double best = -1.0;
+        R = 2;
+        for (int cand = 2; cand <= 256 && cand <= ctx->L; cand *= 2) {
+            const double tasks = (double)ctx->n_chains * ((ctx->L + cand - 1) / cand) * nseg;
+            const double waves = tasks / warps;
+            const double score = (waves < 1.0 ? waves : waves / ceil(waves)) * cand / (cand + 2.0);
+            if (score > best) { best = score; R = cand; }
+        }
+        p.nrb = (ctx->L + R - 1) / R;
+        p.ntasks = (long long)ctx->n_chains * p.nrb * nseg;
+    } else {
+        R = 512 / p.nvec;                                        // about 16 vectors per lane and task
+        if (R < 1) R = 1;
+        if (R > ctx->L) R = ctx->L;
+        p.nrb = (ctx->L + R - 1) / R;
+        p.ntasks = (long long)ctx->n_chains * p.nrb;
+    }
     p.rows_per_task = R;
-    p.nrb = (ctx->L + R - 1) / R;
-    p.ntasks = (long long)ctx->n_chains * p.nrb;
     if (uniform) {
         shaken_alt_thresholds(J[0], p.utab);
         p.gtab = nullptr;
@@ -800,7 +818,7 @@ static int run_alt_impl(shaken_ctx *ctx, const double *J, bool uniform, int64_t 
     }
     const int wpb = ALT_THREADS / 32;
     long long blocks = (p.ntasks + wpb - 1) / wpb;
-    const long long cap = (long long)ctx->num_sms * 8;
+    const long long cap = (long long)ctx->num_sms * (strips ? 2 : 8);
     const int grid = (int)(blocks < cap ? blocks : cap);
     const size_t rec_stride = (size_t)ctx->n_chains * SHAKEN_N_OBS;
 
@@ -810,15 +828,18 @@ static int run_alt_impl(shaken_ctx *ctx, const double *J, bool uniform, int64_t 
         p.rec = nullptr;
         make_step_keys(ctx->seed, 2 * t, p.keys);
         if (ctx->packed) alt_half<0, false, true><<<grid, ALT_THREADS, 0, ctx->stream>>>(p);
+        else if (strips) alt_strip_i8<0, false><<<grid, ALT_THREADS, 0, ctx->stream>>>(p);
         else alt_half<0, false, false><<<grid, ALT_THREADS, 0, ctx->stream>>>(p);
         make_step_keys(ctx->seed, 2 * t + 1, p.keys);
         if (rec) {
             p.rec = ctx->d_rec + (size_t)ctx->n_rec * rec_stride;
             if (ctx->packed) alt_half<1, true, true><<<grid, ALT_THREADS, 0, ctx->stream>>>(p);
+            else if (strips) alt_strip_i8<1, true><<<grid, ALT_THREADS, 0, ctx->stream>>>(p);
             else alt_half<1, true, false><<<grid, ALT_THREADS, 0, ctx->stream>>>(p);
             ctx->n_rec++;
         } else {
             if (ctx->packed) alt_half<1, false, true><<<grid, ALT_THREADS, 0, ctx->stream>>>(p);
+            else if (strips) alt_strip_i8<1, false><<<grid, ALT_THREADS, 0, ctx->stream>>>(p);
             else alt_half<1, false, false><<<grid, ALT_THREADS, 0, ctx->stream>>>(p);
         }
         CU(cudaGetLastError());
