@@ -82,6 +82,46 @@ __device__ __forceinline__ uint4 alt_vector_i8(const uint32_t (&c)[6], const uin
     return make_uint4(out[0], out[1], out[2], out[3]);
 }
 
+// Packed word: the 16 redrawn bits (parity PC) from the bit-sliced neighbour count k = s0 + 2 s1 + 4 s2.  Site j of the
+// word's redrawn sites sits at bit 2j + PC and draws rnd[j].  For q = j & 3 the four sites j = 4m + q lie in byte m at
+// bit 2q + PC, so one word W_q collects, per byte, 4 s0 + 8 s1 + 16 s2 = the byte offset of A[k] in `tab`: six
+// shift-and-mask operations serve four sites, then one PRMT, one LDS and one predicated add per site.
+template <int FROM, int TO>
+__device__ __forceinline__ uint32_t shift_bit(uint32_t x)
+{
+    if constexpr (FROM >= TO) return x >> (FROM - TO);
+    else return x << (TO - FROM);
+}
+
+template <int PC>
+__device__ __forceinline__ uint32_t alt_offsets_pk(uint32_t s0, uint32_t s1, uint32_t s2, int q)
+{
+    // bit (2q + PC) of every byte of s0, s1, s2 moved to bits 2, 3, 4 of that byte
+    switch (q) {
+        case 0: return (shift_bit<0 + PC, 2>(s0) & 0x04040404u) | (shift_bit<0 + PC, 3>(s1) & 0x08080808u) | (shift_bit<0 + PC, 4>(s2) & 0x10101010u);
+        case 1: return (shift_bit<2 + PC, 2>(s0) & 0x04040404u) | (shift_bit<2 + PC, 3>(s1) & 0x08080808u) | (shift_bit<2 + PC, 4>(s2) & 0x10101010u);
+        case 2: return (shift_bit<4 + PC, 2>(s0) & 0x04040404u) | (shift_bit<4 + PC, 3>(s1) & 0x08080808u) | (shift_bit<4 + PC, 4>(s2) & 0x10101010u);
+        default: return (shift_bit<6 + PC, 2>(s0) & 0x04040404u) | (shift_bit<6 + PC, 3>(s1) & 0x08080808u) | (shift_bit<6 + PC, 4>(s2) & 0x10101010u);
+    }
+}
+
+template <int PC>
+__device__ __forceinline__ uint32_t alt_bits_pk(uint32_t s0, uint32_t s1, uint32_t s2, const uint32_t (&rnd)[16], const uint32_t *tab)
+{
+    uint32_t nb = 0;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        const uint32_t W = alt_offsets_pk<PC>(s0, s1, s2, q);
+#pragma unroll
+        for (int m = 0; m < 4; ++m) {
+            const uint32_t off = __byte_perm(W, 0u, 0x4440u | (uint32_t)m);
+            const uint32_t T = *reinterpret_cast<const uint32_t *>(reinterpret_cast<const char *>(tab) + off);
+            nb = add_if_less(nb, rnd[4 * m + q], T, 1u << (8 * m + 2 * q + PC));
+        }
+    }
+    return nb;
+}
+
 // generic form: lanes stride over the (row, vector) pairs of a block of rows -- any L, also rows much narrower than a warp
 template <int HALF, bool OBS, bool PACKED>
 __global__ void __launch_bounds__(ALT_THREADS) alt_half(const __grid_constant__ AltParams p)
@@ -138,18 +178,10 @@ __global__ void __launch_bounds__(ALT_THREADS) alt_half(const __grid_constant__ 
                 const uint32_t ab = a & b, axb = a ^ b, lr = lw & rw, lxr = lw ^ rw;
                 const uint32_t s0 = axb ^ lxr, s1 = (ab ^ lr) ^ (axb & lxr), s2 = ab & lr;
                 const uint32_t n0 = (uint32_t)r * (uint32_t)(L >> 3) + 4u * (uint32_t)v;
-                uint32_t nb = 0;
+                uint32_t rnd[16];
 #pragma unroll
-                for (int q = 0; q < 4; ++q) {
-                    uint32_t rnd[4];
-                    philox_site_words(n0 + (uint32_t)q, p.keys, ck, rnd);
-#pragma unroll
-                    for (int i = 0; i < 4; ++i) {
-                        const int bit = 2 * (4 * q + i) + pc;
-                        const uint32_t k = ((s0 >> bit) & 1u) | (((s1 >> bit) & 1u) << 1) | (((s2 >> bit) & 1u) << 2);
-                        nb |= (rnd[i] < tab[k] ? 1u : 0u) << bit;
-                    }
-                }
+                for (int q = 0; q < 4; ++q) philox_site_words(n0 + (uint32_t)q, p.keys, ck, rnd + 4 * q);
+                const uint32_t nb = pc ? alt_bits_pk<1>(s0, s1, s2, rnd, tab) : alt_bits_pk<0>(s0, s1, s2, rnd, tab);
                 const uint32_t active = 0x55555555u << pc;
                 const uint32_t o = (c & ~active) | nb;
                 row[v] = o;
