@@ -127,6 +127,8 @@ template <int HALF, bool OBS, bool PACKED>
 __global__ void __launch_bounds__(ALT_THREADS) alt_half(const __grid_constant__ AltParams p)
 {
     __shared__ uint32_t s_tab[ALT_THREADS / 32][8];
+    let_next_kernel_launch();                                      // programmatic dependent launch (kernels_common.cuh)
+    wait_for_previous_kernel();
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int L = p.L, nvec = p.nvec;
     const int wpr = PACKED ? nvec : 4 * nvec;                      // 32-bit words per row
@@ -236,6 +238,8 @@ template <int HALF, bool OBS>
 __global__ void __launch_bounds__(ALT_THREADS, 2) alt_strip_i8(const __grid_constant__ AltParams p)
 {
     __shared__ uint32_t s_tab[ALT_THREADS / 32][8];
+    let_next_kernel_launch();                                      // programmatic dependent launch (kernels_common.cuh)
+    wait_for_previous_kernel();
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int L = p.L, nvec = p.nvec, wpr = 4 * nvec;
     const int nseg = (nvec + 31) >> 5;

@@ -417,8 +417,8 @@ extern "C" int shaken_init(shaken_ctx *ctx, int mode)
 // (a3)-(a8) the step loop
 // ---------------------------------------------------------------------------------------------------
 // launch with programmatic stream serialization (see kernels_common.cuh: wait_for_previous_kernel)
-template <typename K>
-static void launch_pdl(K kernel, int grid, int threads, cudaStream_t stream, const StepParams &p)
+template <typename K, typename P>
+static void launch_pdl(K kernel, int grid, int threads, cudaStream_t stream, const P &p)
 {
     cudaLaunchConfig_t cfg;
     memset(&cfg, 0, sizeof(cfg));
@@ -827,20 +827,20 @@ static int run_alt_impl(shaken_ctx *ctx, const double *J, bool uniform, int64_t 
         const bool rec = obs_every > 0 && (t + 1) % (uint64_t)obs_every == 0;
         p.rec = nullptr;
         make_step_keys(ctx->seed, 2 * t, p.keys);
-        if (ctx->packed) alt_half<0, false, true><<<grid, ALT_THREADS, 0, ctx->stream>>>(p);
-        else if (strips) alt_strip_i8<0, false><<<grid, ALT_THREADS, 0, ctx->stream>>>(p);
-        else alt_half<0, false, false><<<grid, ALT_THREADS, 0, ctx->stream>>>(p);
+        if (ctx->packed) launch_pdl(alt_half<0, false, true>, grid, ALT_THREADS, ctx->stream, p);
+        else if (strips) launch_pdl(alt_strip_i8<0, false>, grid, ALT_THREADS, ctx->stream, p);
+        else launch_pdl(alt_half<0, false, false>, grid, ALT_THREADS, ctx->stream, p);
         make_step_keys(ctx->seed, 2 * t + 1, p.keys);
         if (rec) {
             p.rec = ctx->d_rec + (size_t)ctx->n_rec * rec_stride;
-            if (ctx->packed) alt_half<1, true, true><<<grid, ALT_THREADS, 0, ctx->stream>>>(p);
-            else if (strips) alt_strip_i8<1, true><<<grid, ALT_THREADS, 0, ctx->stream>>>(p);
-            else alt_half<1, true, false><<<grid, ALT_THREADS, 0, ctx->stream>>>(p);
+            if (ctx->packed) launch_pdl(alt_half<1, true, true>, grid, ALT_THREADS, ctx->stream, p);
+            else if (strips) launch_pdl(alt_strip_i8<1, true>, grid, ALT_THREADS, ctx->stream, p);
+            else launch_pdl(alt_half<1, true, false>, grid, ALT_THREADS, ctx->stream, p);
             ctx->n_rec++;
         } else {
-            if (ctx->packed) alt_half<1, false, true><<<grid, ALT_THREADS, 0, ctx->stream>>>(p);
-            else if (strips) alt_strip_i8<1, false><<<grid, ALT_THREADS, 0, ctx->stream>>>(p);
-            else alt_half<1, false, false><<<grid, ALT_THREADS, 0, ctx->stream>>>(p);
+            if (ctx->packed) launch_pdl(alt_half<1, false, true>, grid, ALT_THREADS, ctx->stream, p);
+            else if (strips) launch_pdl(alt_strip_i8<1, false>, grid, ALT_THREADS, ctx->stream, p);
+            else launch_pdl(alt_half<1, false, false>, grid, ALT_THREADS, ctx->stream, p);
         }
         CU(cudaGetLastError());
         ctx->launches += 2;
