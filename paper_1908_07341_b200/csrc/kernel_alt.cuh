@@ -20,6 +20,7 @@
 #include <type_traits>
 
 #include "kernels_common.cuh"
+#include "kernel_small.cuh"
 
 namespace shaken {
 
@@ -319,6 +320,105 @@ __global__ void __launch_bounds__(ALT_THREADS, 2) alt_strip_i8(const __grid_cons
             warp_add_to(rec + 4, 2 * a1 - ah / 2);
             warp_add_to(rec + 5, 2 * a1 - av / 2);
         }
+    }
+}
+
+// Small lattices (L <= 128): one CTA per coupling group keeps the sigma arrays of its members in shared memory and ONE
+// launch advances n_steps full steps (block barrier between half-steps), as kernel_small.cuh does for the shaken
+// dynamics -- a launch per half-step would be pure launch latency here.  Every Philox call is made once per group and
+// serves all its members; the coalescence test is one block-wide vote per step; the sums of a recorded
+// step go through shared-memory atomics.  p.tau is not used.
+__host__ __device__ inline size_t alt_small_smem_bytes(int L, int G) { return (size_t)G * L * L; }
+
+__global__ void __launch_bounds__(256) alt_small_i8(const __grid_constant__ SmallParams p)
+{
+    extern __shared__ __align__(16) uint32_t smem[];
+    __shared__ uint32_t s_tab[SMALL_GROUP_MAX][8];
+    __shared__ int s_acc[SMALL_GROUP_MAX][4];
+    const int L = p.L, W = L >> 2, nvec = L >> 4, nvecs = L * nvec, G = p.group;
+    const int words = L * W;
+    const int gi = blockIdx.x, chain_first = gi * G, tid = threadIdx.x;
+    for (int m = 0; m < G; ++m) {
+        const uint32_t *gs = reinterpret_cast<const uint32_t *>(p.sigma + (size_t)(chain_first + m) * L * L);
+        for (int i = tid; i < words; i += blockDim.x) smem[m * words + i] = gs[i];
+    }
+    if (tid < G * 8) {
+        const int m = tid >> 3, i = tid & 7;
+        // entry i = A[4 - i]: addressed by 4 * (number of -1 neighbours), see alt_vector_i8
+        s_tab[m][i] = i < 5 ? (p.gtab ? p.gtab[(size_t)(chain_first + m) * 8 + 4 - i] : p.utab[4 - i]) : 0u;
+        if (i < 4) s_acc[m][i] = 0;
+    }
+    __syncthreads();
+
+    bool coalesced = p.coal ? p.coal[gi] >= 0 : true;   // block-uniform
+    long long nrec = 0;
+    for (long long s = 0; s < p.n_steps; ++s) {
+        const unsigned long long t = p.t0 + (unsigned long long)s;
+        const bool rec = p.obs_every > 0 && (t + 1) % (unsigned long long)p.obs_every == 0;
+#pragma unroll 1
+        for (int half = 0; half < 2; ++half) {
+            uint32_t xa2, xb0;
+            ChainKeys ck;
+            device_half_step_keys(p.keys, 2ull * t + (unsigned)half, p.chain0 + (uint32_t)chain_first, xa2, xb0, ck);
+            const bool sums = rec && half == 1;
+#pragma unroll 1
+            for (int c = tid; c < nvecs; c += blockDim.x) {
+                const int r = c / nvec, v = c - r * nvec;
+                uint32_t rnd[8];
+                const uint32_t n0 = (uint32_t)(r * (L >> 3) + 2 * v);
+                philox_site_words(n0, p.keys, xa2, xb0, ck, rnd);
+                philox_site_words(n0 + 1u, p.keys, xa2, xb0, ck, rnd + 4);
+                const int at = r * W + 4 * v;
+                const int au = (r + 1 == L ? 0 : r + 1) * W + 4 * v, ad = (r == 0 ? L - 1 : r - 1) * W + 4 * v;
+                const int ap = r * W + (v == 0 ? W - 1 : 4 * v - 1), an = r * W + (v + 1 == nvec ? 0 : 4 * v + 4);
+                const int pc = (r + half) & 1;
+#pragma unroll 1
+                for (int m = 0; m < G; ++m) {
+                    uint32_t *sg = smem + m * words;
+                    const uint4 c4 = *reinterpret_cast<const uint4 *>(sg + at);
+                    const uint32_t cw[6] = {sg[ap], c4.x, c4.y, c4.z, c4.w, sg[an]};
+                    uint32_t fu[4], fd[4];
+                    minus4(*reinterpret_cast<const uint4 *>(sg + au), fu);
+                    minus4(*reinterpret_cast<const uint4 *>(sg + ad), fd);
+                    int mM = 0, b1 = 0, bh = 0, bv = 0;
+                    uint4 o;
+                    if (sums) o = pc ? alt_vector_i8<1, true>(cw, fu, fd, rnd, s_tab[m], mM, b1, bh, bv) : alt_vector_i8<0, true>(cw, fu, fd, rnd, s_tab[m], mM, b1, bh, bv);
+                    else o = pc ? alt_vector_i8<1, false>(cw, fu, fd, rnd, s_tab[m], mM, b1, bh, bv) : alt_vector_i8<0, false>(cw, fu, fd, rnd, s_tab[m], mM, b1, bh, bv);
+                    *reinterpret_cast<uint4 *>(sg + at) = o;
+                    if (sums) {
+                        atomicAdd(&s_acc[m][0], mM);
+                        atomicAdd(&s_acc[m][1], 2 * b1 - bh / 2);
+                        atomicAdd(&s_acc[m][2], 2 * b1 - bv / 2);
+                    }
+                }
+            }
+            __syncthreads();
+        }
+        if (!coalesced) {                                 // T = min{n : X_n = Y_n}, in full steps
+            uint32_t diff = 0;
+            for (int i = tid; i < (G - 1) * words; i += blockDim.x) {
+                const int m = 1 + i / words, w = i - (m - 1) * words;
+                diff |= smem[w] ^ smem[m * words + w];
+            }
+            if (!__syncthreads_or(diff != 0)) {
+                coalesced = true;
+                if (tid == 0) p.coal[gi] = (long long)(t + 1);
+            }
+        }
+        if (rec) {
+            if (tid < G) {
+                long long *out = p.rec + ((size_t)nrec * p.n_chains + chain_first + tid) * 6;
+                out[0] = s_acc[tid][0];
+                out[4] = s_acc[tid][1];
+                out[5] = s_acc[tid][2];
+                s_acc[tid][0] = s_acc[tid][1] = s_acc[tid][2] = 0;   // next used after the barrier of a later half-step
+            }
+            ++nrec;
+        }
+    }
+    for (int m = 0; m < G; ++m) {
+        uint32_t *gs = reinterpret_cast<uint32_t *>(p.sigma + (size_t)(chain_first + m) * L * L);
+        for (int i = tid; i < words; i += blockDim.x) gs[i] = smem[m * words + i];
     }
 }
 

@@ -816,6 +816,36 @@ static int run_alt_impl(shaken_ctx *ctx, const double *J, bool uniform, int64_t 
         CU(cudaStreamSynchronize(ctx->stream));
         p.gtab = ctx->d_tab;
     }
+    // small lattices: one CTA per coupling group, sigma in shared memory, the whole run in one launch
+    if (!ctx->packed && ctx->variant == 0 && ctx->L <= SMALL_L_MAX && ctx->group <= SMALL_GROUP_MAX) {
+        SmallParams sp;
+        memset(&sp, 0, sizeof(sp));
+        sp.sigma = (uint8_t *)ctx->d_sigma;
+        sp.tau = nullptr;
+        sp.L = ctx->L;
+        sp.n_chains = ctx->n_chains;
+        sp.group = ctx->group;
+        sp.coal = ctx->group > 1 ? ctx->d_coal : nullptr;
+        sp.chain0 = ctx->chain0;
+        sp.t0 = ctx->step;
+        sp.n_steps = n_steps;
+        sp.obs_every = obs_every;
+        sp.rec = ctx->d_rec ? ctx->d_rec + (size_t)ctx->n_rec * ctx->n_chains * SHAKEN_N_OBS : nullptr;
+        sp.gtab = p.gtab;
+        memcpy(sp.utab, p.utab, sizeof(sp.utab));
+        make_step_keys(ctx->seed, 0, sp.keys);
+        const int nvecs = ctx->L * ctx->L / 16;
+        const int threads = nvecs >= 256 ? 256 : ((nvecs + 31) / 32) * 32;
+        const size_t smem = alt_small_smem_bytes(ctx->L, ctx->group);
+        if (smem > 40 * 1024) CU(cudaFuncSetAttribute(alt_small_i8, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        alt_small_i8<<<ctx->n_chains / ctx->group, threads, smem, ctx->stream>>>(sp);
+        CU(cudaGetLastError());
+        ctx->launches++;
+        ctx->step += (uint64_t)n_steps;
+        ctx->n_rec += n_new;
+        return SHAKEN_OK;
+    }
+
     const int wpb = ALT_THREADS / 32;
     long long blocks = (p.ntasks + wpb - 1) / wpb;
     const long long cap = (long long)ctx->num_sms * (strips ? 2 : 8);

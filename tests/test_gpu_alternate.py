@@ -39,6 +39,28 @@ def test_alternate_runs_match_oracle_bit_for_bit(L, n_chains, packed, J, init, s
         assert np.array_equal(s.observables(), o.observables()), "records differ"
 
 
+@pytest.mark.parametrize("L,n_chains,group", [(16, 3, 1), (32, 6, 2), (64, 2, 1), (128, 3, 3), (48, 8, 4)])
+def test_alternate_small_lattice_path_and_per_half_step_kernels_agree_with_oracle(L, n_chains, group):
+    """L <= 128 runs in one launch with sigma in shared memory (alt_small_i8); variant 3 forces the per-half-step
+    kernels.  Both against the oracle, with per-chain couplings, records every other step and coalescence times."""
+    seed, steps = 900 + L, 25
+    J = np.repeat(np.linspace(0.15, 0.5, n_chains // group), group)
+    o = so.Oracle(L, n_chains, seed)
+    o.set_coupling(group)
+    o.init(2 if group > 1 else 0)
+    o.run_alternate(J, steps, 2)
+    for variant in (0, 3):
+        with shaken.Shaken(L, n_chains, seed, max_records=steps) as s:
+            s.set_variant(variant)
+            s.set_coupling(group)
+            s.init(shaken.INIT_SANDWICH if group > 1 else 0)
+            s.run_alternate(J, 10, 2)
+            s.run_alternate(J, steps - 10, 2)
+            assert np.array_equal(s.get_spins(0), o.get_spins(0)), variant
+            assert np.array_equal(s.observables(), o.observables()), variant
+            assert np.array_equal(s.coalescence(), o.coalescence()), variant
+
+
 def test_alternate_grid_of_couplings_resume_and_chain_offset():
     L, n_chains, seed = 80, 5, 41
     J = np.array([0.1, 0.3, 0.44, 0.6, 0.9])
