@@ -52,6 +52,9 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--variant", type=int, default=0)
+    ap.add_argument("--dynamics", default="shaken", choices=["shaken", "alternate"],
+                    help="alternate: the even/odd heat bath on the square lattice (PAPER.md:276) on the same lattice, "
+                         "chains, J and record cadence as the named workload; a step redraws every site once")
     return ap.parse_args()
 
 
@@ -119,10 +122,14 @@ class ClockSampler:
 
 
 # ----------------------------------------------------------------------------------------- reference arm = oracle
-def oracle_sample_step(w, src, band_rows):
+def oracle_sample_step(w, src, band_rows, alternate=False):
     """One bounded 'step' of the oracle: both half-steps of `band_rows` rows of chain 0 of the workload."""
     from oracle import shaken_oracle as so
 
+    if alternate:
+        a = so.alt_half_step_rows(src, w.seed, 0, w.J[0], 0, 0, 0, band_rows)
+        b = so.alt_half_step_rows(src, w.seed, 0, w.J[0], 0, 1, 0, band_rows)
+        return a, b
     a = so.half_step_rows(src, w.seed, 0, w.J[0], w.q[0], 0, 0, 0, band_rows)
     b = so.half_step_rows(src, w.seed, 0, w.J[0], w.q[0], 0, 1, 0, band_rows)
     return a, b
@@ -140,20 +147,23 @@ def run_reference(args):
     band = max(1, min(L, (8 << 20) // L))                 # ~8 Mi sites per half-step
     src = np.ones((L, L), dtype=np.int8) if w.init == 1 else np.where(
         np.random.default_rng(w.seed).integers(0, 2, size=(L, L)) == 1, 1, -1).astype(np.int8)
+    alt = args.dynamics == "alternate"
+    per_step = (1 if alt else 2) * band * L                # alternate: each half-step redraws half the sites of the band
     for _ in range(max(args.warmup, 1)):
-        oracle_sample_step(w, src, band)
+        oracle_sample_step(w, src, band, alt)
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        oracle_sample_step(w, src, band)
+        oracle_sample_step(w, src, band, alt)
     dt = time.perf_counter() - t0
-    updates = 2.0 * band * L * args.steps
+    updates = float(per_step) * args.steps
     v = updates / (dt * 1e9)
-    sample = f"{band} rows x {L} columns of one chain, both half-steps, per step ({2 * band * L} site updates)"
+    sample = f"{band} rows x {L} columns of one chain, both half-steps, per step ({per_step} site updates)"
     line = {
         "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "int8", "data": "synthetic",
-        "config": {"workload": w.name, "L": L, "n_chains": w.n_chains, "note": "oracle/shaken_oracle.c on host cores, bounded sample per step"},
+        "config": {"workload": w.name, "L": L, "n_chains": w.n_chains, "dynamics": args.dynamics,
+                   "note": "oracle/shaken_oracle.c on host cores, bounded sample per step"},
         "cpu_baseline": {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
         "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -162,7 +172,7 @@ def run_reference(args):
     return 0
 
 
-def cpu_baseline(w):
+def cpu_baseline(w, alternate=False):
     """The oracle as it stands, single thread, about 10-30 s of work on the same workload shape."""
     from oracle import shaken_oracle as so
 
@@ -170,17 +180,21 @@ def cpu_baseline(w):
     L = w.L
     band = max(1, min(L, (256 << 20) // L))               # up to 256 Mi sites per half-step
     src = np.ones((L, L), dtype=np.int8)
-    so.half_step_rows(src, w.seed, 0, w.J[0], w.q[0], 0, 0, 0, min(band, 64))   # warm the code path
+    oracle_sample_step(w, src, min(band, 64), alternate)   # warm the code path
     t0 = time.perf_counter()
     reps = 0
     while True:                                            # whole half-step pairs until about 12 s of CPU work
-        so.half_step_rows(src, w.seed, 0, w.J[0], w.q[0], reps, 0, 0, band)
-        so.half_step_rows(src, w.seed, 0, w.J[0], w.q[0], reps, 1, 0, band)
+        if alternate:
+            so.alt_half_step_rows(src, w.seed, 0, w.J[0], reps, 0, 0, band)
+            so.alt_half_step_rows(src, w.seed, 0, w.J[0], reps, 1, 0, band)
+        else:
+            so.half_step_rows(src, w.seed, 0, w.J[0], w.q[0], reps, 0, 0, band)
+            so.half_step_rows(src, w.seed, 0, w.J[0], w.q[0], reps, 1, 0, band)
         reps += 1
         dt = time.perf_counter() - t0
         if dt >= 12.0 or reps >= 64:
             break
-    upd = 2.0 * band * L * reps
+    upd = (1.0 if alternate else 2.0) * band * L * reps
     return {"value": upd / (dt * 1e9), "unit": UNIT, "cores": 1, "kind": "oracle",
             "sample": f"{reps} x both half-steps of {band} rows x {L} columns of chain 0 ({int(upd)} site updates, {dt:.1f} s)",
             "host_cores_available": os.cpu_count()}
@@ -218,8 +232,12 @@ def run_ours(args):
     J, q = w.J_array(), w.q_array()
     uniform = len(set(w.J)) == 1 and len(set(w.q)) == 1
 
+    alt = args.dynamics == "alternate"
+
     def run(n):
-        if uniform:
+        if alt:
+            s.run_alternate(w.J[0] if uniform else J, n, w.obs_every)
+        elif uniform:
             s.run(w.J[0], w.q[0], n, w.obs_every)
         else:
             s.run_grid(J, q, n, w.obs_every)
@@ -258,7 +276,7 @@ def run_ours(args):
         ms = float(t.item())
         dist.barrier()
 
-    updates_per_rank = 2.0 * n_local * w.L * w.L * K
+    updates_per_rank = (1.0 if alt else 2.0) * n_local * w.L * w.L * K   # alternate: a half-step redraws one colour
     value = world * updates_per_rank / (ms * 1e6)
 
     # ------------------------------------------------------------------ e2e through the C ABI with host buffers
@@ -308,6 +326,10 @@ def run_ours(args):
     bytes_per_update = 0.25 if w.packed else 2.0
     n_half_launches = 2 * K
     sites_per_launch = n_local * w.L * w.L
+    if alt:
+        # in place on one array: a launch reads and writes the whole array to redraw half of its sites
+        bytes_per_update *= 2.0
+        sites_per_launch //= 2
     alg_bytes_per_launch = bytes_per_update * sites_per_launch
     avg_launch_ms = ms / n_half_launches                   # the trailing bond-sum launch (1 of 2K+1) is inside ms
     hbm_achieved = alg_bytes_per_launch / (avg_launch_ms * 1e-3) / 1e9
@@ -315,7 +337,7 @@ def run_ours(args):
     tpath = os.path.join(ROOT, "profiles", "traffic.txt")
     if os.path.exists(tpath):
         try:
-            traffic = json.load(open(tpath)).get(w.name)
+            traffic = json.load(open(tpath)).get(w.name + ("_alt" if alt else ""))
         except Exception:
             traffic = None
     props = torch.cuda.get_device_properties(dev)
@@ -328,7 +350,7 @@ def run_ours(args):
                 "traffic": traffic,
                 "peak_source": "derived (DESIGN.md Rooflines): %d SMs x 4 SMSP x 8 wide multiplies/clk x %.0f MHz; 4.5 IMAD.WIDE per site-update"
                                % (props.multi_processor_count, sm_max_mhz),
-                "kernel": "half_step_pk" if w.packed else "half_step_i8",
+                "kernel": ("alt_half (packed)" if w.packed else "alt_strip_i8") if alt else ("half_step_pk" if w.packed else "half_step_i8"),
                 "algorithmic_ops_per_launch": MULS_PER_SITE * sites_per_launch,
                 "algorithmic_bytes_per_launch": alg_bytes_per_launch, "avg_launch_us": avg_launch_ms * 1e3,
                 "peak_site_updates_per_ns": alu_peak / MULS_PER_SITE,
@@ -339,8 +361,8 @@ def run_ours(args):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "u32 bit-packed" if w.packed else "int8", "data": "synthetic",
-        "config": {"workload": w.name, "L": w.L, "n_chains_per_gpu": n_local, "J": w.J[0] if uniform else "grid",
-                   "q": w.q[0] if uniform else "grid", "obs_every": w.obs_every, "init": w.init, "seed": w.seed,
+        "config": {"workload": w.name, "dynamics": args.dynamics, "L": w.L, "n_chains_per_gpu": n_local, "J": w.J[0] if uniform else "grid",
+                   "q": (w.q[0] if uniform else "grid") if not alt else None, "obs_every": w.obs_every, "init": w.init, "seed": w.seed,
                    "l2": "inputs larger than L2 (2 x %.0f MB per step)" % (shaken_bytes(w) / 1e6) if shaken_bytes(w) > 126e6
                          else "working set fits L2 (launch/latency-bound regime)",
                    "parallelism": "replicas (independent chains, no collective)" if world > 1 else "single GPU"},
@@ -350,7 +372,7 @@ def run_ours(args):
         "roofline": roofline,
     }
     if not args.no_cpu_baseline and world == 1:
-        line["cpu_baseline"] = cpu_baseline(w)
+        line["cpu_baseline"] = cpu_baseline(w, alt)
     elif world > 1:
         line["cpu_baseline"] = None
     print(json.dumps(line))
