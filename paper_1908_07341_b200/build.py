@@ -17,7 +17,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libshaken.so")
 SOURCES = [os.path.join(CSRC, "shaken.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("kernels.cuh", "kernels_common.cuh", "kernel_i8.cuh", "kernel_pk.cuh", "kernel_small.cuh", "kernel_band.cuh", "philox.cuh")] + [os.path.join(ROOT, "include", "shaken.h")]
+DEPS = SOURCES + sorted(os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith(".cuh")) + [os.path.join(ROOT, "include", "shaken.h")]
 
 NVCC_FLAGS = [
     "-O3", "-std=c++17",
