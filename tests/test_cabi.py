@@ -51,6 +51,10 @@ def test_create_validates_arguments_without_a_device():
     assert lib.shaken_run(h, 0.5, 0.5, -1, 0) == shaken.EINVAL
     assert lib.shaken_run(h, 0.5, 0.5, 1, 0) == shaken.ESTATE
     assert b"no spins" in lib.shaken_last_error(h)
+    assert lib.shaken_run_alternate(h, float("inf"), 1, 0) == shaken.EINVAL
+    assert lib.shaken_run_alternate(h, 0.3, 1, -2) == shaken.EINVAL
+    assert lib.shaken_run_alternate(h, 0.3, 1, 0) == shaken.ESTATE
+    assert lib.shaken_run_alternate_grid(h, None, 1, 0) == shaken.EINVAL
     assert lib.shaken_bind(h, None, None, None, 0, None) == shaken.EINVAL
     assert lib.shaken_destroy(h) == 0
     assert lib.shaken_create(C.byref(h), 64, 2, 1, 1) == 0

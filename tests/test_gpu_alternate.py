@@ -144,3 +144,35 @@ def test_alternate_full_size_rows_against_the_oracle():
             assert rec[0, ch, 4] == int((x * np.roll(x, -1, 1)).sum(dtype=np.int64))
             assert rec[0, ch, 5] == int((x * np.roll(x, -1, 0)).sum(dtype=np.int64))
             assert np.all(rec[0, :, 1:4] == 0)
+
+
+def test_alternate_error_paths_and_bookkeeping():
+    with shaken.Shaken(32, 2, 1, max_records=3) as s:
+        s.init(1)
+        for bad in (float("nan"), float("inf")):
+            with pytest.raises(shaken.ShakenError) as ei:
+                s.run_alternate(bad, 1, 0)
+            assert ei.value.code == shaken.EINVAL
+        with pytest.raises(shaken.ShakenError):
+            s.run_alternate(0.3, -1, 0)
+        with pytest.raises(ValueError):
+            s.run_alternate([0.3, 0.3, 0.3], 1, 0)                  # one J per chain
+        assert s.step == 0 and s.observables().shape[0] == 0        # nothing ran
+        s.run_alternate(0.3, 0, 1)
+        assert s.step == 0
+        l0 = s.launch_count
+        s.run_alternate(0.3, 7, 3)                                  # records after global steps 3 and 6
+        assert s.step == 7 and s.observables().shape[0] == 2 and s.launch_count == l0 + 1
+        rec = s.observables()
+        assert np.all(np.abs(rec[:, :, 0]) <= 32 * 32) and np.all(rec[:, :, 0] % 2 == 0)
+        s.run_alternate(20.0, 2, 2)                                 # step 8 is recorded
+        assert s.observables().shape[0] == 3
+        before = s.get_spins(0).copy()
+        with pytest.raises(shaken.ShakenError) as ei:
+            s.run_alternate(0.3, 1, 1)                              # bound record buffer (3 records) is full
+        assert ei.value.code == shaken.ENOSPC
+        assert s.step == 9 and np.array_equal(s.get_spins(0), before)
+    with shaken.Shaken(32, 1, 1, max_records=3) as s:               # all +1 at J = 20 stays all +1: M = L^2, C_x = C_y = L^2
+        s.init(1)
+        s.run_alternate(20.0, 3, 1)
+        assert np.array_equal(s.observables()[:, 0], np.tile([1024, 0, 0, 0, 1024, 1024], (3, 1)))
