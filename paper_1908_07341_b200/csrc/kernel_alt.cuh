@@ -262,56 +262,126 @@ __global__ void __launch_bounds__(ALT_THREADS, 2) alt_strip_i8(const __grid_cons
         const int off_prev = v == 0 ? wpr - 1 : -1, off_next = v + 1 == nvec ? 4 - wpr : 4;
         int accM = 0, a1 = 0, ah = 0, av = 0;
 
-        // rows held: r0 = row r, r1 = row r + 1, r2 = row r + 2 (the "up" of row r + 1, and the next iteration's row r);
-        // fd = minus-flags of row r - 1
-        uint32_t fd[4];
-        minus4(*reinterpret_cast<const uint4 *>(col + (size_t)(r_begin == 0 ? L - 1 : r_begin - 1) * wpr), fd);
-        uint32_t *row = col + (size_t)r_begin * wpr;             // row r
-        AltRow r0 = alt_load_row(row, off_prev, off_next);
-        AltRow r1 = alt_load_row(row + wpr, off_prev, off_next); // L even and r_begin even: rows r + 1 exists
-        const uint32_t *pa = r_begin + 2 >= L ? col : row + 2 * wpr;   // row r + 2 (mod L)
-        AltRow r2 = alt_load_row(pa, off_prev, off_next);
-        uint32_t n0 = (uint32_t)r_begin * (uint32_t)(L >> 3) + 2u * (uint32_t)v;
-        const uint32_t dn = (uint32_t)(L >> 3);
+        // Two schedules of the same walk, chosen by measurement (profiles/r1c_ncu_alt_cfg4.md): the launch with the sums
+        // is 12 % faster when the vectors are fetched two trips ahead (its memory stalls go from 2.7 to 0.3 per issued
+        // instruction); the plain launch is limited by issue slots, and the same change costs it 6 % in extra instructions.
+        if constexpr (OBS) {
+            // rows held: r0 = row r, r1 = row r + 1, r2 = row r + 2 (the "up" of row r + 1, and the next trip's row r);
+            // n3, n4 = the vectors of rows r + 3, r + 4, fetched a trip ago; fd = minus-flags of row r - 1.
+            // Every trip fetches the vectors of rows r + 5, r + 6 (two trips ahead: DRAM latency) and the edge words of rows
+            // r + 3, r + 4 (one trip ahead: their lines are in L1 or L2 by now).  Nothing is fetched past the halo row r_end.
+            // Only the halo row can be row L (= row 0): rows at odd distance from r are odd and L is even.
+            uint32_t fd[4];
+            minus4(*reinterpret_cast<const uint4 *>(col + (size_t)(r_begin == 0 ? L - 1 : r_begin - 1) * wpr), fd);
+            uint32_t *row = col + (size_t)r_begin * wpr;             // row r
+            AltRow r0 = alt_load_row(row, off_prev, off_next);
+            AltRow r1 = alt_load_row(row + wpr, off_prev, off_next); // L even and r_begin even: rows r + 1 exists
+            AltRow r2 = alt_load_row(r_begin + 2 == L ? col : row + 2 * wpr, off_prev, off_next);
+            uint4 n3 = make_uint4(0, 0, 0, 0), n4 = n3;
+            if (r_begin + 2 < r_end) {
+                n3 = *reinterpret_cast<const uint4 *>(row + 3 * wpr);
+                n4 = *reinterpret_cast<const uint4 *>(r_begin + 4 == L ? col : row + 4 * wpr);
+            }
+            uint32_t n0 = (uint32_t)r_begin * (uint32_t)(L >> 3) + 2u * (uint32_t)v;
+            const uint32_t dn = (uint32_t)(L >> 3);
 
-        for (int r = r_begin; r < r_end; r += 2) {
-            // fetch rows r + 3 and r + 4 before computing rows r and r + 1 (not past the strip's upper halo row r_end)
-            AltRow a3, a4;
-            const bool more = r + 2 < r_end;
-            if (more) {
-                a3 = alt_load_row(pa + wpr, off_prev, off_next);               // r + 3 <= r_end - 1 < L: no wrap
-                const uint32_t *p4 = r + 4 >= L ? col : pa + 2 * wpr;
-                a4 = alt_load_row(p4, off_prev, off_next);
-                pa = p4;
+            for (int r = r_begin; r < r_end; r += 2) {
+                const bool more = r + 2 < r_end, more2 = r + 4 < r_end;
+                uint4 m5 = make_uint4(0, 0, 0, 0), m6 = m5;
+                uint32_t e3p = 0, e3n = 0, e4p = 0, e4n = 0;
+                if (more2) {
+                    m5 = *reinterpret_cast<const uint4 *>(row + 5 * wpr);
+                    m6 = *reinterpret_cast<const uint4 *>(r + 6 == L ? col : row + 6 * wpr);
+                }
+                if (more) {
+                    const uint32_t *p3 = row + 3 * wpr, *p4 = r + 4 == L ? col : row + 4 * wpr;
+                    e3p = p3[off_prev]; e3n = p3[off_next];
+                    e4p = p4[off_prev]; e4n = p4[off_next];
+                }
+                uint32_t rnd0[8], rnd1[8];
+                philox_site_words(n0, p.keys, ck, rnd0);
+                philox_site_words(n0 + 1u, p.keys, ck, rnd0 + 4);
+                philox_site_words(n0 + dn, p.keys, ck, rnd1);
+                philox_site_words(n0 + dn + 1u, p.keys, ck, rnd1 + 4);
+                n0 += 2u * dn;
+                int m = 0, b1 = 0, bh = 0, bv = 0;
+                uint32_t f1[4], f2[4], f0[4];
+                minus4(r1.c, f1);
+                minus4(r2.c, f2);
+                minus4(r0.c, f0);
+                const uint32_t c0[6] = {r0.prev, r0.c.x, r0.c.y, r0.c.z, r0.c.w, r0.next};
+                const uint32_t c1[6] = {r1.prev, r1.c.x, r1.c.y, r1.c.z, r1.c.w, r1.next};
+                // even row r: redrawn columns have parity HALF; odd row r + 1: parity 1 - HALF
+                const uint4 o0 = alt_vector_i8<HALF, OBS>(c0, f1, fd, rnd0, tab, m, b1, bh, bv);
+                const uint4 o1 = alt_vector_i8<1 - HALF, OBS>(c1, f2, f0, rnd1, tab, m, b1, bh, bv);
+                if (live) {
+                    *reinterpret_cast<uint4 *>(row) = o0;
+                    *reinterpret_cast<uint4 *>(row + wpr) = o1;
+                    if constexpr (OBS) { accM += m; a1 += b1; ah += bh; av += bv; }
+                }
+                row += 2 * wpr;
+    #pragma unroll
+                for (int j = 0; j < 4; ++j) fd[j] = f1[j];           // flags of the OLD row r + 1: its passive bytes are what row r + 2 reads
+                if (more) {
+                    r0 = r2;
+                    r1.c = n3; r1.prev = e3p; r1.next = e3n;
+                    r2.c = n4; r2.prev = e4p; r2.next = e4n;
+                    n3 = m5;
+                    n4 = m6;
+                }
             }
-            uint32_t rnd0[8], rnd1[8];
-            philox_site_words(n0, p.keys, ck, rnd0);
-            philox_site_words(n0 + 1u, p.keys, ck, rnd0 + 4);
-            philox_site_words(n0 + dn, p.keys, ck, rnd1);
-            philox_site_words(n0 + dn + 1u, p.keys, ck, rnd1 + 4);
-            n0 += 2u * dn;
-            int m = 0, b1 = 0, bh = 0, bv = 0;
-            uint32_t f1[4], f2[4], f0[4];
-            minus4(r1.c, f1);
-            minus4(r2.c, f2);
-            minus4(r0.c, f0);
-            const uint32_t c0[6] = {r0.prev, r0.c.x, r0.c.y, r0.c.z, r0.c.w, r0.next};
-            const uint32_t c1[6] = {r1.prev, r1.c.x, r1.c.y, r1.c.z, r1.c.w, r1.next};
-            // even row r: redrawn columns have parity HALF; odd row r + 1: parity 1 - HALF
-            const uint4 o0 = alt_vector_i8<HALF, OBS>(c0, f1, fd, rnd0, tab, m, b1, bh, bv);
-            const uint4 o1 = alt_vector_i8<1 - HALF, OBS>(c1, f2, f0, rnd1, tab, m, b1, bh, bv);
-            if (live) {
-                *reinterpret_cast<uint4 *>(row) = o0;
-                *reinterpret_cast<uint4 *>(row + wpr) = o1;
-                if constexpr (OBS) { accM += m; a1 += b1; ah += bh; av += bv; }
-            }
-            row += 2 * wpr;
-#pragma unroll
-            for (int j = 0; j < 4; ++j) fd[j] = f1[j];           // flags of the OLD row r + 1: its passive bytes are what row r + 2 reads
-            if (more) {
-                r0 = r2;
-                r1 = a3;
-                r2 = a4;
+        } else {
+            // rows held: r0 = row r, r1 = row r + 1, r2 = row r + 2 (the "up" of row r + 1, and the next iteration's row r);
+            // fd = minus-flags of row r - 1
+            uint32_t fd[4];
+            minus4(*reinterpret_cast<const uint4 *>(col + (size_t)(r_begin == 0 ? L - 1 : r_begin - 1) * wpr), fd);
+            uint32_t *row = col + (size_t)r_begin * wpr;             // row r
+            AltRow r0 = alt_load_row(row, off_prev, off_next);
+            AltRow r1 = alt_load_row(row + wpr, off_prev, off_next); // L even and r_begin even: rows r + 1 exists
+            const uint32_t *pa = r_begin + 2 >= L ? col : row + 2 * wpr;   // row r + 2 (mod L)
+            AltRow r2 = alt_load_row(pa, off_prev, off_next);
+            uint32_t n0 = (uint32_t)r_begin * (uint32_t)(L >> 3) + 2u * (uint32_t)v;
+            const uint32_t dn = (uint32_t)(L >> 3);
+
+            for (int r = r_begin; r < r_end; r += 2) {
+                // fetch rows r + 3 and r + 4 before computing rows r and r + 1 (not past the strip's upper halo row r_end)
+                AltRow a3, a4;
+                const bool more = r + 2 < r_end;
+                if (more) {
+                    a3 = alt_load_row(pa + wpr, off_prev, off_next);               // r + 3 <= r_end - 1 < L: no wrap
+                    const uint32_t *p4 = r + 4 >= L ? col : pa + 2 * wpr;
+                    a4 = alt_load_row(p4, off_prev, off_next);
+                    pa = p4;
+                }
+                uint32_t rnd0[8], rnd1[8];
+                philox_site_words(n0, p.keys, ck, rnd0);
+                philox_site_words(n0 + 1u, p.keys, ck, rnd0 + 4);
+                philox_site_words(n0 + dn, p.keys, ck, rnd1);
+                philox_site_words(n0 + dn + 1u, p.keys, ck, rnd1 + 4);
+                n0 += 2u * dn;
+                int m = 0, b1 = 0, bh = 0, bv = 0;
+                uint32_t f1[4], f2[4], f0[4];
+                minus4(r1.c, f1);
+                minus4(r2.c, f2);
+                minus4(r0.c, f0);
+                const uint32_t c0[6] = {r0.prev, r0.c.x, r0.c.y, r0.c.z, r0.c.w, r0.next};
+                const uint32_t c1[6] = {r1.prev, r1.c.x, r1.c.y, r1.c.z, r1.c.w, r1.next};
+                // even row r: redrawn columns have parity HALF; odd row r + 1: parity 1 - HALF
+                const uint4 o0 = alt_vector_i8<HALF, OBS>(c0, f1, fd, rnd0, tab, m, b1, bh, bv);
+                const uint4 o1 = alt_vector_i8<1 - HALF, OBS>(c1, f2, f0, rnd1, tab, m, b1, bh, bv);
+                if (live) {
+                    *reinterpret_cast<uint4 *>(row) = o0;
+                    *reinterpret_cast<uint4 *>(row + wpr) = o1;
+                    if constexpr (OBS) { accM += m; a1 += b1; ah += bh; av += bv; }
+                }
+                row += 2 * wpr;
+    #pragma unroll
+                for (int j = 0; j < 4; ++j) fd[j] = f1[j];           // flags of the OLD row r + 1: its passive bytes are what row r + 2 reads
+                if (more) {
+                    r0 = r2;
+                    r1 = a3;
+                    r2 = a4;
+                }
             }
         }
         if constexpr (OBS) {
