@@ -49,9 +49,20 @@ struct AltParams {
 // Sums: a1 += sum of redrawn spins, ah += sum of redrawn spin * 4 * (minus among left, right), av likewise for up, down.
 __device__ __forceinline__ uint32_t minus4(uint32_t x) { return x & 0x04040404u; }
 
+// The 5-entry table of a warp sits at a 256-byte aligned shared-memory address, so the address of an entry is the table
+// address with its low byte replaced by the offset byte: one PRMT picks the byte out of the flag sum AND forms the address.
+constexpr int ALT_TAB_WORDS = 64;
+__device__ __forceinline__ uint32_t shared_addr(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ uint32_t lds_u32(uint32_t saddr)
+{
+    uint32_t v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(saddr));
+    return v;
+}
+
 template <int PC, bool OBS>
 __device__ __forceinline__ uint4 alt_vector_i8(const uint32_t (&c)[6], const uint32_t (&fu)[4], const uint32_t (&fd)[4],
-                                               const uint32_t (&rnd)[8], const uint32_t *tab, int &accM, int &a1, int &ah, int &av)
+                                               const uint32_t (&rnd)[8], const uint32_t tab, int &accM, int &a1, int &ah, int &av)
 {
     constexpr uint32_t active = 0x00FF00FFu << (8 * PC);
     uint32_t fc[6], out[4];
@@ -67,8 +78,7 @@ __device__ __forceinline__ uint4 alt_vector_i8(const uint32_t (&c)[6], const uin
         for (int i = 0; i < 2; ++i) {
             constexpr uint32_t FE = 0xFEu;
             const int b = PC + 2 * i;
-            const uint32_t off = __byte_perm(nm, 0u, 0x4440u | (uint32_t)b);
-            const uint32_t T = *reinterpret_cast<const uint32_t *>(reinterpret_cast<const char *>(tab) + off);
+            const uint32_t T = lds_u32(__byte_perm(nm, tab, 0x7650u | (uint32_t)b));
             o = xor_if_less(o, rnd[2 * j + i], T, FE << (8 * b));         // 0xFF ^ 0xFE = +1
         }
         out[j] = o;
@@ -127,7 +137,7 @@ __device__ __forceinline__ uint32_t alt_bits_pk(uint32_t s0, uint32_t s1, uint32
 template <int HALF, bool OBS, bool PACKED>
 __global__ void __launch_bounds__(ALT_THREADS) alt_half(const __grid_constant__ AltParams p)
 {
-    __shared__ uint32_t s_tab[ALT_THREADS / 32][8];
+    __shared__ __align__(256) uint32_t s_tab[ALT_THREADS / 32][ALT_TAB_WORDS];
     let_next_kernel_launch();                                      // programmatic dependent launch (kernels_common.cuh)
     wait_for_previous_kernel();
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -169,8 +179,8 @@ __global__ void __launch_bounds__(ALT_THREADS) alt_half(const __grid_constant__ 
                 philox_site_words(n0, p.keys, ck, rnd);
                 philox_site_words(n0 + 1u, p.keys, ck, rnd + 4);
                 uint4 o;
-                if (pc) o = alt_vector_i8<1, OBS>(c, fu, fd, rnd, tab, accM, a1, accX, accY);
-                else o = alt_vector_i8<0, OBS>(c, fu, fd, rnd, tab, accM, a1, accX, accY);
+                if (pc) o = alt_vector_i8<1, OBS>(c, fu, fd, rnd, shared_addr(tab), accM, a1, accX, accY);
+                else o = alt_vector_i8<0, OBS>(c, fu, fd, rnd, shared_addr(tab), accM, a1, accX, accY);
                 *reinterpret_cast<uint4 *>(row + 4 * v) = o;
             } else {
                 const uint32_t c = row[v], a = up[v], b = dn[v];
@@ -238,13 +248,14 @@ __device__ __forceinline__ void minus4(const uint4 &x, uint32_t (&f)[4])
 template <int HALF, bool OBS>
 __global__ void __launch_bounds__(ALT_THREADS, 2) alt_strip_i8(const __grid_constant__ AltParams p)
 {
-    __shared__ uint32_t s_tab[ALT_THREADS / 32][8];
+    __shared__ __align__(256) uint32_t s_tab[ALT_THREADS / 32][ALT_TAB_WORDS];
     let_next_kernel_launch();                                      // programmatic dependent launch (kernels_common.cuh)
     wait_for_previous_kernel();
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int L = p.L, nvec = p.nvec, wpr = 4 * nvec;
     const int nseg = (nvec + 31) >> 5;
-    uint32_t *tab = s_tab[warp];
+    uint32_t *tab_ptr = s_tab[warp];
+    const uint32_t tab = shared_addr(tab_ptr);
 
     for (long long task = (long long)blockIdx.x * (ALT_THREADS / 32) + warp; task < p.ntasks;
          task += (long long)gridDim.x * (ALT_THREADS / 32)) {
@@ -253,7 +264,7 @@ __global__ void __launch_bounds__(ALT_THREADS, 2) alt_strip_i8(const __grid_cons
         const int rb = rest / nseg, seg = rest - rb * nseg;
         const int r_begin = rb * p.rows_per_task, r_end = min(L, r_begin + p.rows_per_task);
         __syncwarp();
-        if (lane < 5) tab[lane] = p.gtab ? p.gtab[(size_t)chain * 8 + 4 - lane] : p.utab[4 - lane];
+        if (lane < 5) tab_ptr[lane] = p.gtab ? p.gtab[(size_t)chain * 8 + 4 - lane] : p.utab[4 - lane];
         __syncwarp();
         const ChainKeys ck = make_chain_keys(p.keys, p.chain0 + (uint32_t)((chain / p.group) * p.group));
         const bool live = seg * 32 + lane < nvec;
@@ -403,7 +414,7 @@ __host__ __device__ inline size_t alt_small_smem_bytes(int L, int G) { return (s
 __global__ void __launch_bounds__(256) alt_small_i8(const __grid_constant__ SmallParams p)
 {
     extern __shared__ __align__(16) uint32_t smem[];
-    __shared__ uint32_t s_tab[SMALL_GROUP_MAX][8];
+    __shared__ __align__(256) uint32_t s_tab[SMALL_GROUP_MAX][ALT_TAB_WORDS];
     __shared__ int s_acc[SMALL_GROUP_MAX][4];
     const int L = p.L, W = L >> 2, nvec = L >> 4, nvecs = L * nvec, G = p.group;
     const int words = L * W;
@@ -452,8 +463,9 @@ __global__ void __launch_bounds__(256) alt_small_i8(const __grid_constant__ Smal
                     minus4(*reinterpret_cast<const uint4 *>(sg + ad), fd);
                     int mM = 0, b1 = 0, bh = 0, bv = 0;
                     uint4 o;
-                    if (sums) o = pc ? alt_vector_i8<1, true>(cw, fu, fd, rnd, s_tab[m], mM, b1, bh, bv) : alt_vector_i8<0, true>(cw, fu, fd, rnd, s_tab[m], mM, b1, bh, bv);
-                    else o = pc ? alt_vector_i8<1, false>(cw, fu, fd, rnd, s_tab[m], mM, b1, bh, bv) : alt_vector_i8<0, false>(cw, fu, fd, rnd, s_tab[m], mM, b1, bh, bv);
+                    const uint32_t tb = shared_addr(s_tab[m]);
+                    if (sums) o = pc ? alt_vector_i8<1, true>(cw, fu, fd, rnd, tb, mM, b1, bh, bv) : alt_vector_i8<0, true>(cw, fu, fd, rnd, tb, mM, b1, bh, bv);
+                    else o = pc ? alt_vector_i8<1, false>(cw, fu, fd, rnd, tb, mM, b1, bh, bv) : alt_vector_i8<0, false>(cw, fu, fd, rnd, tb, mM, b1, bh, bv);
                     *reinterpret_cast<uint4 *>(sg + at) = o;
                     if (sums) {
                         atomicAdd(&s_acc[m][0], mM);
