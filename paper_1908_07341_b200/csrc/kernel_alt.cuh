@@ -117,7 +117,7 @@ __device__ __forceinline__ uint32_t alt_offsets_pk(uint32_t s0, uint32_t s1, uin
 }
 
 template <int PC>
-__device__ __forceinline__ uint32_t alt_bits_pk(uint32_t s0, uint32_t s1, uint32_t s2, const uint32_t (&rnd)[16], const uint32_t *tab)
+__device__ __forceinline__ uint32_t alt_bits_pk(uint32_t s0, uint32_t s1, uint32_t s2, const uint32_t (&rnd)[16], const uint32_t tab)
 {
     uint32_t nb = 0;
 #pragma unroll
@@ -125,8 +125,7 @@ __device__ __forceinline__ uint32_t alt_bits_pk(uint32_t s0, uint32_t s1, uint32
         const uint32_t W = alt_offsets_pk<PC>(s0, s1, s2, q);
 #pragma unroll
         for (int m = 0; m < 4; ++m) {
-            const uint32_t off = __byte_perm(W, 0u, 0x4440u | (uint32_t)m);
-            const uint32_t T = *reinterpret_cast<const uint32_t *>(reinterpret_cast<const char *>(tab) + off);
+            const uint32_t T = lds_u32(__byte_perm(W, tab, 0x7650u | (uint32_t)m));
             nb = add_if_less(nb, rnd[4 * m + q], T, 1u << (8 * m + 2 * q + PC));
         }
     }
@@ -194,7 +193,7 @@ __global__ void __launch_bounds__(ALT_THREADS) alt_half(const __grid_constant__ 
                 uint32_t rnd[16];
 #pragma unroll
                 for (int q = 0; q < 4; ++q) philox_site_words(n0 + (uint32_t)q, p.keys, ck, rnd + 4 * q);
-                const uint32_t nb = pc ? alt_bits_pk<1>(s0, s1, s2, rnd, tab) : alt_bits_pk<0>(s0, s1, s2, rnd, tab);
+                const uint32_t nb = pc ? alt_bits_pk<1>(s0, s1, s2, rnd, shared_addr(tab)) : alt_bits_pk<0>(s0, s1, s2, rnd, shared_addr(tab));
                 const uint32_t active = 0x55555555u << pc;
                 const uint32_t o = (c & ~active) | nb;
                 row[v] = o;
