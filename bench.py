@@ -284,21 +284,19 @@ def run_ours(args):
     if not args.no_e2e:
         nsp = n_local * w.L * w.L
         h_sigma = torch.empty(nsp, dtype=torch.int8).pin_memory()
-        h_tau = torch.empty(nsp, dtype=torch.int8).pin_memory()
         h_out = torch.empty(nsp, dtype=torch.int8).pin_memory()
         n_rec = K // max(w.obs_every, 1) if w.obs_every else 0
         h_rec = torch.zeros(max(n_rec, 1) * n_local * 6, dtype=torch.int64).pin_memory()
         s.get_spins_into(0, h_sigma.data_ptr())
-        s.get_spins_into(1, h_tau.data_ptr())
         s.clear_records()
         s.step = 0
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize(dev)
         t0 = time.perf_counter()
+        # sigma is the whole input of a run: half-step 0 redraws every tau from sigma alone (eq. 15; SURVEY 8(c) reading 6,
+        # "the dynamics never reads the initial tau"), and the alternate dynamics has no tau
         s.set_spins_from(0, h_sigma.data_ptr())
-        if not alt:
-            s.set_spins_from(1, h_tau.data_ptr())
         run(K)
         got = s.observables_into(h_rec.data_ptr(), max(n_rec, 1))
         s.get_spins_into(0, h_out.data_ptr())
@@ -309,10 +307,10 @@ def run_ours(args):
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
             dt = float(t.item())
         e2e = {"value": world * updates_per_rank / (dt * 1e9), "unit": UNIT,
-               "h2d_bytes_per_step": (1 if alt else 2) * nsp / K, "d2h_bytes_per_step": (nsp + got * n_local * 48) / K,
+               "h2d_bytes_per_step": nsp / K, "d2h_bytes_per_step": (nsp + got * n_local * 48) / K,
                "ms_total": dt * 1e3,
-               "what": ("shaken_set_spins(sigma) from pinned host + shaken_run_alternate(K)" if alt else
-                        "shaken_set_spins(sigma,tau) from pinned host + shaken_run(K)") + " + shaken_observables + shaken_get_spins(sigma) to host"}
+               "what": "shaken_set_spins(sigma) from pinned host + " + ("shaken_run_alternate(K)" if alt else "shaken_run(K)") +
+                       " + shaken_observables + shaken_get_spins(sigma) to host"}
 
     if rank != 0:
         if world > 1:
