@@ -224,7 +224,9 @@ int64_t shaken_launch_count(const shaken_ctx *ctx);
 
 /* Kernel variant: 0 = automatic (default); other values select a specific code path for measurement and tests
  * (DESIGN.md "Kernels"): 1 PRMT index extraction, 2 the round-1 v2 kernel, 3 generic strip kernels also for L <= 128,
- * 4 shared-memory index extraction, 5 paired lookup, 6 IDP extraction, 7 two 256-thread blocks per SM, 8 per-warp task lists, 9 paired lookup with tensor-core observable sums.  Results never depend on the variant. */
+ * 4 shared-memory index extraction, 5 paired lookup, 6 IDP extraction, 7 two 256-thread blocks per SM, 8 per-warp task lists,
+ * 9 paired lookup with tensor-core observable sums.  shaken_run_alternate only distinguishes 0 from the rest: any other
+ * value keeps it on the per-half-step kernels also for L <= 128.  Results never depend on the variant. */
 int shaken_set_variant(shaken_ctx *ctx, int variant);
 
 /* Message for the most recent error on this context ("" if none).  ctx may be NULL (creation errors). */
