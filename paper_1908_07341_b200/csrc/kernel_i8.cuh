@@ -50,6 +50,9 @@ __global__ void __launch_bounds__(THREADS, MINB) half_step_i8(const __grid_const
     constexpr bool OBS = (FLAGS & F_OBS) != 0;
     constexpr bool BONDS = (FLAGS & F_BONDS) != 0;
     constexpr bool UPDATE = (FLAGS & F_NOUPDATE) == 0;
+    // carry the round-0 Philox product by additions (philox.cuh): measured +1.6 % on launches with sums (their IDP.4A load
+    // the multiplier pipe further), -0.6 % on plain ones, so only the former do it
+    constexpr bool PRODUCT = (FLAGS & (F_OBS | F_BONDS)) != 0;
     static_assert(!(BONDS && HALF == 1), "bond sums ride on half-step 0");
 
     __shared__ uint32_t s_tabs[PERWARP ? WPB : 1][64];
@@ -174,8 +177,14 @@ __global__ void __launch_bounds__(THREADS, MINB) half_step_i8(const __grid_const
             const uint8_t *pc = sbase + (size_t)r * L + c0;          // this lane's 16 spins of the current row
             const uint8_t *pe = sbase + (size_t)r * L + ce;          // the word holding the horizontal edge spin
             uint8_t *pd = dbase + (size_t)r * L + c0;
+            // Philox counter word 0 of the lane's first call in the row is n = r * L/4 + 4 cv; only its product with M0 is
+            // needed, and that is carried from call to call and from row to row by 64-bit additions (philox.cuh)
             uint32_t n = (uint32_t)r * (uint32_t)L4 + (uint32_t)cv * 4u;
             const uint32_t nstep = (uint32_t)(dir * L4);
+            uint32_t ph, pl;
+            mul_wide(PHILOX_M0, n, ph, pl);
+            const long long pstep = (long long)PHILOX_M0 * (long long)(dir * L4);
+            const uint32_t pstep_hi = (uint32_t)((unsigned long long)pstep >> 32), pstep_lo = (uint32_t)pstep;
             uint32_t *const my_idx = &s_idx[0][EXTRACT == EXTRACT_SMEM ? threadIdx.x : 0];
             const uint32_t lane8 = (uint32_t)lane * 8u;
 
@@ -208,7 +217,13 @@ __global__ void __launch_bounds__(THREADS, MINB) half_step_i8(const __grid_const
                     uint32_t out = PACKADD ? 0x01010101u : 0xFFFFFFFFu;
                     if (UPDATE) {
                         uint32_t rw[4];
-                        philox_site_words(n + (uint32_t)j, p.keys, ck, rw);
+                        if constexpr (PRODUCT) {
+                            uint32_t qh = ph, ql = pl;                 // M0 * (n + j)
+                            if (j) add64(qh, ql, (uint32_t)(((unsigned long long)PHILOX_M0 * j) >> 32), (uint32_t)((unsigned long long)PHILOX_M0 * j));
+                            philox_site_words_prod(qh, ql, p.keys, p.keys.xa2, p.keys.xb0, ck, rw);
+                        } else {
+                            philox_site_words(n + (uint32_t)j, p.keys, ck, rw);
+                        }
                         uint32_t Tp[4];
                         if (EXTRACT == EXTRACT_PAIR) {
                             // one IDP.4A per pair forms the whole byte offset: (2 c_even) * 128 + (32 c_odd) * 64 + lane * 8
@@ -280,7 +295,8 @@ __global__ void __launch_bounds__(THREADS, MINB) half_step_i8(const __grid_const
                 }
                 if (UPDATE && (!OBSMMA || live)) *reinterpret_cast<uint4 *>(pd) = make_uint4(ow[0], ow[1], ow[2], ow[3]);
                 pc += stride; pe += stride; pd += stride;
-                n += nstep;
+                if constexpr (PRODUCT) add64(ph, pl, pstep_hi, pstep_lo);
+                else n += nstep;
             };
 
             // three row buffers rotate roles (vertical neighbour / current / prefetched) without register moves
