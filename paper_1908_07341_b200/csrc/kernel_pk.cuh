@@ -112,8 +112,11 @@ __global__ void __launch_bounds__(PK_THREADS, 1) half_step_pk(const __grid_const
             const uint32_t *pc = sbase + (size_t)r0 * W + cv;
             const uint32_t *pe = sbase + (size_t)r0 * W + ce;
             uint32_t *pd = dbase + (size_t)r0 * W + cv;
-            uint32_t n = (uint32_t)r0 * (uint32_t)L4 + (uint32_t)cv * 8u;
-            const uint32_t nstep = (uint32_t)(dir * L4);
+            // M0 * (Philox counter word 0 of the word's first call), carried by 64-bit additions (philox.cuh)
+            uint32_t ph, pl;
+            mul_wide(PHILOX_M0, (uint32_t)r0 * (uint32_t)L4 + (uint32_t)cv * 8u, ph, pl);
+            const long long pstep = (long long)PHILOX_M0 * (long long)(dir * L4);
+            const uint32_t pstep_hi = (uint32_t)((unsigned long long)pstep >> 32), pstep_lo = (uint32_t)pstep;
 
             // the row in use, and the next two already on their way (prefetch distance 2)
             uint32_t V = __ldg(sbase + (size_t)rh * W + cv);
@@ -147,7 +150,9 @@ __global__ void __launch_bounds__(PK_THREADS, 1) half_step_pk(const __grid_const
 #pragma unroll
                     for (int q = 0; q < 8; ++q) {
                         uint32_t rw[4];
-                        philox_site_words(n + (uint32_t)q, p.keys, ck, rw);
+                        uint32_t qh = ph, ql = pl;                     // M0 * (n + q)
+                        if (q) add64(qh, ql, (uint32_t)(((unsigned long long)PHILOX_M0 * q) >> 32), (uint32_t)((unsigned long long)PHILOX_M0 * q));
+                        philox_site_words_prod(qh, ql, p.keys, p.keys.xa2, p.keys.xb0, ck, rw);
                         const int m = q >> 1, j0 = (q & 1) * 2;
                         const uint32_t o01 = __dp4a(P[j0], 0x80u << (8 * m), lane8), o23 = __dp4a(P[j0 + 1], 0x80u << (8 * m), lane8);
                         const uint2 t01 = *reinterpret_cast<const uint2 *>(reinterpret_cast<const char *>(s_pair) + o01);
@@ -176,7 +181,7 @@ __global__ void __launch_bounds__(PK_THREADS, 1) half_step_pk(const __grid_const
                 }
                 V = S; S0 = S1; E0 = E1; S1 = S2; E1 = E2;
                 pc += stride; pe += stride; pd += stride;
-                n += nstep;
+                add64(ph, pl, pstep_hi, pstep_lo);
             }
             if (OBS || BONDS) {
                 const int ns = rows * 32;
