@@ -319,7 +319,8 @@ def run_ours(args):
 
     # ------------------------------------------------------------------ roofline of the half-step kernel
     # The half-step is bound by plain integer arithmetic, not by HBM: 32 random bits per site
-    # cost 4.5 IMAD.WIDE (18 per Philox4x32-10 call of 4 sites, after hoisting), and a warp-wide IMAD.WIDE holds the
+    # cost 4.25 IMAD.WIDE (17 per Philox4x32-10 call of 4 sites: rounds 0-1 hoisted, the round-0 product carried by
+    # additions; the plain launches spend 18, which is faster for them), and a warp-wide IMAD.WIDE holds the
     # SMSP's 16-lane multiplier for 4 cycles.  peak = n_SM * 4 SMSP * 8 lane-multiplies/clk * max SM clock.
     # The HBM view (BASELINE.json's "% of HBM roofline") is reported next to it.
     hbm_peak, peak_src = measured_peak()
@@ -343,12 +344,12 @@ def run_ours(args):
     props = torch.cuda.get_device_properties(dev)
     clk = sampler.summary() or {}
     sm_max_mhz = clk.get("sm_max_mhz") or 1965.0
-    MULS_PER_SITE = 4.5
+    MULS_PER_SITE = 4.25
     alu_peak = props.multi_processor_count * 4 * 8 * sm_max_mhz * 1e6 / 1e9      # G IMAD.WIDE lane-ops / s
     alu_achieved = MULS_PER_SITE * sites_per_launch / (avg_launch_ms * 1e-3) / 1e9
     roofline = {"bound": "alu", "achieved": alu_achieved, "peak": alu_peak, "unit": "G IMAD.WIDE/s", "frac": alu_achieved / alu_peak,
                 "traffic": traffic,
-                "peak_source": "derived (DESIGN.md Rooflines): %d SMs x 4 SMSP x 8 wide multiplies/clk x %.0f MHz; 4.5 IMAD.WIDE per site-update"
+                "peak_source": "derived (DESIGN.md Rooflines): %d SMs x 4 SMSP x 8 wide multiplies/clk x %.0f MHz; 4.25 IMAD.WIDE per site-update"
                                % (props.multi_processor_count, sm_max_mhz),
                 "kernel": ("alt_half (packed)" if w.packed else "alt_strip_i8") if alt else ("half_step_pk" if w.packed else "half_step_i8"),
                 "algorithmic_ops_per_launch": MULS_PER_SITE * sites_per_launch,
