@@ -308,11 +308,13 @@ __global__ void __launch_bounds__(ALT_THREADS, 2) alt_strip_i8(const __grid_cons
                     e3p = p3[off_prev]; e3n = p3[off_next];
                     e4p = p4[off_prev]; e4n = p4[off_next];
                 }
-                uint32_t rnd0[8], rnd1[8];
-                philox_site_words(n0, p.keys, ck, rnd0);
-                philox_site_words(n0 + 1u, p.keys, ck, rnd0 + 4);
-                philox_site_words(n0 + dn, p.keys, ck, rnd1);
-                philox_site_words(n0 + dn + 1u, p.keys, ck, rnd1 + 4);
+                uint32_t rr[4][4];
+                {
+                    const uint32_t nn[4] = {n0, n0 + 1u, n0 + dn, n0 + dn + 1u};
+                    philox_site_words_xn<4>(nn, p.keys, p.keys.xa2, p.keys.xb0, ck, rr);
+                }
+                const uint32_t rnd0[8] = {rr[0][0], rr[0][1], rr[0][2], rr[0][3], rr[1][0], rr[1][1], rr[1][2], rr[1][3]};
+                const uint32_t rnd1[8] = {rr[2][0], rr[2][1], rr[2][2], rr[2][3], rr[3][0], rr[3][1], rr[3][2], rr[3][3]};
                 n0 += 2u * dn;
                 int m = 0, b1 = 0, bh = 0, bv = 0;
                 uint32_t f1[4], f2[4], f0[4];
@@ -363,11 +365,13 @@ __global__ void __launch_bounds__(ALT_THREADS, 2) alt_strip_i8(const __grid_cons
                     a4 = alt_load_row(p4, off_prev, off_next);
                     pa = p4;
                 }
-                uint32_t rnd0[8], rnd1[8];
-                philox_site_words(n0, p.keys, ck, rnd0);
-                philox_site_words(n0 + 1u, p.keys, ck, rnd0 + 4);
-                philox_site_words(n0 + dn, p.keys, ck, rnd1);
-                philox_site_words(n0 + dn + 1u, p.keys, ck, rnd1 + 4);
+                uint32_t rr[4][4];
+                {
+                    const uint32_t nn[4] = {n0, n0 + 1u, n0 + dn, n0 + dn + 1u};
+                    philox_site_words_xn<4>(nn, p.keys, p.keys.xa2, p.keys.xb0, ck, rr);
+                }
+                const uint32_t rnd0[8] = {rr[0][0], rr[0][1], rr[0][2], rr[0][3], rr[1][0], rr[1][1], rr[1][2], rr[1][3]};
+                const uint32_t rnd1[8] = {rr[2][0], rr[2][1], rr[2][2], rr[2][3], rr[3][0], rr[3][1], rr[3][2], rr[3][3]};
                 n0 += 2u * dn;
                 int m = 0, b1 = 0, bh = 0, bv = 0;
                 uint32_t f1[4], f2[4], f0[4];

@@ -134,6 +134,47 @@ __device__ __forceinline__ void philox_site_words(uint32_t n, const StepKeys &K,
     philox_site_words_prod(h0, l0, K, xa2, xb0, C, r);
 }
 
+// N independent calls advanced round by round (the source order a scheduler would want: N multiply chains in flight)
+template <int N>
+__device__ __forceinline__ void philox_site_words_xn(const uint32_t (&n)[N], const StepKeys &K, const uint32_t xa2, const uint32_t xb0,
+                                                     const ChainKeys &C, uint32_t (&r)[N][4])
+{
+    uint32_t c0[N], c1[N], c2[N], c3[N];
+#pragma unroll
+    for (int t = 0; t < N; ++t) {
+        uint32_t h0, l0, h1, l1;
+        mul_wide(PHILOX_M0, n[t], h0, l0);
+        const uint32_t a2 = h0 ^ xa2, a3 = l0;
+        mul_wide(PHILOX_M1, a2, h1, l1);
+        c0[t] = h1 ^ xb0; c1[t] = l1; c2[t] = a3 ^ C.xb2;
+    }
+#pragma unroll
+    for (int t = 0; t < N; ++t) {
+        uint32_t h0, l0, h1, l1;
+        mul_wide(PHILOX_M0, c0[t], h0, l0);
+        mul_wide(PHILOX_M1, c2[t], h1, l1);
+        c0[t] = h1 ^ c1[t] ^ K.k0[2];
+        c1[t] = l1;
+        c2[t] = h0 ^ C.xd2;
+        c3[t] = l0;
+    }
+#pragma unroll
+    for (int i = 3; i < 10; ++i) {
+#pragma unroll
+        for (int t = 0; t < N; ++t) {
+            uint32_t h0, l0, h1, l1;
+            mul_wide(PHILOX_M0, c0[t], h0, l0);
+            mul_wide(PHILOX_M1, c2[t], h1, l1);
+            c0[t] = h1 ^ c1[t] ^ K.k0[i];
+            c1[t] = l1;
+            c2[t] = h0 ^ c3[t] ^ K.k1[i];
+            c3[t] = l0;
+        }
+    }
+#pragma unroll
+    for (int t = 0; t < N; ++t) { r[t][0] = c0[t]; r[t][1] = c1[t]; r[t][2] = c2[t]; r[t][3] = c3[t]; }
+}
+
 // 64-bit (hi:lo) += (ahi:alo), as two 32-bit additions with carry (kept off the multiplier pipe on purpose)
 __device__ __forceinline__ void add64(uint32_t &hi, uint32_t &lo, uint32_t ahi, uint32_t alo)
 {
