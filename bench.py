@@ -52,6 +52,7 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--variant", type=int, default=0)
+    ap.add_argument("--cpu-multicore-leg", action="store_true", help=argparse.SUPPRESS)
     ap.add_argument("--dynamics", default="shaken", choices=["shaken", "alternate"],
                     help="alternate: the even/odd heat bath on the square lattice (PAPER.md:276) on the same lattice, "
                          "chains, J and record cadence as the named workload; a step redraws every site once")
@@ -198,6 +199,54 @@ def cpu_baseline(w, alternate=False):
     return {"value": upd / (dt * 1e9), "unit": UNIT, "cores": 1, "kind": "oracle",
             "sample": f"{reps} x both half-steps of {band} rows x {L} columns of chain 0 ({int(upd)} site updates, {dt:.1f} s)",
             "host_cores_available": os.cpu_count()}
+
+
+_MC = {}
+
+
+def _mc_band(args):
+    """Worker of cpu_baseline_multicore: one band of rows of one half-step by the oracle; returns a checksum only."""
+    from oracle import shaken_oracle as so
+
+    w_seed, J, q, t, half, r0, nrows, alternate = args
+    src = _MC["src"]
+    if alternate:
+        out = so.alt_half_step_rows(src, w_seed, 0, J, t, half, r0, nrows)
+    else:
+        out = so.half_step_rows(src, w_seed, 0, J, q, t, half, r0, nrows)
+    return int(out.sum(dtype=np.int64))
+
+
+def cpu_baseline_multicore(w, alternate=False):
+    """SURVEY 8(d), optional second line: the same oracle, unchanged, with the rows of a half-step split over all host
+    cores by processes (legal because the randomness is a function of the site index).  About 5-10 s."""
+    import multiprocessing as mp
+
+    from oracle import shaken_oracle as so
+
+    so.build()
+    cores = os.cpu_count() or 1
+    L = w.L
+    band = max(cores, min(L, (256 << 20) // L))
+    _MC["src"] = np.ones((L, L), dtype=np.int8)            # inherited by the forked workers, never pickled
+    bounds = np.linspace(0, band, cores + 1).astype(int)
+    with mp.get_context("fork").Pool(cores) as pool:
+        def half(t, h):
+            jobs = [(w.seed, w.J[0], w.q[0], t, h, int(bounds[i]), int(bounds[i + 1] - bounds[i]), alternate) for i in range(cores)]
+            return pool.map(_mc_band, jobs)
+        half(0, 0)                                         # warm the workers
+        t0 = time.perf_counter()
+        reps = 0
+        while True:
+            half(reps, 0)
+            half(reps, 1)
+            reps += 1
+            dt = time.perf_counter() - t0
+            if dt >= 5.0 or reps >= 64:
+                break
+    upd = (1.0 if alternate else 2.0) * band * L * reps
+    return {"value": upd / (dt * 1e9), "unit": UNIT, "cores": cores, "kind": "oracle, rows split over processes",
+            "sample": f"{reps} x both half-steps of {band} rows x {L} columns of chain 0 ({int(upd)} site updates, {dt:.1f} s)"}
 
 
 # ----------------------------------------------------------------------------------------- our arm
@@ -374,6 +423,13 @@ def run_ours(args):
     }
     if not args.no_cpu_baseline and world == 1:
         line["cpu_baseline"] = cpu_baseline(w, alt)
+        try:
+            # in a fresh interpreter (this one holds a CUDA context and must not be forked), bounded in time
+            out = subprocess.run([sys.executable, os.path.abspath(__file__), "--cpu-multicore-leg", "--workload", args.workload,
+                                  "--dynamics", args.dynamics], capture_output=True, text=True, timeout=240).stdout
+            line["cpu_baseline_multicore"] = json.loads(out.strip().splitlines()[-1])
+        except Exception as e:                             # never let the optional leg cost the bench line
+            line["cpu_baseline_multicore"] = {"unavailable": repr(e)[:200]}
     elif world > 1:
         line["cpu_baseline"] = None
     print(json.dumps(line))
@@ -389,6 +445,9 @@ def shaken_bytes(w):
 
 def main():
     args = parse_args()
+    if args.cpu_multicore_leg:
+        print(json.dumps(cpu_baseline_multicore(workload(args.workload), args.dynamics == "alternate")))
+        return 0
     if args.impl == "reference":
         return run_reference(args)
     return run_ours(args)
