@@ -190,9 +190,13 @@ __global__ void __launch_bounds__(ALT_THREADS) alt_half(const __grid_constant__ 
                 const uint32_t ab = a & b, axb = a ^ b, lr = lw & rw, lxr = lw ^ rw;
                 const uint32_t s0 = axb ^ lxr, s1 = (ab ^ lr) ^ (axb & lxr), s2 = ab & lr;
                 const uint32_t n0 = (uint32_t)r * (uint32_t)(L >> 3) + 4u * (uint32_t)v;
-                uint32_t rnd[16];
-#pragma unroll
-                for (int q = 0; q < 4; ++q) philox_site_words(n0 + (uint32_t)q, p.keys, ck, rnd + 4 * q);
+                uint32_t rr[4][4];
+                {
+                    const uint32_t nn[4] = {n0, n0 + 1u, n0 + 2u, n0 + 3u};
+                    philox_site_words_xn<4>(nn, p.keys, p.keys.xa2, p.keys.xb0, ck, rr);
+                }
+                const uint32_t rnd[16] = {rr[0][0], rr[0][1], rr[0][2], rr[0][3], rr[1][0], rr[1][1], rr[1][2], rr[1][3],
+                                          rr[2][0], rr[2][1], rr[2][2], rr[2][3], rr[3][0], rr[3][1], rr[3][2], rr[3][3]};
                 const uint32_t nb = pc ? alt_bits_pk<1>(s0, s1, s2, rnd, shared_addr(tab)) : alt_bits_pk<0>(s0, s1, s2, rnd, shared_addr(tab));
                 const uint32_t active = 0x55555555u << pc;
                 const uint32_t o = (c & ~active) | nb;
