@@ -147,12 +147,18 @@ __global__ void __launch_bounds__(PK_THREADS, 1) half_step_pk(const __grid_const
                     }
 #pragma unroll
                     for (int j = 0; j < 4; ++j) P[j] = C[2 * j] + 8u * C[2 * j + 1];
+                    uint32_t RW[4][4];
 #pragma unroll
                     for (int q = 0; q < 8; ++q) {
-                        uint32_t rw[4];
-                        uint32_t qh = ph, ql = pl;                     // M0 * (n + q)
-                        if (q) add64(qh, ql, (uint32_t)(((unsigned long long)PHILOX_M0 * q) >> 32), (uint32_t)((unsigned long long)PHILOX_M0 * q));
-                        philox_site_words_prod(qh, ql, p.keys, p.keys.xa2, p.keys.xb0, ck, rw);
+                        if ((q & 3) == 0) {                            // four calls at a time, round by round
+                            uint32_t qh[4] = {ph, ph, ph, ph}, ql[4] = {pl, pl, pl, pl};   // M0 * (n + q + t)
+#pragma unroll
+                            for (int t = 0; t < 4; ++t)
+                                if (q + t) add64(qh[t], ql[t], (uint32_t)(((unsigned long long)PHILOX_M0 * (q + t)) >> 32), (uint32_t)((unsigned long long)PHILOX_M0 * (q + t)));
+                            const uint32_t nn[4] = {0u, 0u, 0u, 0u};
+                            philox_site_words_xn<4, true>(nn, p.keys, p.keys.xa2, p.keys.xb0, ck, RW, qh, ql);
+                        }
+                        const uint32_t (&rw)[4] = RW[q & 3];
                         const int m = q >> 1, j0 = (q & 1) * 2;
                         const uint32_t o01 = __dp4a(P[j0], 0x80u << (8 * m), lane8), o23 = __dp4a(P[j0 + 1], 0x80u << (8 * m), lane8);
                         const uint2 t01 = *reinterpret_cast<const uint2 *>(reinterpret_cast<const char *>(s_pair) + o01);

@@ -135,15 +135,18 @@ __device__ __forceinline__ void philox_site_words(uint32_t n, const StepKeys &K,
 }
 
 // N independent calls advanced round by round (the source order a scheduler would want: N multiply chains in flight)
-template <int N>
+// PROD: n[t] is not used, (ph[t]:pl[t]) = M0 * n[t] is supplied (see philox_site_words_prod)
+template <int N, bool PROD = false>
 __device__ __forceinline__ void philox_site_words_xn(const uint32_t (&n)[N], const StepKeys &K, const uint32_t xa2, const uint32_t xb0,
-                                                     const ChainKeys &C, uint32_t (&r)[N][4])
+                                                     const ChainKeys &C, uint32_t (&r)[N][4], const uint32_t *ph = nullptr,
+                                                     const uint32_t *pl = nullptr)
 {
     uint32_t c0[N], c1[N], c2[N], c3[N];
 #pragma unroll
     for (int t = 0; t < N; ++t) {
         uint32_t h0, l0, h1, l1;
-        mul_wide(PHILOX_M0, n[t], h0, l0);
+        if constexpr (PROD) { h0 = ph[t]; l0 = pl[t]; }
+        else mul_wide(PHILOX_M0, n[t], h0, l0);
         const uint32_t a2 = h0 ^ xa2, a3 = l0;
         mul_wide(PHILOX_M1, a2, h1, l1);
         c0[t] = h1 ^ xb0; c1[t] = l1; c2[t] = a3 ^ C.xb2;
