@@ -817,7 +817,9 @@ static int run_alt_impl(shaken_ctx *ctx, const double *J, bool uniform, int64_t 
         p.gtab = ctx->d_tab;
     }
     // small lattices: one CTA per coupling group, sigma in shared memory, the whole run in one launch
-    if (!ctx->packed && ctx->variant == 0 && ctx->L <= SMALL_L_MAX && ctx->group <= SMALL_GROUP_MAX) {
+    // (also mid-size chains, L <= 288, when there are enough of them to fill the machine, as in run_impl)
+    if (!ctx->packed && ctx->variant == 0 && ctx->group <= SMALL_GROUP_MAX && alt_small_smem_bytes(ctx->L, ctx->group) <= 200 * 1024 &&
+        (ctx->L <= SMALL_L_MAX || (ctx->L <= SMALL_L_BATCH_MAX && 2 * (ctx->n_chains / ctx->group) >= ctx->num_sms))) {
         SmallParams sp;
         memset(&sp, 0, sizeof(sp));
         sp.sigma = (uint8_t *)ctx->d_sigma;

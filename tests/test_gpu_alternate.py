@@ -61,6 +61,25 @@ def test_alternate_small_lattice_path_and_per_half_step_kernels_agree_with_oracl
             assert np.array_equal(s.coalescence(), o.coalescence()), variant
 
 
+def test_alternate_batch_of_mid_size_chains_runs_in_the_one_cta_per_chain_path():
+    """80 chains of 208^2 are enough to fill the machine, so the run takes the shared-memory path (one launch) although
+    L > 128; variant 3 takes the per-half-step kernels (13 vectors per row: the generic form).  Both against the oracle."""
+    L, n_chains, seed, steps = 208, 80, 77, 4
+    J = np.linspace(0.2, 0.6, n_chains)
+    o = so.Oracle(L, n_chains, seed)
+    o.init(0)
+    o.run_alternate(J, steps, 2)
+    for variant, launches in ((0, 1), (3, 2 * steps)):
+        with shaken.Shaken(L, n_chains, seed, max_records=steps) as s:
+            s.set_variant(variant)
+            s.init(0)
+            l0 = s.launch_count
+            s.run_alternate(J, steps, 2)
+            assert s.launch_count - l0 == launches
+            assert np.array_equal(s.get_spins(0), o.get_spins(0)), variant
+            assert np.array_equal(s.observables(), o.observables()), variant
+
+
 def test_alternate_grid_of_couplings_resume_and_chain_offset():
     L, n_chains, seed = 80, 5, 41
     J = np.array([0.1, 0.3, 0.44, 0.6, 0.9])
