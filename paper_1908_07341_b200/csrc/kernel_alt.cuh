@@ -440,9 +440,12 @@ __global__ void __launch_bounds__(256) alt_small_i8(const __grid_constant__ Smal
 
     bool coalesced = p.coal ? p.coal[gi] >= 0 : true;   // block-uniform
     long long nrec = 0;
+    // full steps until the next recorded one: a countdown instead of a 64-bit modulo per step
+    long long until_rec = p.obs_every > 0 ? p.obs_every - (long long)(p.t0 % (unsigned long long)p.obs_every) : 0;
     for (long long s = 0; s < p.n_steps; ++s) {
         const unsigned long long t = p.t0 + (unsigned long long)s;
-        const bool rec = p.obs_every > 0 && (t + 1) % (unsigned long long)p.obs_every == 0;
+        const bool rec = p.obs_every > 0 && --until_rec == 0;
+        if (rec) until_rec = p.obs_every;
 #pragma unroll 1
         for (int half = 0; half < 2; ++half) {
             uint32_t xa2, xb0;

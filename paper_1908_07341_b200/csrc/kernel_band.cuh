@@ -216,6 +216,8 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) band_run_i8(const __grid_cons
 
     long long *pending = nullptr;
     long long nrec = 0;
+    // full steps until the next recorded one: a countdown instead of a 64-bit modulo per step
+    long long until_rec = p.obs_every > 0 ? p.obs_every - (long long)(p.t0 % (unsigned long long)p.obs_every) : 0;
 #pragma unroll 1
     for (long long h = 0; h < 2 * p.n_steps; ++h) {
         const long long s = h >> 1;
@@ -250,7 +252,8 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) band_run_i8(const __grid_cons
         __syncthreads();
 
         // record (M_sigma, M_tau, E_J, E_q now; C_x, C_y at the start of the next half-step 0)
-        if (half == 1 && p.obs_every > 0 && (t + 1) % (unsigned long long)p.obs_every == 0) {
+        if (half == 1 && p.obs_every > 0 && --until_rec == 0) {
+            until_rec = p.obs_every;
             long long *dst = p.rec + ((size_t)nrec * p.n_chains + chain) * 6;
             int v[6] = {0, 0, 0, 0, 0, 0};
             for (int c = tid; c < ncalls; c += BAND_THREADS) {
