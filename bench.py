@@ -312,8 +312,8 @@ def run_ours(args):
     launches = s.launch_count - l0
     if rank == 0:
         # nvidia-smi needs ~50 ms per sample: keep the same launch sequence running right after the timed region
-        # until at least 0.5 s of load has been sampled (records are discarded; obs cadence unchanged)
-        t_end = time.perf_counter() + max(0.5 - ms * 1e-3, 0.0)
+        # until at least 1.5 s of load has been sampled (records are discarded; obs cadence unchanged)
+        t_end = time.perf_counter() + max(1.5 - ms * 1e-3, 0.0)
         while time.perf_counter() < t_end:
             s.clear_records()
             run(K)
