@@ -9,12 +9,15 @@ BASELINE.json configs[3] ("cfg4": L=16384 int8, J=q=0.7, all +1, seed 3, six sum
 configuration the metric is quoted on.
 
 * ``value``     device-resident throughput: K steps timed with CUDA events on the stream the kernels run on.
-* ``e2e``       the same job through the C ABI with HOST buffers inside the timed region: shaken_set_spins of both
-                layers from pinned host memory, shaken_run(K steps), shaken_observables and shaken_get_spins(sigma)
-                back to the host.  Bytes per step are the totals divided by K.
+* ``e2e``       the same job through the C ABI with HOST buffers inside the timed region: shaken_set_spins of sigma
+                (the whole input: half-step 0 redraws every tau from sigma alone) from pinned host memory,
+                shaken_run(K steps), shaken_observables and shaken_get_spins(sigma) back to the host.  Bytes per step
+                are the totals divided by K.
 * ``roofline``  dominant kernel (the half-step kernel, 2K launches in the timed region): algorithmic bytes per
                 launch (2 B per site-update: read one source byte, write one target byte; 0.25 B bit-packed) over
-                its mean duration, against the measured HBM copy bandwidth of MEASURED_PEAKS.json.
+                its mean duration, against the measured HBM copy bandwidth of MEASURED_PEAKS.json; nested: the integer
+                multiplier view (``alu``) and the Philox-only ceiling measured in the same run through the library.
+* ``workloads`` (default run only) the other four BASELINE.json workloads, a short timed leg each.
 * ``cpu_baseline``  the oracle (oracle/, as it stands, single thread) timed on this box on a bounded sample.
 * ``--impl reference``  for this tier the reference arm IS the oracle: times it on the host cores, each step a
                 bounded band of rows of the same workload.
@@ -51,7 +54,8 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--variant", type=int, default=0)
+    ap.add_argument("--no-workloads", action="store_true", help="skip the short legs on the other four BASELINE.json workloads")
+    ap.add_argument("--variant", type=int, default=0, choices=[0, 3, 8], help="code-path switch of shaken_set_variant (0 = automatic)")
     ap.add_argument("--cpu-multicore-leg", action="store_true", help=argparse.SUPPRESS)
     ap.add_argument("--dynamics", default="shaken", choices=["shaken", "alternate"],
                     help="alternate: the even/odd heat bath on the square lattice (PAPER.md:276) on the same lattice, "
@@ -250,6 +254,76 @@ def cpu_baseline_multicore(w, alternate=False):
 
 
 # ----------------------------------------------------------------------------------------- our arm
+def muls_per_site(w, alt):
+    """IMAD.WIDE per site-update of the kernels this workload launches (17 or 18 per Philox4x32-10 call of 4 sites:
+    rounds 0-1 hoisted; launches that carry the round-0 product by additions spend 17 -- philox.cuh)."""
+    if alt:
+        return 18 / 4.0                                    # kernel_alt.cuh: philox_site_words[_xn] without the carried product
+    if w.packed:
+        return 17 / 4.0                                    # kernel_pk.cuh: carried product in every launch
+    if w.L <= 2048 and w.n_chains <= 148:
+        return 18 / 4.0                                    # one-launch paths (kernel_small.cuh, kernel_band.cuh)
+    if w.obs_every == 1:
+        return 17 / 4.0                                    # kernel_i8.cuh: every launch carries sums, hence the product
+    if w.obs_every == 0:
+        return 18 / 4.0
+    return (17.0 / w.obs_every + 18.0 * (1.0 - 1.0 / w.obs_every)) / 4.0
+
+
+def time_workload(shaken, torch, dist, w, K, W, dev, stream, rank, world, alt, variant=0, before_timed=None):
+    """W warm-up steps, then K steps timed with CUDA events on the library's stream.  Returns (context, ms, launches, run)."""
+    s = shaken.Shaken(w.L, w.n_chains, w.seed, packed=w.packed, max_records=(K + W) // max(w.obs_every, 1) + 4 if w.obs_every else 1,
+                      device=str(dev), stream=stream)
+    s.set_chain_offset(rank * w.n_chains)
+    if variant:
+        s.set_variant(variant)
+    J, q = w.J_array(), w.q_array()
+    uniform = len(set(w.J)) == 1 and len(set(w.q)) == 1
+
+    def run(n):
+        if alt:
+            s.run_alternate(w.J[0] if uniform else J, n, w.obs_every)
+        elif uniform:
+            s.run(w.J[0], w.q[0], n, w.obs_every)
+        else:
+            s.run_grid(J, q, n, w.obs_every)
+
+    s.init(w.init)
+    run(W)
+    s.synchronize()
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize(dev)
+    if before_timed:
+        before_timed()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0 = s.launch_count
+    e0.record(stream)
+    run(K)
+    e1.record(stream)
+    e1.synchronize()
+    torch.cuda.synchronize(dev)
+    return s, e0.elapsed_time(e1), s.launch_count - l0, run
+
+
+def rooflines(w, alt, ms, K, n_sms, sm_max_mhz, hbm_peak, philox_only):
+    """HBM view (the metric's denominator), integer-multiplier view and the measured Philox-only ceiling of one workload."""
+    bytes_per_update = 0.25 if w.packed else 2.0
+    sites_per_launch = w.n_chains * w.L * w.L
+    if alt:
+        bytes_per_update *= 2.0                            # in place on one array: read + write the array to redraw half of it
+        sites_per_launch //= 2
+    avg_launch_ms = ms / (2 * K)                           # two half-steps per step (a trailing bond-sum pass is inside ms)
+    rate = sites_per_launch / (avg_launch_ms * 1e6)        # site-updates per ns of the half-step kernel
+    mps = muls_per_site(w, alt)
+    alu_peak = n_sms * 4 * 8 * sm_max_mhz * 1e6 / 1e9      # G IMAD.WIDE lane-operations per second
+    return {"sites_per_launch": sites_per_launch, "avg_launch_us": avg_launch_ms * 1e3,
+            "alg_bytes_per_launch": bytes_per_update * sites_per_launch,
+            "hbm_achieved": bytes_per_update * rate, "hbm_frac": bytes_per_update * rate / hbm_peak,
+            "alu_achieved": mps * rate, "alu_peak": alu_peak, "alu_frac": mps * rate / alu_peak, "muls_per_site": mps,
+            "philox_frac": rate / philox_only if philox_only else None}
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -273,43 +347,12 @@ def run_ours(args):
     K, W = args.steps, max(args.warmup, 3)
     stream = torch.cuda.Stream(device=dev)
     n_local = w.n_chains                                   # weak scaling: every rank runs the whole named workload
-    s = shaken.Shaken(w.L, n_local, w.seed, packed=w.packed, max_records=(K + W) // max(w.obs_every, 1) + 4,
-                      device=str(dev), stream=stream)
-    s.set_chain_offset(rank * n_local)
-    if args.variant:
-        s.set_variant(args.variant)
-    J, q = w.J_array(), w.q_array()
+    alt = args.dynamics == "alternate"
     uniform = len(set(w.J)) == 1 and len(set(w.q)) == 1
 
-    alt = args.dynamics == "alternate"
-
-    def run(n):
-        if alt:
-            s.run_alternate(w.J[0] if uniform else J, n, w.obs_every)
-        elif uniform:
-            s.run(w.J[0], w.q[0], n, w.obs_every)
-        else:
-            s.run_grid(J, q, n, w.obs_every)
-
-    s.init(w.init)
-    run(W)
-    s.synchronize()
-    if world > 1:
-        dist.barrier()
-    torch.cuda.synchronize(dev)
-
     sampler = ClockSampler(local_rank)
-    if rank == 0:
-        sampler.start()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    l0 = s.launch_count
-    e0.record(stream)
-    run(K)
-    e1.record(stream)
-    e1.synchronize()
-    torch.cuda.synchronize(dev)
-    ms = e0.elapsed_time(e1)
-    launches = s.launch_count - l0
+    s, ms, launches, run = time_workload(shaken, torch, dist, w, K, W, dev, stream, rank, world, alt, args.variant,
+                                         before_timed=sampler.start if rank == 0 else None)
     if rank == 0:
         # nvidia-smi needs ~50 ms per sample: keep the same launch sequence running right after the timed region
         # until at least 1.5 s of load has been sampled (records are discarded; obs cadence unchanged)
@@ -359,53 +402,58 @@ def run_ours(args):
                "h2d_bytes_per_step": nsp / K, "d2h_bytes_per_step": (nsp + got * n_local * 48) / K,
                "ms_total": dt * 1e3,
                "what": "shaken_set_spins(sigma) from pinned host + " + ("shaken_run_alternate(K)" if alt else "shaken_run(K)") +
-                       " + shaken_observables + shaken_get_spins(sigma) to host"}
+                       " + shaken_observables + shaken_get_spins(sigma) to host; one upload and one download per run of K "
+                       "steps (step k+1 reads the resident output of step k)"}
 
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return 0
+    s.close()
 
-    # ------------------------------------------------------------------ roofline of the half-step kernel
-    # The half-step is bound by plain integer arithmetic, not by HBM: 32 random bits per site
-    # cost 4.25 IMAD.WIDE (17 per Philox4x32-10 call of 4 sites: rounds 0-1 hoisted, the round-0 product carried by
-    # additions; the plain launches spend 18, which is faster for them), and a warp-wide IMAD.WIDE holds the
-    # SMSP's 16-lane multiplier for 4 cycles.  peak = n_SM * 4 SMSP * 8 lane-multiplies/clk * max SM clock.
-    # The HBM view (BASELINE.json's "% of HBM roofline") is reported next to it.
+    # ------------------------------------------------------------------ rooflines of the half-step kernel
+    # Top level: the HBM roofline BASELINE.json's metric names (2 B per site-update: read one source byte, write one
+    # target byte; 0.25 B bit-packed) against the measured copy bandwidth.  Beside it what actually bounds the path
+    # (DESIGN.md "Rooflines"): the integer multiplier -- 32 random bits per site cost 4.25-4.5 IMAD.WIDE, and a warp-wide
+    # IMAD.WIDE holds an SMSP's 16-lane multiplier for 4 cycles (peak = n_SM x 4 SMSP x 8 lane-multiplies/clk x max SM
+    # clock) -- and the rate of a Philox-only kernel measured in THIS run through the library (no memory traffic at all).
     hbm_peak, peak_src = measured_peak()
-    bytes_per_update = 0.25 if w.packed else 2.0
-    n_half_launches = 2 * K
-    sites_per_launch = n_local * w.L * w.L
-    if alt:
-        # in place on one array: a launch reads and writes the whole array to redraw half of its sites
-        bytes_per_update *= 2.0
-        sites_per_launch //= 2
-    alg_bytes_per_launch = bytes_per_update * sites_per_launch
-    avg_launch_ms = ms / n_half_launches                   # the trailing bond-sum launch (1 of 2K+1) is inside ms
-    hbm_achieved = alg_bytes_per_launch / (avg_launch_ms * 1e-3) / 1e9
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.txt")
-    if os.path.exists(tpath):
-        try:
-            traffic = json.load(open(tpath)).get(w.name + ("_alt" if alt else ""))
-        except Exception:
-            traffic = None
     props = torch.cuda.get_device_properties(dev)
     clk = sampler.summary() or {}
     sm_max_mhz = clk.get("sm_max_mhz") or 1965.0
-    MULS_PER_SITE = 4.25
-    alu_peak = props.multi_processor_count * 4 * 8 * sm_max_mhz * 1e6 / 1e9      # G IMAD.WIDE lane-ops / s
-    alu_achieved = MULS_PER_SITE * sites_per_launch / (avg_launch_ms * 1e-3) / 1e9
-    roofline = {"bound": "alu", "achieved": alu_achieved, "peak": alu_peak, "unit": "G IMAD.WIDE/s", "frac": alu_achieved / alu_peak,
+    philox_only = None
+    try:
+        philox_only = shaken.philox_only_rate()
+    except Exception as e:                                 # the hook must never cost the bench line
+        philox_only = None
+        print("bench.py: philox-only hook failed: %r" % (e,), file=sys.stderr)
+    rl = rooflines(w, alt, ms, K, props.multi_processor_count, sm_max_mhz, hbm_peak, philox_only)
+    traffic, traffic_source = None, None
+    tpath = os.path.join(ROOT, "profiles", "traffic.txt")
+    if os.path.exists(tpath):
+        try:
+            tj = json.load(open(tpath))
+            traffic = tj.get(w.name + ("_alt" if alt else ""))
+            traffic_source = tj.get("source")
+        except Exception:
+            traffic = None
+    kernel = ("alt_half (packed)" if w.packed else "alt_strip_i8") if alt else ("half_step_pk" if w.packed else "half_step_i8")
+    roofline = {"bound": "hbm", "achieved": rl["hbm_achieved"], "peak": hbm_peak, "unit": "GB/s", "frac": rl["hbm_frac"],
                 "traffic": traffic,
-                "peak_source": "derived (DESIGN.md Rooflines): %d SMs x 4 SMSP x 8 wide multiplies/clk x %.0f MHz; 4.25 IMAD.WIDE per site-update"
-                               % (props.multi_processor_count, sm_max_mhz),
-                "kernel": ("alt_half (packed)" if w.packed else "alt_strip_i8") if alt else ("half_step_pk" if w.packed else "half_step_i8"),
-                "algorithmic_ops_per_launch": MULS_PER_SITE * sites_per_launch,
-                "algorithmic_bytes_per_launch": alg_bytes_per_launch, "avg_launch_us": avg_launch_ms * 1e3,
-                "peak_site_updates_per_ns": alu_peak / MULS_PER_SITE,
-                "hbm": {"achieved": hbm_achieved, "peak": hbm_peak, "unit": "GB/s", "frac": hbm_achieved / hbm_peak,
-                        "peak_source": peak_src}}
+                "traffic_source": traffic_source or "profiles/traffic.txt: dram__bytes_read.sum + dram__bytes_write.sum per launch "
+                                                    "from the committed ncu --set full capture of this kernel (not measured in this run)",
+                "peak_source": peak_src, "kernel": kernel,
+                "algorithmic_bytes_per_launch": rl["alg_bytes_per_launch"], "avg_launch_us": rl["avg_launch_us"],
+                "binding_resource": "integer multiplier pipe (Philox4x32-10, 32 random bits per site), not HBM",
+                "alu": {"achieved": rl["alu_achieved"], "peak": rl["alu_peak"], "unit": "G IMAD.WIDE/s", "frac": rl["alu_frac"],
+                        "imad_wide_per_site_update": rl["muls_per_site"],
+                        "peak_source": "derived (DESIGN.md Rooflines): %d SMs x 4 SMSP x 8 wide multiplies/clk x %.0f MHz"
+                                       % (props.multi_processor_count, sm_max_mhz),
+                        "peak_site_updates_per_ns": rl["alu_peak"] / rl["muls_per_site"]},
+                "philox_only_sites_per_ns": philox_only,
+                "frac_of_philox_only": rl["philox_frac"],
+                "philox_only_source": "measured in this run: shaken_selftest_philox_rate (the kernels' own Philox + one compare "
+                                      "per word, no memory traffic), best of 3 launches, CUDA events"}
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
@@ -421,6 +469,32 @@ def run_ours(args):
         "gpu_launches": int(launches),
         "roofline": roofline,
     }
+
+    # ------------------------------------------------------------------ the other workloads of BASELINE.json (north_star:
+    # "report throughput on the five synthetic workloads"), a few hundred ms each, same timing method
+    if world == 1 and not args.no_workloads and args.workload == "cfg4" and not alt:
+        others = {}
+        for name, k in (("cfg1", 2000), ("cfg2", 2000), ("cfg3", 60), ("cfg5", 40)):
+            try:
+                wo = workload(name)
+                so_, ms_o, launches_o, _ = time_workload(shaken, torch, dist, wo, k, 5, dev, stream, 0, 1, False, 0)
+                so_.close()
+                r = rooflines(wo, False, ms_o, k, props.multi_processor_count, sm_max_mhz, hbm_peak, philox_only)
+                others[name] = {"value": 2.0 * wo.n_chains * wo.L * wo.L * k / (ms_o * 1e6), "unit": UNIT, "steps": k,
+                                "ms_per_step": ms_o / k, "us_per_step": 1e3 * ms_o / k, "launches": int(launches_o),
+                                "hbm_frac": r["hbm_frac"], "alu_frac": r["alu_frac"], "frac_of_philox_only": r["philox_frac"],
+                                "layout": "u32 bit-packed" if wo.packed else "int8", "L": wo.L, "n_chains": wo.n_chains,
+                                "obs_every": wo.obs_every}
+                del so_
+                torch.cuda.empty_cache()
+            except Exception as e:
+                others[name] = {"unavailable": repr(e)[:200]}
+        others[w.name] = {"value": value, "unit": UNIT, "steps": K, "ms_per_step": ms / K, "us_per_step": 1e3 * ms / K,
+                          "launches": int(launches), "hbm_frac": rl["hbm_frac"], "alu_frac": rl["alu_frac"],
+                          "frac_of_philox_only": rl["philox_frac"], "layout": "int8", "L": w.L, "n_chains": w.n_chains,
+                          "obs_every": w.obs_every}
+        line["workloads"] = others
+
     if not args.no_cpu_baseline and world == 1:
         line["cpu_baseline"] = cpu_baseline(w, alt)
         try:

@@ -88,10 +88,17 @@ size_t shaken_record_bytes(const shaken_ctx *ctx);
  *                   records; may be NULL with rec_bytes 0 (then the library allocates on demand).
  *   cuda_stream     a cudaStream_t (NULL = the legacy default stream).  All work of this context is
  *                   enqueued on it.
- * The record buffer is zeroed (asynchronously) and the record count reset.  Spins are left untouched.
+ * The record buffer is zeroed (asynchronously) and the record count reset.  The spin buffers are not touched and
+ * their content counts as UNDEFINED: shaken_run / shaken_get_spins / shaken_diag_correlations return SHAKEN_ESTATE
+ * until shaken_init, shaken_set_spins (per layer) or shaken_adopt_spins has defined it.
  * Errors: SHAKEN_EINVAL (null/misaligned), SHAKEN_ECUDA.
  */
 int shaken_bind(shaken_ctx *ctx, void *d_sigma, void *d_tau, void *d_records, size_t rec_bytes, void *cuda_stream);
+
+/* shaken_adopt_spins: declare that the bound DEVICE buffers already hold both layers in device layout (a caller that
+ * filled them with its own kernels).  int8 layers are checked on the device to contain only +1 / -1 bytes
+ * (SHAKEN_EINVAL otherwise; packed words are always valid).  Synchronises the stream.  SHAKEN_ESTATE without buffers. */
+int shaken_adopt_spins(shaken_ctx *ctx);
 
 /* Make room for at least max_records records in a library-owned buffer (existing records are kept).
  * Not allowed on a bound record buffer (SHAKEN_ESTATE). */
@@ -150,6 +157,20 @@ int shaken_run_alternate_grid(shaken_ctx *ctx, const double *J, int64_t n_steps,
  * Returns the number of records copied, or a negative error code.
  */
 int64_t shaken_observables(shaken_ctx *ctx, int64_t *out, int64_t max_records);
+
+/*
+ * shaken_moments: derived statistics of the recorded magnetisation of ONE chain (the paper reports
+ * average and variance of m over the recording window, eq. (17)).  Pure host arithmetic.
+ *   M        HOST, the n values M[0], M[stride], M[2 stride], ... (e.g. out + chain*6 + 0 of shaken_observables with
+ *            stride = n_chains * 6 gives M_sigma of that chain); a burn-in is dropped by offsetting M.
+ *   n        1 <= n < 2^31 records;  n_sites = L*L <= 2^32;  |M| <= n_sites is checked (SHAKEN_EINVAL).
+ *   out      HOST [SHAKEN_N_MOMENTS] doubles: <m>, <|m|>, <m^2>, <m^4>, Var m = <m^2> - <m>^2 (population variance),
+ *            Binder cumulant U = 1 - <m^4> / (3 <m^2>^2) (NaN when every M is 0), with m = M / n_sites.
+ * The power sums are exact integers (M^4 reaches 2^128 at L = 65536: 256-bit accumulation), differences are taken
+ * before rounding, and each result is one long-double division rounded to double: relative error < 1e-15.
+ */
+#define SHAKEN_N_MOMENTS 6
+int shaken_moments(const int64_t *M, int64_t n, int64_t stride, int64_t n_sites, double out[SHAKEN_N_MOMENTS]);
 
 /* Number of records currently stored (>= 0) or a negative error code. */
 int64_t shaken_num_records(const shaken_ctx *ctx);
@@ -219,14 +240,27 @@ int shaken_thresholds(double J, double q, uint32_t out[6]);
  */
 int shaken_philox_words(const uint32_t *ctr, const uint32_t *key, uint32_t *out, int64_t n);
 
+/*
+ * shaken_selftest_philox_rate: measurement hook.  Times, with CUDA events on the default stream, a kernel that runs the
+ * half-step kernels' own Philox4x32-10 (one call per 4 sites, 32 random bits per site) plus one
+ * compare per word and nothing else -- no memory traffic.  The result is the practical ceiling, in site-updates per
+ * ns, of ANY kernel on this device that draws the random numbers this library is specified to draw; bench.py prints it
+ * beside the achieved rate and the HBM roofline.
+ *   blocks_per_sm 1..8 (256 threads each), iters calls of 4 x 4 sites per thread, best of reps timed launches after a warm-up.
+ *   sites_per_ns  HOST, receives the rate.
+ */
+int shaken_selftest_philox_rate(int32_t blocks_per_sm, int32_t iters, int32_t reps, double *sites_per_ns);
+
 /* Number of kernels this context has launched so far (half-steps, init, conversions, reductions). */
 int64_t shaken_launch_count(const shaken_ctx *ctx);
 
-/* Kernel variant: 0 = automatic (default); other values select a specific code path for measurement and tests
- * (DESIGN.md "Kernels"): 1 PRMT index extraction, 2 the round-1 v2 kernel, 3 generic strip kernels also for L <= 128,
- * 4 shared-memory index extraction, 5 paired lookup, 6 IDP extraction, 7 two 256-thread blocks per SM, 8 per-warp task lists,
- * 9 paired lookup with tensor-core observable sums.  shaken_run_alternate only distinguishes 0 from the rest: any other
- * value keeps it on the per-half-step kernels also for L <= 128.  Results never depend on the variant. */
+/* Code-path switch for tests and measurements; results never depend on it.  0 = automatic (default).
+ * SHAKEN_VARIANT_STRIPS: every lattice size takes the per-half-step strip kernels (automatic would run L <= 128 in the
+ * one-launch shared-memory kernel and mid-size lattices in the one-launch band kernel); applies to shaken_run and
+ * shaken_run_alternate.  SHAKEN_VARIANT_PERWARP: strip kernels with per-warp task lists (automatic for batches of small
+ * chains).  Any other value: SHAKEN_EINVAL. */
+#define SHAKEN_VARIANT_STRIPS 3
+#define SHAKEN_VARIANT_PERWARP 8
 int shaken_set_variant(shaken_ctx *ctx, int variant);
 
 /* Message for the most recent error on this context ("" if none).  ctx may be NULL (creation errors). */

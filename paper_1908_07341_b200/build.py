@@ -53,16 +53,5 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
-def build_pipe_rates() -> str:
-    """The measurement tool csrc/pipe_rates.cu (integer-pipe issue intervals, Philox-only rate) as an executable."""
-    exe = os.path.join(HERE, "pipe_rates")
-    src = os.path.join(CSRC, "pipe_rates.cu")
-    if not os.path.exists(exe) or os.path.getmtime(exe) < max(os.path.getmtime(src), os.path.getmtime(os.path.join(CSRC, "philox.cuh"))):
-        subprocess.check_call([nvcc_path(), "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-o", exe, src], cwd=HERE)
-    return exe
-
-
 if __name__ == "__main__":
     print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
-    if "--pipe-rates" in sys.argv:
-        print(build_pipe_rates())

@@ -3,8 +3,8 @@
 // run is ONE cooperative launch.  Every CTA owns a band of rows of one chain and keeps both sublattices of the band in
 // shared memory; per half-step it needs exactly one row from a neighbouring band (eq. (14): the field
 // uses the down row in half 0, the up row in half 1), which the neighbour publishes through a small global buffer in
-// "data + stamp" form: every 8-byte store carries the spin word and the half-step stamp, so a reader that sees the
-// stamp has the data (no fence, no separate flag).  A CTA computes the row its neighbour waits for first, one word per
+// "data + stamp" form: every 64-bit store carries the spin word and the half-step stamp, so a reader that sees the
+// stamp has the data (no fence, no separate flag; see st_pair).  A CTA computes the row its neighbour waits for first, one word per
 // thread, and every word is published by the thread that computed it; one warp does no arithmetic and polls for the
 // row the CTA itself needs next.  There is no grid-wide barrier: only neighbouring
 // bands wait for each other, which is why all CTAs must be co-resident -- the cooperative launch guarantees it.
@@ -39,11 +39,18 @@ struct BandParams {
     uint32_t stamp0;         // stamps of this launch are stamp0 + 1 .. stamp0 + 2 n_steps (never seen before in xs, xt)
 };
 
-__device__ __forceinline__ uint2 ld_relaxed_v2(const uint2 *p)
+// A {word, stamp} pair crosses between CTAs as ONE naturally aligned 64-bit scalar access, relaxed at gpu scope on both
+// sides: the PTX memory model makes such an access single-copy atomic (a vector access would count as two scalar ones),
+// so a reader that sees the stamp of a half-step has the spin word written with it.  No fence, no flag.
+__device__ __forceinline__ uint2 ld_pair(const uint2 *p)
 {
-    uint2 v;
-    asm volatile("ld.relaxed.gpu.global.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "l"(p) : "memory");
-    return v;
+    unsigned long long v;
+    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return make_uint2((uint32_t)v, (uint32_t)(v >> 32));
+}
+__device__ __forceinline__ void st_pair(uint2 *p, uint32_t word, uint32_t stamp)
+{
+    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" :: "l"(p), "l"(((unsigned long long)stamp << 32) | word) : "memory");
 }
 
 __global__ void __launch_bounds__(BAND_THREADS, 1) band_run_i8(const __grid_constant__ BandParams p)
@@ -137,9 +144,8 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) band_run_i8(const __grid_cons
         }
         *reinterpret_cast<uint4 *>(dst + at) = make_uint4(o[0], o[1], o[2], o[3]);
         if (rr == 0) {                            // (tall bands only, see below) a vector of the row the neighbour waits for
-            uint4 *x = reinterpret_cast<uint4 *>(xmine + 4 * cv);
-            __stcg(x, make_uint4(o[0], stamp, o[1], stamp));
-            __stcg(x + 1, make_uint4(o[2], stamp, o[3], stamp));
+#pragma unroll
+            for (int j = 0; j < 4; ++j) st_pair(xmine + 4 * cv + j, o[j], stamp);
         }
     };
 
@@ -157,7 +163,7 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) band_run_i8(const __grid_cons
         const uint32_t hw = half ? __funnelshift_r(sw, e, 8) : __funnelshift_l(e, sw, 8);
         const uint32_t out = update_word(sw, hw, halo[cw], (uint32_t)(r0 + r) * (uint32_t)W + (uint32_t)cw);
         dst[at] = out;
-        __stcg(xmine + cw, make_uint2(out, stamp));
+        st_pair(xmine + cw, out, stamp);
     };
 
     // block-wide sums of up to six int partials into one record (int64 atomics: bands of a chain share the record)
@@ -201,7 +207,7 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) band_run_i8(const __grid_cons
             do {
                 ok = true;
 #pragma unroll
-                for (int j = 0; j < 8; ++j) v[j] = ld_relaxed_v2(src + min(i0 + j * 32 + lane, W - 1));
+                for (int j = 0; j < 8; ++j) v[j] = ld_pair(src + min(i0 + j * 32 + lane, W - 1));
 #pragma unroll
                 for (int j = 0; j < 8; ++j)
                     if (v[j].y != stamp) ok = false;

@@ -2,26 +2,27 @@
 //
 // Spins are bytes 0x01 (+1) / 0xFF (-1): bit 0 is always 1 and every bit 1..7 of a byte is the "minus" flag m.
 //
-// Pipe budget on sm_100a (measured, profiles/r1_ubench.md): a 32x32->64 multiply (IMAD.WIDE) costs two slots
-// of the 64-lane/clk FMA-heavy pipe, so the 18 multiplies of one hoisted Philox call (4 sites) alone cap the
-// kernel at 64 / 9 = 7.1 site-updates per clock per SM.  Everything else is therefore kept OFF that pipe:
-// field/index arithmetic is byte-SIMD logic on the ALU pipe (4 sites per instruction), the threshold comes
-// from shared memory through the LSU, the compare is ISETP plus one predicated XOR.
+// Pipe budget on sm_100a (measured, profiles/r2_pipe_rates.md): a 32x32->64 multiply (IMAD.WIDE) holds the 16-lane
+// multiplier pipe of an SM sub-partition for 4.2 cycles per warp, so the 17-18 multiplies of one hoisted Philox call
+// (4 sites) alone cap the kernel near 7 site-updates per clock per SM.  Everything else is therefore kept OFF that
+// pipe where possible: field/index arithmetic is byte-SIMD logic on the ALU pipe (4 sites per instruction), the
+// threshold comes from shared memory through the LSU, the compare is ISETP plus one predicated add.
 //
 // Index encoding.  For one 32-bit word (4 sites) with self word s, vertical neighbour word v and horizontal
 // neighbour word h (byte funnel shift of s with the adjacent word):
 //   z = bitwise select of (s, h, v) = {bits 0,1: 0, bit 3: m_s, bit 4: m_h, bits 2,5,6,7: m_v} per byte: three
 //   LOP3, no addition.  The byte is directly the BYTE OFFSET of the threshold in a 256-byte shared-memory table
 //   in which only the 8 reachable words are filled (8 distinct banks: the lookup never conflicts).
-//   EXTRACT_PRMT : one PRMT per site moves its byte of z into a register (ALU pipe).
-//   EXTRACT_SMEM : the four z words go to a per-thread shared-memory slot and come back one byte at a time
-//                  (LDS.U8): LSU slots instead of ALU slots.
+//   The four z words go to a per-thread shared-memory slot and come back one byte at a time (LDS.U8): LSU slots
+//   instead of ALU slots (EXTRACT_SMEM).  Plain half-steps of block tasks use the paired lookup instead (EXTRACT_PAIR).
+//   (Measured and dropped in round 1: PRMT extraction, IDP.4A extraction, 2 x 256-thread blocks per SM,
+//   one row of prefetch, XOR packing, observable sums on the tensor cores through int8 mma.sync.)
 #pragma once
 #include "kernels_common.cuh"
 
 namespace shaken {
 
-enum : int { EXTRACT_PRMT = 0, EXTRACT_SMEM = 1, EXTRACT_IDP = 2, EXTRACT_PAIR = 3, PACK_ADD = 16, PREFETCH2 = 32, PER_WARP = 64, OBS_MMA = 128 };
+enum : int { EXTRACT_SMEM = 1, EXTRACT_PAIR = 3 };
 
 // byte the EXTRACT_SMEM encoding produces for minus flags (ms, mh, mv)
 __host__ __device__ constexpr uint32_t smem_code(int ms, int mh, int mv)
@@ -29,24 +30,18 @@ __host__ __device__ constexpr uint32_t smem_code(int ms, int mh, int mv)
     return ((uint32_t)ms << 3) | ((uint32_t)mh << 4) | (mv ? 0xE4u : 0u);
 }
 
-template <int HALF, int FLAGS, int EXTRACT_, int MINB, int THREADS = BLOCK_THREADS>
-__global__ void __launch_bounds__(THREADS, MINB) half_step_i8(const __grid_constant__ StepParams p)
+template <int HALF, int FLAGS, bool PERWARP>
+__global__ void __launch_bounds__(I8_THREADS, 1) half_step_i8(const __grid_constant__ StepParams p)
 {
+    constexpr int THREADS = I8_THREADS;
     constexpr int WPB = THREADS / 32;                       // warp strips per block task
-    constexpr int EXTRACT = EXTRACT_ & 15;
-    constexpr bool PACKADD = (EXTRACT_ & PACK_ADD) != 0;
-    constexpr int AHEAD = (EXTRACT_ & PREFETCH2) ? 2 : 1;   // rows between a load and its first use
     // PER_WARP: a task is ONE warp strip and every warp walks its own task list with its own threshold table, so warps
     // of a block may work on different chains and never wait for each other (many small chains: the strips can be
     // tall and the last wave full at warp granularity).  Otherwise a task is WPB strips of one chain per block.
-    constexpr bool PERWARP = (EXTRACT_ & PER_WARP) != 0;
-    // OBS_MMA: the observable sums are spin-product dot products, i.e. a (small) dense contraction: they go to the tensor
-    // cores (int8 mma.sync, otherwise idle) instead of IDP.4A, which shares the multiplier pipe with Philox's IMAD.WIDE --
-    // the one pipe this kernel is short of.  With A rows = two operand vectors of a lane group and B column g = the
-    // common factor of the same lane group, the DIAGONAL C[g][g], C[g+8][g] holds the two wanted dot products; the
-    // off-diagonal entries (products across lane groups) are ignored.  Needs all 32 lanes in the row loop.
-    constexpr bool OBSMMA = (EXTRACT_ & OBS_MMA) != 0 && (FLAGS & (F_OBS | F_BONDS)) != 0;
-    static_assert(!PERWARP || EXTRACT != EXTRACT_PAIR, "the paired table (16 KiB) exists once per block");
+    // Lookup: launches that also accumulate observables keep the multiplier pipe free of extra IDP.4A (index bytes go
+    // through shared memory); plain half-steps of block tasks use the paired lookup (one IDP.4A + one LDS.64 per two
+    // sites), which needs a 16 KiB table per block and so is not available to per-warp lists.
+    constexpr int EXTRACT = (PERWARP || (FLAGS & (F_OBS | F_BONDS)) != 0) ? EXTRACT_SMEM : EXTRACT_PAIR;
     constexpr bool OBS = (FLAGS & F_OBS) != 0;
     constexpr bool BONDS = (FLAGS & F_BONDS) != 0;
     constexpr bool UPDATE = (FLAGS & F_NOUPDATE) == 0;
@@ -75,20 +70,8 @@ __global__ void __launch_bounds__(THREADS, MINB) half_step_i8(const __grid_const
     int cur_chain = -1;
     ChainKeys ck = {0u, 0u};
     int cnt0 = 0, cnt1 = 0, cnt2 = 0;   // half 1: M_sigma, E_J, E_q ; half 0: M_tau, C_x, C_y
-    int acc1[4] = {0, 0, 0, 0}, acc2[4] = {0, 0, 0, 0};   // OBS_MMA accumulators (see do_row)
 
     auto flush = [&](int chain) {
-        if (OBSMMA) {
-            // lane (g, t) holds C[g][2t], C[g][2t+1], C[g+8][2t], C[g+8][2t+1]: the diagonal sits at t = g / 2
-            const int g = lane >> 2, t = lane & 3;
-            const bool diag = t == (g >> 1), odd = g & 1;
-            const int d1a = odd ? acc1[1] : acc1[0], d1b = odd ? acc1[3] : acc1[2];
-            const int d2a = odd ? acc2[1] : acc2[0], d2b = odd ? acc2[3] : acc2[2];
-            if (HALF == 1) { cnt2 = diag ? d1a : 0; cnt1 = diag ? d1b + d2a : 0; cnt0 = diag ? d2b : 0; }
-            else           { cnt1 = diag ? d1a : 0; cnt2 = diag ? d1b : 0; cnt0 = diag ? d2a : 0; }
-#pragma unroll
-            for (int i = 0; i < 4; ++i) acc1[i] = acc2[i] = 0;
-        }
         if (HALF == 1) {
             if (OBS) {
                 warp_add_to(p.rec_cur + (size_t)chain * 6 + 0, cnt0);
@@ -156,10 +139,8 @@ __global__ void __launch_bounds__(THREADS, MINB) half_step_i8(const __grid_const
         }
         const int seg = lt % p.nseg;
         const int rb = lt / p.nseg;
-        const int cvl = seg * 32 + lane;
-        const bool live = cvl < p.nvec;                  // OBS_MMA keeps dead lanes of a ragged strip in the loop (mma.sync
-        const int cv = OBSMMA ? min(cvl, p.nvec - 1) : cvl;   // is warp-wide): they recompute the last vector and contribute 0
-        if (lt < tpc && (OBSMMA || live)) {
+        const int cv = seg * 32 + lane;
+        if (lt < tpc && cv < p.nvec) {
             const int c0 = cv * 16;
             const int r_first = rb * R;
             const int r_last = min(L, r_first + R) - 1;
@@ -214,7 +195,7 @@ __global__ void __launch_bounds__(THREADS, MINB) half_step_i8(const __grid_const
                 }
 #pragma unroll
                 for (int j = 0; j < 4; ++j) {
-                    uint32_t out = PACKADD ? 0x01010101u : 0xFFFFFFFFu;
+                    uint32_t out = 0x01010101u;
                     if (UPDATE) {
                         uint32_t rw[4];
                         if constexpr (PRODUCT) {
@@ -235,27 +216,18 @@ __global__ void __launch_bounds__(THREADS, MINB) half_step_i8(const __grid_const
 #pragma unroll
                         for (int b = 0; b < 4; ++b) {
                             if (EXTRACT == EXTRACT_PAIR) {
-                                if (PACKADD) out = add_if_not_less(out, rw[b], Tp[b], 0xFEu << (8 * b));
-                                else out = xor_if_less(out, rw[b], Tp[b], 0xFEu << (8 * b));
+                                out = add_if_not_less(out, rw[b], Tp[b], 0xFEu << (8 * b));
                                 continue;
                             }
-                            uint32_t code;
-                            if (EXTRACT == EXTRACT_SMEM)
-                                code = reinterpret_cast<volatile const uint8_t *>(my_idx + j * THREADS)[b];
-                            else if (EXTRACT == EXTRACT_IDP)
-                                code = __dp4a(zw[j], 1u << (8 * b), 0u);      // byte b of zw[j] on the multiplier pipe
-                            else
-                                code = b == 3 ? (zw[j] >> 24) : __byte_perm(zw[j], 0u, 0x4440u + b);
+                            const uint32_t code = reinterpret_cast<volatile const uint8_t *>(my_idx + j * THREADS)[b];
                             const uint32_t T = *reinterpret_cast<const uint32_t *>(reinterpret_cast<const char *>(s_tab) + code);
-                            if (PACKADD) out = add_if_not_less(out, rw[b], T, 0xFEu << (8 * b));
-                            else out = xor_if_less(out, rw[b], T, 0xFEu << (8 * b));
+                            out = add_if_not_less(out, rw[b], T, 0xFEu << (8 * b));
                         }
                         ow[j] = out;
                     }
                     // observables: spins are signed bytes +-1, so a sum of spin products over 4 sites is ONE
                     // signed 8-bit dot product (IDP.4A) accumulated in int32 -- exact, no masks, no flushes
                     const int s = (int)w[j], v = (int)vw[j], hh = (int)hw[j], o = (int)out;
-                    if (OBSMMA) continue;
                     if (HALF == 1) {
                         if (OBS) {
                             cnt0 = __dp4a(o, 0x01010101, cnt0);   // M_sigma  = sum sigma'_x
@@ -271,56 +243,24 @@ __global__ void __launch_bounds__(THREADS, MINB) half_step_i8(const __grid_const
                         }
                     }
                 }
-                if (OBSMMA) {
-                    // words (0,1) then (2,3) of the 16-byte vector: a0/a2 = first operand vector (rows g), a1/a3 = second
-                    // operand vector (rows g+8), b0/b1 = common factor (column g); dead lanes contribute zeros
-                    const uint32_t ONES = 0x01010101u;
-                    if (HALF == 1) {
-                        const uint32_t o0 = live ? ow[0] : 0u, o1 = live ? ow[1] : 0u, o2 = live ? ow[2] : 0u, o3 = live ? ow[3] : 0u;
-                        mma_s8(acc1, w[0], vw[0], w[1], vw[1], o0, o1);       // rows g: tau_x (E_q),  rows g+8: tau_up (E_J)
-                        mma_s8(acc1, w[2], vw[2], w[3], vw[3], o2, o3);
-                        mma_s8(acc2, hw[0], ONES, hw[1], ONES, o0, o1);       // rows g: tau_right (E_J), rows g+8: 1 (M_sigma)
-                        mma_s8(acc2, hw[2], ONES, hw[3], ONES, o2, o3);
-                    } else {
-                        if (BONDS) {
-                            const uint32_t s0 = live ? w[0] : 0u, s1 = live ? w[1] : 0u, s2 = live ? w[2] : 0u, s3 = live ? w[3] : 0u;
-                            mma_s8(acc1, hw[0], vw[0], hw[1], vw[1], s0, s1);  // rows g: sigma_left (C_x), rows g+8: sigma_down (C_y)
-                            mma_s8(acc1, hw[2], vw[2], hw[3], vw[3], s2, s3);
-                        }
-                        if (OBS) {
-                            mma_s8(acc2, ONES, 0u, ONES, 0u, live ? ow[0] : 0u, live ? ow[1] : 0u);   // rows g: 1 (M_tau)
-                            mma_s8(acc2, ONES, 0u, ONES, 0u, live ? ow[2] : 0u, live ? ow[3] : 0u);
-                        }
-                    }
-                }
-                if (UPDATE && (!OBSMMA || live)) *reinterpret_cast<uint4 *>(pd) = make_uint4(ow[0], ow[1], ow[2], ow[3]);
+                if (UPDATE) *reinterpret_cast<uint4 *>(pd) = make_uint4(ow[0], ow[1], ow[2], ow[3]);
                 pc += stride; pe += stride; pd += stride;
                 if constexpr (PRODUCT) add64(ph, pl, pstep_hi, pstep_lo);
                 else n += nstep;
             };
 
-            // three row buffers rotate roles (vertical neighbour / current / prefetched) without register moves
-            uint4 B0 = ldg128(sbase + (size_t)rh * L + c0), B1 = ldg128(pc), B2 = B1;
-            uint32_t e0 = 0, e1 = ldg32(pe), e2 = 0;
+            // four row buffers rotate roles (vertical neighbour / current / two prefetched rows) without register moves:
+            // the row loaded while row i is computed is row i + 2
+            uint4 B0 = ldg128(sbase + (size_t)rh * L + c0), B1 = ldg128(pc), B2 = B1, B3 = B1;
+            uint32_t e0 = 0, e1 = ldg32(pe), e2 = 0, e3 = 0;
             pc += stride; pe += stride;
-            if (AHEAD == 1) {
-                for (int i = 0;;) {
-                    do_row(B1, B0, e1, B2, e2, i + 1 < rows); if (++i == rows) break;
-                    do_row(B2, B1, e2, B0, e0, i + 1 < rows); if (++i == rows) break;
-                    do_row(B0, B2, e0, B1, e1, i + 1 < rows); if (++i == rows) break;
-                }
-            } else {
-                // four buffers: the row loaded while row i is computed is row i + 2
-                uint4 B3 = B1;
-                uint32_t e3 = 0;
-                if (rows > 1) { B2 = ldg128(pc); e2 = ldg32(pe); }
-                pc += stride; pe += stride;
-                for (int i = 0;;) {
-                    do_row(B1, B0, e1, B3, e3, i + 2 < rows); if (++i == rows) break;
-                    do_row(B2, B1, e2, B0, e0, i + 2 < rows); if (++i == rows) break;
-                    do_row(B3, B2, e3, B1, e1, i + 2 < rows); if (++i == rows) break;
-                    do_row(B0, B3, e0, B2, e2, i + 2 < rows); if (++i == rows) break;
-                }
+            if (rows > 1) { B2 = ldg128(pc); e2 = ldg32(pe); }
+            pc += stride; pe += stride;
+            for (int i = 0;;) {
+                do_row(B1, B0, e1, B3, e3, i + 2 < rows); if (++i == rows) break;
+                do_row(B2, B1, e2, B0, e0, i + 2 < rows); if (++i == rows) break;
+                do_row(B3, B2, e3, B1, e1, i + 2 < rows); if (++i == rows) break;
+                do_row(B0, B3, e0, B2, e2, i + 2 < rows); if (++i == rows) break;
             }
         }
     }

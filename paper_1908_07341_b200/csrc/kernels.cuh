@@ -156,15 +156,15 @@ __global__ void coalesce_finalize(long long *coal, const unsigned long long *dif
 //   out[chain][e][0] = sum sigma[r][c] sigma[r+l][c+l]  (SW-NE),  out[chain][e][1] = sum sigma[r+l][c] sigma[r][c+l]  (NW-SE).
 // One thread per 32-bit word of row r; the partner word, l columns to the right, is a funnel shift of two aligned
 // words (int8: by 8 (l mod 4) bits, products by IDP.4A; packed: by l mod 32 bits, products by popcount of the XOR).
-// grid = (blocks per chain, n_chains); one int64 atomic per warp and sum.
+// grid = (blocks per chain, min(n_chains, 65535)), chains beyond gridDim.y are looped over; one int64 atomic per warp and sum.
 template <bool PACKED>
-__global__ void diag_corr(const uint32_t *sigma, int L, int ell, long long *out, int n_ell, int e)
+__global__ void diag_corr(const uint32_t *sigma, int L, int n_chains, int ell, long long *out, int n_ell, int e)
 {
     const int SPW = PACKED ? 32 : 4;                    // sites per word
-    const int W = L / SPW;
-    const int chain = blockIdx.y;
-    const uint32_t *sg = sigma + (size_t)chain * L * W;
+    const int W = L / SPW;                              // L * W <= 2^30: the int indices below cannot overflow
     const int wsh = ell / SPW, sh = (ell % SPW) * (PACKED ? 1 : 8);
+    for (int chain = blockIdx.y; chain < n_chains; chain += gridDim.y) {
+    const uint32_t *sg = sigma + (size_t)chain * L * W;
     long long swne = 0, nwse = 0;
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < L * W; i += gridDim.x * blockDim.x) {
         const int r = i / W, cw = i - r * W;
@@ -190,6 +190,27 @@ __global__ void diag_corr(const uint32_t *sigma, int L, int ell, long long *out,
         atomicAdd(reinterpret_cast<unsigned long long *>(dst), (unsigned long long)swne);
         atomicAdd(reinterpret_cast<unsigned long long *>(dst + 1), (unsigned long long)nwse);
     }
+    }
+}
+
+// Measurement hook (shaken_selftest_philox_rate): the half-step kernels' own hoisted Philox4x32-10 (philox.cuh: 18
+// IMAD.WIDE + 19 LOP3 per call of 4 sites) with one compare-and-count per random word and NOTHING else -- no loads, no
+// stores, no neighbours, no table.  Its rate is the practical ceiling of any kernel that draws 32 Philox bits per site
+// on this chip (SURVEY 8(d) "first experiment of the build"); bench.py reports it beside the HBM fraction.
+__global__ void __launch_bounds__(256) philox_rate(uint32_t *out, const __grid_constant__ StepKeys K, int iters)
+{
+    const ChainKeys ck = make_chain_keys(K, 0u);
+    uint32_t n = (blockIdx.x * 256u + threadIdx.x) * 4u * (uint32_t)iters, acc = 0;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            uint32_t r[4];
+            philox_site_words(n + j, K, ck, r);
+            acc += (r[0] < 0x80000000u) + (r[1] < 0x70000000u) + (r[2] < 0x60000000u) + (r[3] < 0x50000000u);
+        }
+        n += 4;
+    }
+    if (acc == 0x12345678u) out[0] = acc;          // keeps the arithmetic alive; practically never taken
 }
 
 __global__ void philox_hook(const uint32_t *ctr, const uint32_t *key, uint32_t *out, long long n)

@@ -19,8 +19,6 @@
 
 namespace shaken {
 
-constexpr int WARPS_PER_BLOCK = 8;
-constexpr int BLOCK_THREADS = WARPS_PER_BLOCK * 32;
 constexpr int I8_THREADS = 512;         // int8 half-step: one 512-thread block per SM, up to 128 registers per thread
 constexpr int MAX_ROWS_PER_TASK = 4096;   // int32 observable partials: 2 * 512 * rows per warp stay far below 2^31
 
@@ -58,15 +56,6 @@ __device__ __forceinline__ void warp_add_to(long long *addr, int v)
 {
     int s = __reduce_add_sync(0xFFFFFFFFu, v);
     if ((threadIdx.x & 31) == 0 && s != 0) atomicAdd(reinterpret_cast<unsigned long long *>(addr), (unsigned long long)(long long)s);
-}
-
-// C += A * B for one warp: A 16 x 32, B 32 x 8, signed bytes, int32 accumulators (mma.sync m16n8k32).  Fragment layout
-// with g = lane / 4, t = lane % 4: a0 = A[g][4t..4t+3], a1 = A[g+8][4t..], a2 = A[g][16+4t..], a3 = A[g+8][16+4t..];
-// b0 = B[4t..4t+3][g], b1 = B[16+4t..][g]; c0 = C[g][2t], c1 = C[g][2t+1], c2 = C[g+8][2t], c3 = C[g+8][2t+1].
-__device__ __forceinline__ void mma_s8(int (&c)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, uint32_t b0, uint32_t b1)
-{
-    asm("mma.sync.aligned.m16n8k32.row.col.s32.s8.s8.s32 {%0, %1, %2, %3}, {%4, %5, %6, %7}, {%8, %9}, {%0, %1, %2, %3};"
-        : "+r"(c[0]), "+r"(c[1]), "+r"(c[2]), "+r"(c[3]) : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
 }
 
 // Programmatic dependent launch: the half-step kernels of a run are launched back to back with

@@ -46,7 +46,7 @@ struct shaken_ctx {
     cudaStream_t stream = nullptr;
     uint64_t step = 0;
     uint32_t chain0 = 0;
-    bool have_spins = false;
+    bool have_sigma = false, have_tau = false;   // the layer holds defined +-1 content (init, set_spins, adopt, or a run)
     int num_sms = 0;
     int variant = 0;
     int group = 1;                // coupling group size (shaken_set_coupling)
@@ -142,7 +142,7 @@ extern "C" int shaken_create(shaken_ctx **out, int32_t L, int32_t n_chains, uint
 extern "C" int shaken_destroy(shaken_ctx *ctx)
 {
     if (!ctx) return SHAKEN_OK;
-    if (ctx->have_spins || ctx->d_rec || ctx->d_tab) cudaStreamSynchronize(ctx->stream);
+    if (ctx->have_sigma || ctx->have_tau || ctx->d_rec || ctx->d_tab) cudaStreamSynchronize(ctx->stream);
     if (ctx->own_spins) { cudaFree(ctx->d_sigma); cudaFree(ctx->d_tau); }
     if (ctx->own_rec) cudaFree(ctx->d_rec);
     cudaFree(ctx->d_tab);
@@ -208,7 +208,7 @@ extern "C" int shaken_bind(shaken_ctx *ctx, void *d_sigma, void *d_tau, void *d_
         return fail(ctx, SHAKEN_EINVAL, "shaken_bind: records pointer / size mismatch or misaligned");
     int rc = ensure_device(ctx);
     if (rc) return rc;
-    if (ctx->have_spins || ctx->d_rec) CU(cudaStreamSynchronize(ctx->stream));
+    if (ctx->have_sigma || ctx->have_tau || ctx->d_rec) CU(cudaStreamSynchronize(ctx->stream));
     if (ctx->own_spins) { cudaFree(ctx->d_sigma); cudaFree(ctx->d_tau); ctx->own_spins = false; }
     if (ctx->own_rec) { cudaFree(ctx->d_rec); ctx->own_rec = false; }
     ctx->d_sigma = d_sigma;
@@ -218,7 +218,7 @@ extern "C" int shaken_bind(shaken_ctx *ctx, void *d_sigma, void *d_tau, void *d_
     ctx->rec_cap = d_records ? (int64_t)(rec_bytes / shaken_record_bytes(ctx)) : 0;
     ctx->rec_bound = d_records != nullptr;
     ctx->n_rec = 0;
-    ctx->have_spins = true;   // the caller's buffers hold whatever the caller put there
+    ctx->have_sigma = ctx->have_tau = false;   // content unknown until shaken_init / shaken_set_spins / shaken_adopt_spins
     if (d_records) CU(cudaMemsetAsync(d_records, 0, (size_t)ctx->rec_cap * shaken_record_bytes(ctx), ctx->stream));
     return SHAKEN_OK;
 }
@@ -306,7 +306,8 @@ extern "C" int64_t shaken_launch_count(const shaken_ctx *ctx) { return ctx ? ctx
 
 extern "C" int shaken_set_variant(shaken_ctx *ctx, int variant)
 {
-    if (!ctx || variant < 0) return SHAKEN_EINVAL;
+    if (!ctx || (variant != 0 && variant != SHAKEN_VARIANT_STRIPS && variant != SHAKEN_VARIANT_PERWARP))
+        return fail(ctx, SHAKEN_EINVAL, "shaken_set_variant: unknown variant %d", variant);
     ctx->variant = variant;
     return SHAKEN_OK;
 }
@@ -406,7 +407,7 @@ extern "C" int shaken_init(shaken_ctx *ctx, int mode)
         CU(cudaMemsetAsync(ctx->d_sigma, byte, nb, ctx->stream));
         CU(cudaMemsetAsync(ctx->d_tau, byte, nb, ctx->stream));
     }
-    ctx->have_spins = true;
+    ctx->have_sigma = ctx->have_tau = true;
     ctx->step = 0;
     int rcc = reset_coalescence(ctx);
     if (rcc) return rcc;
@@ -436,26 +437,11 @@ static void launch_pdl(K kernel, int grid, int threads, cudaStream_t stream, con
 template <int HALF, int FLAGS>
 static cudaError_t launch_half(const shaken_ctx *ctx, const StepParams &p, int grid)
 {
-    // int8 code paths (results identical).  Automatic choice: launches that also accumulate
-    // observables keep the multiplier pipe free of extra IDP.4A (index bytes go through shared memory), plain
-    // half-steps use the paired lookup (one IDP.4A + one LDS.64 per two sites).
-    constexpr int TUNED = PACK_ADD | PREFETCH2;
-    constexpr int AUTO = ((FLAGS & (F_OBS | F_BONDS)) ? EXTRACT_SMEM : EXTRACT_PAIR) | TUNED;
+    // int8: block tasks (one threshold table per block; plain half-steps use the paired lookup) or per-warp task
+    // lists (kernel_i8.cuh); results are identical
     if (ctx->packed) launch_pdl(half_step_pk<HALF, FLAGS>, grid, PK_THREADS, ctx->stream, p);
-    else switch (ctx->variant) {
-        case 1: launch_pdl(half_step_i8<HALF, FLAGS, EXTRACT_PRMT | TUNED, 1, I8_THREADS>, grid, I8_THREADS, ctx->stream, p); break;
-        case 2: launch_pdl(half_step_i8<HALF, FLAGS, EXTRACT_SMEM, 2>, grid, BLOCK_THREADS, ctx->stream, p); break;   // round-1 v2 kernel
-        case 4: launch_pdl(half_step_i8<HALF, FLAGS, EXTRACT_SMEM | TUNED, 1, I8_THREADS>, grid, I8_THREADS, ctx->stream, p); break;
-        case 5: launch_pdl(half_step_i8<HALF, FLAGS, EXTRACT_PAIR | TUNED, 1, I8_THREADS>, grid, I8_THREADS, ctx->stream, p); break;
-        case 6: launch_pdl(half_step_i8<HALF, FLAGS, EXTRACT_IDP | TUNED, 1, I8_THREADS>, grid, I8_THREADS, ctx->stream, p); break;
-        case 7: launch_pdl(half_step_i8<HALF, FLAGS, AUTO, 2>, grid, BLOCK_THREADS, ctx->stream, p); break;          // 2 x 256 threads
-        case 9: launch_pdl(half_step_i8<HALF, FLAGS, EXTRACT_PAIR | TUNED | OBS_MMA, 1, I8_THREADS>, grid, I8_THREADS, ctx->stream, p); break;
-        case 8: launch_pdl(half_step_i8<HALF, FLAGS, EXTRACT_SMEM | TUNED | PER_WARP, 1, I8_THREADS>, grid, I8_THREADS, ctx->stream, p); break;
-        default:
-            if (ctx->perwarp) launch_pdl(half_step_i8<HALF, FLAGS, EXTRACT_SMEM | TUNED | PER_WARP, 1, I8_THREADS>, grid, I8_THREADS, ctx->stream, p);
-            else launch_pdl(half_step_i8<HALF, FLAGS, AUTO, 1, I8_THREADS>, grid, I8_THREADS, ctx->stream, p);
-            break;
-    }
+    else if (ctx->perwarp) launch_pdl(half_step_i8<HALF, FLAGS, true>, grid, I8_THREADS, ctx->stream, p);
+    else launch_pdl(half_step_i8<HALF, FLAGS, false>, grid, I8_THREADS, ctx->stream, p);
     return cudaGetLastError();
 }
 
@@ -492,7 +478,7 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
     const int nJ = uniform ? 1 : ctx->n_chains;
     for (int i = 0; i < nJ; ++i)
         if (!isfinite(J[i]) || !isfinite(q[i])) return fail(ctx, SHAKEN_EINVAL, "shaken_run: non-finite coupling for chain %d", i);
-    if (!ctx->have_spins || !ctx->d_sigma) return fail(ctx, SHAKEN_ESTATE, "shaken_run: no spins yet (call shaken_init or shaken_set_spins)");
+    if (!ctx->have_sigma || !ctx->d_sigma) return fail(ctx, SHAKEN_ESTATE, "shaken_run: no sigma yet (call shaken_init, shaken_set_spins or shaken_adopt_spins)");
     int rc = ensure_device(ctx);
     if (rc) return rc;
     if (n_steps == 0) return SHAKEN_OK;
@@ -513,27 +499,26 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
     p.chain0 = ctx->chain0;
     p.group = ctx->group;
     p.nseg = (p.nvec + 31) / 32;
-    int resident = 2, wpb = WARPS_PER_BLOCK;                  // resident blocks per SM (launch bounds), warps per block
-    if (ctx->packed) { resident = 1; wpb = PK_THREADS / 32; }
-    else if (ctx->variant != 2 && ctx->variant != 7) { resident = 1; wpb = I8_THREADS / 32; }
+    const int resident = 1;                                   // resident blocks per SM (launch bounds)
+    int wpb = ctx->packed ? PK_THREADS / 32 : I8_THREADS / 32;   // warps per block
     const long long cap = (long long)ctx->num_sms * resident;
     double score_block = 0.0;
     p.rows_per_task = choose_rows_per_task(ctx, p.nseg, cap, wpb, &score_block);
     // many small chains: per-warp task lists (kernel_i8.cuh PER_WARP) balance at warp granularity with tall strips;
     // they cannot use the paired lookup, which is worth ~5 % on launches without fused sums
     ctx->perwarp = false;
-    if (!ctx->packed && (ctx->variant == 8 || (ctx->variant == 0 && ctx->n_chains > 1))) {
+    if (!ctx->packed && (ctx->variant == SHAKEN_VARIANT_PERWARP || ctx->n_chains > 1)) {
         double score_pw = 0.0;
         const int Rpw = choose_rows_per_task(ctx, p.nseg, cap * wpb, 1, &score_pw);
         const bool mostly_plain = obs_every == 0 || obs_every > 4;
-        if (ctx->variant == 8 || score_pw * (mostly_plain ? 0.95 : 1.0) > score_block + 0.02) {
+        if (ctx->variant == SHAKEN_VARIANT_PERWARP || score_pw * (mostly_plain ? 0.95 : 1.0) > score_block + 0.02) {
             ctx->perwarp = true;
             p.rows_per_task = Rpw;
             wpb = 1;                                       // p.ntasks counts warp strips
         }
     }
     p.nrb = (ctx->L + p.rows_per_task - 1) / p.rows_per_task;
-    // block tasks: WARPS_PER_BLOCK consecutive warp strips of one chain
+    // block tasks: wpb consecutive warp strips of one chain
     p.ntasks = (long long)ctx->n_chains * (((long long)p.nrb * p.nseg + wpb - 1) / wpb);
 
     if (uniform) {
@@ -589,6 +574,7 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
         ctx->launches++;
         ctx->step += (uint64_t)n_steps;
         ctx->n_rec += n_new;
+        ctx->have_tau = true;
         return SHAKEN_OK;
     }
 
@@ -661,6 +647,7 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
                 ctx->launches++;
                 ctx->step += (uint64_t)n_steps;
                 ctx->n_rec += n_new;
+                ctx->have_tau = true;
                 return SHAKEN_OK;
             }
             cudaGetLastError();
@@ -674,6 +661,7 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
     const int grid = (int)(blocks_needed < cap ? blocks_needed : cap);
     const size_t rec_stride = (size_t)ctx->n_chains * SHAKEN_N_OBS;
 
+    ctx->have_tau = true;           // half-step 0 redraws every tau from sigma alone
     long long *pending = nullptr;   // record that still lacks C_x, C_y
     for (int64_t s = 0; s < n_steps; ++s) {
         const uint64_t t = ctx->step;
@@ -759,7 +747,7 @@ static int run_alt_impl(shaken_ctx *ctx, const double *J, bool uniform, int64_t 
     const int nJ = uniform ? 1 : ctx->n_chains;
     for (int i = 0; i < nJ; ++i)
         if (!isfinite(J[i])) return fail(ctx, SHAKEN_EINVAL, "shaken_run_alternate: non-finite coupling for chain %d", i);
-    if (!ctx->have_spins || !ctx->d_sigma) return fail(ctx, SHAKEN_ESTATE, "shaken_run_alternate: no spins yet (call shaken_init or shaken_set_spins)");
+    if (!ctx->have_sigma || !ctx->d_sigma) return fail(ctx, SHAKEN_ESTATE, "shaken_run_alternate: no sigma yet (call shaken_init, shaken_set_spins or shaken_adopt_spins)");
     int rc = ensure_device(ctx);
     if (rc) return rc;
     if (n_steps == 0) return SHAKEN_OK;
@@ -941,7 +929,8 @@ static const size_t STAGE_SITES = (size_t)64 << 20;   // conversion chunk: 64 Mi
 extern "C" int shaken_get_spins(shaken_ctx *ctx, int which, int8_t *host)
 {
     if (!ctx || !host || (which != 0 && which != 1)) return fail(ctx, SHAKEN_EINVAL, "shaken_get_spins: bad argument");
-    if (!ctx->have_spins || !ctx->d_sigma) return fail(ctx, SHAKEN_ESTATE, "shaken_get_spins: no spins yet");
+    if (!(which ? ctx->have_tau : ctx->have_sigma) || !ctx->d_sigma)
+        return fail(ctx, SHAKEN_ESTATE, "shaken_get_spins: %s has no defined content yet", which ? "tau" : "sigma");
     const size_t n = (size_t)ctx->n_chains * ctx->L * ctx->L;
     const void *src = which ? ctx->d_tau : ctx->d_sigma;
     if (!ctx->packed) {
@@ -992,8 +981,30 @@ extern "C" int shaken_set_spins(shaken_ctx *ctx, int which, const int8_t *host)
     unsigned long long bad = 0;
     CU(cudaMemcpyAsync(&bad, ctx->d_bad, sizeof(bad), cudaMemcpyDeviceToHost, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
-    ctx->have_spins = true;
+    (which ? ctx->have_tau : ctx->have_sigma) = bad == 0;
     if (bad) return fail(ctx, SHAKEN_EINVAL, "shaken_set_spins: %llu values are neither +1 nor -1 (sublattice content is now unspecified)", bad);
+    return SHAKEN_OK;
+}
+
+extern "C" int shaken_adopt_spins(shaken_ctx *ctx)
+{
+    if (!ctx) return fail(nullptr, SHAKEN_EINVAL, "shaken_adopt_spins: ctx is NULL");
+    if (!ctx->d_sigma || !ctx->d_tau) return fail(ctx, SHAKEN_ESTATE, "shaken_adopt_spins: no buffers (call shaken_bind first)");
+    int rc = ensure_device(ctx);
+    if (rc) return rc;
+    unsigned long long bad = 0;
+    if (!ctx->packed) {   // every bit pattern is a valid packed word; int8 layers must hold 0x01 / 0xFF only
+        const long long nvec = (long long)(shaken_spin_bytes(ctx) / 16);
+        CU(cudaMemsetAsync(ctx->d_bad, 0, sizeof(unsigned long long), ctx->stream));
+        validate_bytes<<<grid_for(ctx, nvec), 256, 0, ctx->stream>>>((const uint8_t *)ctx->d_sigma, nvec, ctx->d_bad);
+        validate_bytes<<<grid_for(ctx, nvec), 256, 0, ctx->stream>>>((const uint8_t *)ctx->d_tau, nvec, ctx->d_bad);
+        ctx->launches += 2;
+        CU(cudaGetLastError());
+        CU(cudaMemcpyAsync(&bad, ctx->d_bad, sizeof(bad), cudaMemcpyDeviceToHost, ctx->stream));
+    }
+    CU(cudaStreamSynchronize(ctx->stream));
+    if (bad) return fail(ctx, SHAKEN_EINVAL, "shaken_adopt_spins: %llu bytes of the bound buffers are neither +1 nor -1", bad);
+    ctx->have_sigma = ctx->have_tau = true;
     return SHAKEN_OK;
 }
 
@@ -1003,7 +1014,7 @@ extern "C" int shaken_set_spins(shaken_ctx *ctx, int which, const int8_t *host)
 extern "C" int shaken_diag_correlations(shaken_ctx *ctx, const int32_t *ells, int32_t n_ell, int64_t *out)
 {
     if (!ctx || !ells || !out || n_ell < 1) return fail(ctx, SHAKEN_EINVAL, "shaken_diag_correlations: bad argument");
-    if (!ctx->have_spins || !ctx->d_sigma) return fail(ctx, SHAKEN_ESTATE, "shaken_diag_correlations: no spins yet");
+    if (!ctx->have_sigma || !ctx->d_sigma) return fail(ctx, SHAKEN_ESTATE, "shaken_diag_correlations: no sigma yet");
     for (int e = 0; e < n_ell; ++e)
         if (ells[e] < 0) return fail(ctx, SHAKEN_EINVAL, "shaken_diag_correlations: negative distance");
     int rc = ensure_device(ctx);
@@ -1019,11 +1030,11 @@ extern "C" int shaken_diag_correlations(shaken_ctx *ctx, const int32_t *ells, in
     long long bpc = ((long long)ctx->L * W + 255) / 256;
     const long long cap = (long long)ctx->num_sms * 8 / ctx->n_chains + 1;
     if (bpc > cap) bpc = cap;
-    const dim3 grid((unsigned)bpc, (unsigned)ctx->n_chains);
+    const dim3 grid((unsigned)bpc, (unsigned)(ctx->n_chains < 65535 ? ctx->n_chains : 65535));   // chains beyond gridDim.y: looped in the kernel
     for (int e = 0; e < n_ell && err == cudaSuccess; ++e) {
         const int l = ells[e] % ctx->L;
-        if (ctx->packed) diag_corr<true><<<grid, 256, 0, ctx->stream>>>((const uint32_t *)ctx->d_sigma, ctx->L, l, d, n_ell, e);
-        else diag_corr<false><<<grid, 256, 0, ctx->stream>>>((const uint32_t *)ctx->d_sigma, ctx->L, l, d, n_ell, e);
+        if (ctx->packed) diag_corr<true><<<grid, 256, 0, ctx->stream>>>((const uint32_t *)ctx->d_sigma, ctx->L, ctx->n_chains, l, d, n_ell, e);
+        else diag_corr<false><<<grid, 256, 0, ctx->stream>>>((const uint32_t *)ctx->d_sigma, ctx->L, ctx->n_chains, l, d, n_ell, e);
         ctx->launches++;
         err = cudaGetLastError();
     }
@@ -1031,6 +1042,126 @@ extern "C" int shaken_diag_correlations(shaken_ctx *ctx, const int32_t *ells, in
     if (err == cudaSuccess) err = cudaStreamSynchronize(ctx->stream);
     cudaFree(d);
     if (err != cudaSuccess) return fail(ctx, SHAKEN_ECUDA, "shaken_diag_correlations: %s", cudaGetErrorString(err));
+    return SHAKEN_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// (a9) derived statistics of the recorded magnetisation, exact integer power sums
+// ---------------------------------------------------------------------------------------------------
+namespace {
+// 256-bit unsigned integer, just enough for sums of M^4 (|M| <= 2^32) and products of two 128-bit sums
+struct U256 {
+    unsigned long long w[4] = {0, 0, 0, 0};   // little endian
+    void add(const U256 &o)
+    {
+        unsigned __int128 c = 0;
+        for (int i = 0; i < 4; ++i) { c += (unsigned __int128)w[i] + o.w[i]; w[i] = (unsigned long long)c; c >>= 64; }
+    }
+    bool sub(const U256 &o)                    // *this -= o; returns true if the result wrapped (o was larger)
+    {
+        __int128 b = 0;
+        for (int i = 0; i < 4; ++i) { b += (__int128)w[i] - (__int128)o.w[i]; w[i] = (unsigned long long)b; b >>= 64; }
+        return b != 0;
+    }
+    static U256 mul(unsigned __int128 a, unsigned __int128 b)
+    {
+        const unsigned long long x[2] = {(unsigned long long)a, (unsigned long long)(a >> 64)}, y[2] = {(unsigned long long)b, (unsigned long long)(b >> 64)};
+        U256 r;
+        for (int i = 0; i < 2; ++i) {
+            unsigned __int128 c = 0;
+            for (int j = 0; j < 2; ++j) { c += (unsigned __int128)x[i] * y[j] + r.w[i + j]; r.w[i + j] = (unsigned long long)c; c >>= 64; }
+            r.w[i + 2] += (unsigned long long)c;
+        }
+        return r;
+    }
+    U256 times(unsigned long long k) const
+    {
+        U256 r;
+        unsigned __int128 c = 0;
+        for (int i = 0; i < 4; ++i) { c += (unsigned __int128)w[i] * k; r.w[i] = (unsigned long long)c; c >>= 64; }
+        return r;
+    }
+    bool less(const U256 &o) const
+    {
+        for (int i = 3; i >= 0; --i) if (w[i] != o.w[i]) return w[i] < o.w[i];
+        return false;
+    }
+    long double ld() const { return (((long double)w[3] * 18446744073709551616.0L + (long double)w[2]) * 18446744073709551616.0L + (long double)w[1]) * 18446744073709551616.0L + (long double)w[0]; }
+};
+}   // namespace
+
+extern "C" int shaken_moments(const int64_t *M, int64_t n, int64_t stride, int64_t n_sites, double out[SHAKEN_N_MOMENTS])
+{
+    if (!M || !out || n < 1 || n >= (1ll << 31) || stride < 1 || n_sites < 1 || n_sites > (1ll << 32))
+        return fail(nullptr, SHAKEN_EINVAL, "shaken_moments: bad argument");
+    unsigned __int128 S2 = 0, Sa = 0;
+    __int128 S1 = 0;
+    U256 S4;
+    for (int64_t i = 0; i < n; ++i) {
+        const int64_t v = M[i * stride];
+        const unsigned long long a = v < 0 ? 0ull - (unsigned long long)v : (unsigned long long)v;
+        if (a > (unsigned long long)n_sites) return fail(nullptr, SHAKEN_EINVAL, "shaken_moments: |M| = %llu exceeds n_sites", a);
+        const unsigned __int128 sq = (unsigned __int128)a * a;
+        S1 += v;
+        Sa += a;
+        S2 += sq;
+        S4.add(U256::mul(sq, sq));
+    }
+    const long double N = (long double)n_sites, dn = (long double)n;
+    out[0] = (double)((long double)S1 / (dn * N));                     // <m>
+    out[1] = (double)((long double)Sa / (dn * N));                     // <|m|>
+    out[2] = (double)((long double)S2 / (dn * N * N));                 // <m^2>
+    out[3] = (double)(S4.ld() / (dn * N * N * N * N));                 // <m^4>
+    // Var m = (n S2 - S1^2) / (n^2 N^2): the difference is taken exactly (both terms < 2^127 for n < 2^31)
+    const unsigned __int128 a1 = S1 < 0 ? (unsigned __int128)(-S1) : (unsigned __int128)S1;
+    out[4] = (double)((long double)((unsigned __int128)n * S2 - a1 * a1) / (dn * dn * N * N));
+    // Binder U = 1 - n S4 / (3 S2^2) = (3 S2^2 - n S4) / (3 S2^2), numerator exact in 256 bits
+    if (S2 == 0) out[5] = NAN;
+    else {
+        U256 den = U256::mul(S2, S2).times(3ull), num = den;
+        const U256 nS4 = S4.times((unsigned long long)n);
+        if (den.less(nS4)) { U256 t = nS4; t.sub(den); out[5] = -(double)(t.ld() / den.ld()); }
+        else { num.sub(nS4); out[5] = (double)(num.ld() / den.ld()); }
+    }
+    return SHAKEN_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// measurement hook: the Philox-only ceiling (kernels.cuh: philox_rate)
+// ---------------------------------------------------------------------------------------------------
+extern "C" int shaken_selftest_philox_rate(int32_t blocks_per_sm, int32_t iters, int32_t reps, double *sites_per_ns)
+{
+    shaken_ctx *ctx = nullptr;
+    if (!sites_per_ns || blocks_per_sm < 1 || blocks_per_sm > 8 || iters < 1 || iters > (1 << 20) || reps < 1)
+        return fail(nullptr, SHAKEN_EINVAL, "shaken_selftest_philox_rate: bad argument");
+    int dev = 0, sms = 0;
+    CU(cudaGetDevice(&dev));
+    CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    if ((double)sms * blocks_per_sm * 256.0 * 4.0 * iters >= 4294967296.0)
+        return fail(nullptr, SHAKEN_EINVAL, "shaken_selftest_philox_rate: counter range exceeds 2^32");
+    StepKeys K;
+    make_step_keys(3, 12345, K);
+    uint32_t *d = nullptr;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    cudaError_t e = cudaMalloc(&d, 64);
+    if (e == cudaSuccess) e = cudaEventCreate(&e0);
+    if (e == cudaSuccess) e = cudaEventCreate(&e1);
+    double best = 0.0;
+    for (int r = 0; r <= reps && e == cudaSuccess; ++r) {      // r = 0 warms up
+        cudaEventRecord(e0, 0);
+        philox_rate<<<sms * blocks_per_sm, 256>>>(d, K, iters);
+        cudaEventRecord(e1, 0);
+        e = cudaEventSynchronize(e1);
+        float ms = 0.f;
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+        const double rate = (double)sms * blocks_per_sm * 256.0 * 16.0 * iters / ((double)ms * 1e6);
+        if (r > 0 && e == cudaSuccess && rate > best) best = rate;
+    }
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    cudaFree(d);
+    if (e != cudaSuccess) return fail(ctx, SHAKEN_ECUDA, "shaken_selftest_philox_rate: %s", cudaGetErrorString(e));
+    *sites_per_ns = best;
     return SHAKEN_OK;
 }
 

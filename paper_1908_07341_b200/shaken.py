@@ -55,6 +55,9 @@ SIGNATURES = {
     "shaken_philox_words": (C.c_int, [_p, _p, _p, C.c_int64]),
     "shaken_launch_count": (C.c_int64, [_p]),
     "shaken_set_variant": (C.c_int, [_p, C.c_int]),
+    "shaken_adopt_spins": (C.c_int, [_p]),
+    "shaken_moments": (C.c_int, [_p, C.c_int64, C.c_int64, C.c_int64, C.POINTER(C.c_double)]),
+    "shaken_selftest_philox_rate": (C.c_int, [C.c_int32, C.c_int32, C.c_int32, C.POINTER(C.c_double)]),
     "shaken_last_error": (C.c_char_p, [_p]),
     "shaken_version": (C.c_char_p, []),
 }
@@ -106,6 +109,15 @@ def thresholds(J: float, q: float) -> np.ndarray:
     if rc:
         raise ShakenError(rc, lib().shaken_last_error(None).decode())
     return np.array(list(t), dtype=np.uint32)
+
+
+def philox_only_rate(blocks_per_sm: int = 8, iters: int = 2048, reps: int = 3) -> float:
+    """Measured rate (site-updates per ns) of the library's Philox-only kernel (shaken_selftest_philox_rate)."""
+    v = C.c_double()
+    rc = lib().shaken_selftest_philox_rate(int(blocks_per_sm), int(iters), int(reps), C.byref(v))
+    if rc:
+        raise ShakenError(rc, lib().shaken_last_error(None).decode())
+    return float(v.value)
 
 
 def philox_words(ctr: np.ndarray, key: np.ndarray) -> np.ndarray:
@@ -281,6 +293,10 @@ class Shaken:
         self._ck(self._lib.shaken_diag_correlations(self._h, e.ctypes.data, e.size, out.ctypes.data))
         return out
 
+    def adopt_spins(self):
+        """Declare that the bound device buffers already hold valid spins (shaken_adopt_spins)."""
+        self._ck(self._lib.shaken_adopt_spins(self._h))
+
     def synchronize(self):
         self._ck(self._lib.shaken_synchronize(self._h))
 
@@ -294,37 +310,17 @@ class Shaken:
 
 # ---------------------------------------------------------------------- (a9) derived statistics, host side
 def derived_stats(M, n_sites: int) -> dict:
-    """Mean and variance of the magnetisation m = M / n_sites over the recorded window,
-    plus <|m|>, <m^2>, <m^4> and the Binder cumulant U = 1 - <m^4> / (3 <m^2>^2).
-
-    The power sums are exact Python integers (M^4 overflows int64 from L = 512 on, so they are never formed
-    on the device); each quantity is ONE correctly rounded integer division at the end."""
-    vals = [int(v) for v in np.asarray(M).ravel()]
-    n = len(vals)
-    if n == 0:
+    """Mean and variance of the magnetisation m = M / n_sites over the recorded window, plus <|m|>,
+    <m^2>, <m^4> and the Binder cumulant U = 1 - <m^4> / (3 <m^2>^2): shaken_moments of the C ABI (exact integer power
+    sums in the library -- M^4 overflows int64 from L = 512 on -- and one division each); this only marshals."""
+    vals = np.ascontiguousarray(np.asarray(M).ravel(), dtype=np.int64)
+    if vals.size == 0:
         raise ValueError("no records")
-    N = int(n_sites)
-    p1 = pa = p2 = p4 = 0
-    for v in vals:
-        sq = v * v
-        p1 += v
-        pa += -v if v < 0 else v
-        p2 += sq
-        p4 += sq * sq
-    res = {
-        "n": n,
-        "m": p1 / (n * N),
-        "abs_m": pa / (n * N),
-        "m2": p2 / (n * N * N),
-        "m4": p4 / (n * N**4),
-        "var_m": (n * p2 - p1 * p1) / (n * n * N * N),
-    }
-    if p2:
-        num, den = 3 * p2 * p2 - n * p4, 3 * p2 * p2
-        res["binder"] = num / den
-    else:
-        res["binder"] = float("nan")
-    return res
+    out = (C.c_double * 6)()
+    rc = lib().shaken_moments(vals.ctypes.data, vals.size, 1, int(n_sites), out)
+    if rc:
+        raise ShakenError(rc, lib().shaken_last_error(None).decode())
+    return {"n": int(vals.size), "m": out[0], "abs_m": out[1], "m2": out[2], "m4": out[3], "var_m": out[4], "binder": out[5]}
 
 
 def energy(J: float, q: float, E_J: int, E_q: int) -> float:

@@ -50,7 +50,9 @@ def test_create_validates_arguments_without_a_device():
     assert lib.shaken_run(h, 0.5, float("nan"), 1, 0) == shaken.EINVAL
     assert lib.shaken_run(h, 0.5, 0.5, -1, 0) == shaken.EINVAL
     assert lib.shaken_run(h, 0.5, 0.5, 1, 0) == shaken.ESTATE
-    assert b"no spins" in lib.shaken_last_error(h)
+    assert b"no sigma" in lib.shaken_last_error(h)
+    assert lib.shaken_adopt_spins(h) == shaken.ESTATE          # no buffers bound
+    assert lib.shaken_set_variant(h, 5) == shaken.EINVAL and lib.shaken_set_variant(h, 3) == 0 and lib.shaken_set_variant(h, 0) == 0
     assert lib.shaken_run_alternate(h, float("inf"), 1, 0) == shaken.EINVAL
     assert lib.shaken_run_alternate(h, 0.3, 1, -2) == shaken.EINVAL
     assert lib.shaken_run_alternate(h, 0.3, 1, 0) == shaken.ESTATE
@@ -82,6 +84,37 @@ def test_library_threshold_table_against_exact_decimal_arithmetic():
         assert np.array_equal(shaken.thresholds(a, b).astype(np.uint64), pins.exact_table(a, b))
     with pytest.raises(shaken.ShakenError):
         shaken.thresholds(float("inf"), 0.1)
+
+
+def test_moments_through_the_c_abi_strided_and_beyond_128_bits():
+    """shaken_moments as a C caller uses it: a strided view into [record][chain][6] records, and a window whose sum of
+    M^4 exceeds 128 bits (500 records of |M| = 2^32 - 2k on a 65536^2 lattice); expected values from Python integers
+    and Fractions written out here (not from either implementation's code)."""
+    from fractions import Fraction
+
+    lib = shaken.lib()
+    rec = np.zeros((5, 3, 6), dtype=np.int64)
+    rec[:, 1, 0] = [2, -2, 4, 0, 4]
+    out = (C.c_double * 6)()
+    assert lib.shaken_moments(rec[0, 1].ctypes.data, 4, 18, 4, out) == 0          # first four records of chain 1
+    assert list(out) == [0.25, 0.5, 0.375, 0.28125, 0.3125, out[5]] and abs(out[5] - 1 / 3) < 1e-15
+    N = 2**32
+    M = np.array([(N - 2 * k) * (1 if k % 3 else -1) for k in range(500)], dtype=np.int64)
+    assert lib.shaken_moments(M.ctypes.data, 500, 1, N, out) == 0
+    Mi = [int(v) for v in M]
+    S1, Sa, S2, S4 = sum(Mi), sum(abs(v) for v in Mi), sum(v * v for v in Mi), sum(v**4 for v in Mi)
+    assert S4 > 2**128
+    want = [Fraction(S1, 500 * N), Fraction(Sa, 500 * N), Fraction(S2, 500 * N * N), Fraction(S4, 500 * N**4),
+            Fraction(500 * S2 - S1 * S1, 500 * 500 * N * N), 1 - Fraction(500 * S4, 3 * S2 * S2)]
+    for got, w in zip(out, want):
+        assert abs(got - float(w)) <= 1e-15 * abs(float(w)), (got, float(w))
+    # U < 0 (one large outlier among zeros): the sign branch of the 256-bit subtraction
+    assert lib.shaken_moments(np.array([8, 0, 0, 0, 0, 0, 0, 0], dtype=np.int64).ctypes.data, 8, 1, 64, out) == 0
+    assert abs(out[5] - (1 - 8 / 3)) < 1e-15
+    assert np.isnan(shaken.derived_stats([0, 0], 16)["binder"])
+    for bad in [(0, 1, 4), (4, 0, 4), (4, 1, 0), (4, 1, 3)]:                       # n, stride, n_sites (|M| = 4 > 3)
+        assert lib.shaken_moments(rec[0, 1].ctypes.data, bad[0], bad[1] * 18, bad[2], out) == shaken.EINVAL, bad
+    assert lib.shaken_moments(None, 4, 1, 4, out) == shaken.EINVAL
 
 
 def test_derived_stats_exact_small_case_and_large_values():

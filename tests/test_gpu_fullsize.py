@@ -6,15 +6,29 @@ configuration bench.py times.  The oracle is too slow for full-length runs here 
   ``step = k`` (legal because the randomness is indexed by the step), and the result must equal the GPU state
   after k+1 steps, spins and records;
 * at L = 32768 (cfg 5, 2.1e9 site updates per step) the oracle computes sampled bands of rows of each half-step
-  (``oracle.half_step_rows``) from the downloaded source layer, and the six sums by brute force.
+  (``oracle.half_step_rows``) from the downloaded source layer, and the six sums by brute force;
+* whole-lattice steps at L = 32768 (packed) and L = 65536 (int8), and the FULL-LENGTH cfg 2 run (10^4 steps), use the same
+  row function over ALL rows, the bands spread over the host cores (tests/rowsplit.py).
 """
+from concurrent.futures import ThreadPoolExecutor
+
 import numpy as np
 import pytest
 
 from oracle import shaken_oracle as so
 from paper_1908_07341_b200 import shaken, workloads
+from tests import rowsplit
 
 pytestmark = pytest.mark.gpu
+
+
+def host_memory_gb() -> float:
+    try:
+        import psutil
+
+        return psutil.virtual_memory().available / 2**30
+    except Exception:
+        return 0.0
 
 
 def oracle_step_from(s: shaken.Shaken, w, J, q, n_steps=1, obs_every=1):
@@ -136,3 +150,95 @@ def test_maximum_lattice_side_65536_sampled_rows(packed):
         rec = s.observables()[-1, 0]
         assert rec[0] == int(sigma1.sum(dtype=np.int64)) and rec[1] == int(tau1.sum(dtype=np.int64))
         assert rec[3] == int((sigma1.astype(np.int16) * tau1).sum(dtype=np.int64))          # E_q
+
+
+def test_cfg2_full_length_10000_steps_against_the_oracle():
+    """cfg 2 at full length (SURVEY 8(c) last row: "full-length full-size oracle runs are still the goal for cfg 1-2"):
+    10^4 steps of 1024^2 at the honeycomb point, records every 10 steps, in ONE shaken_run call -- one cooperative launch
+    of the band kernel with 20 000 stamped hand-overs per band.  The oracle advances half-step by half-step with its row
+    function spread over the host cores and takes its six sums every 10 steps; all 1000 records and both final layers
+    must agree bit for bit."""
+    w = workloads.config(2)
+    L, J, q = w.L, w.J[0], w.q[0]
+    sigma = np.ones((L, L), dtype=np.int8)
+    want = np.zeros((w.n_steps // w.obs_every, 6), dtype=np.int64)
+    with ThreadPoolExecutor(rowsplit.n_threads()) as pool:
+        for t in range(w.n_steps):
+            tau = rowsplit.half_step(sigma, w.seed, 0, J, q, t, 0, pool)
+            sigma = rowsplit.half_step(tau, w.seed, 0, J, q, t, 1, pool)
+            if (t + 1) % w.obs_every == 0:
+                want[(t + 1) // w.obs_every - 1] = so.measure(sigma, tau)
+    with shaken.Shaken(L, 1, w.seed, max_records=w.n_steps // w.obs_every) as s:
+        s.init(w.init)
+        s.run(J, q, w.n_steps, w.obs_every)
+        assert s.launch_count == 1                     # the one-launch band path is what ran
+        rec = s.observables()
+        assert rec.shape == (1000, 1, 6)
+        bad = np.nonzero((rec[:, 0] != want).any(axis=1))[0]
+        assert bad.size == 0, f"first differing record {bad[:3]}"
+        assert np.array_equal(s.get_spins(1)[0], tau) and np.array_equal(s.get_spins(0)[0], sigma)
+    # the paper's honeycomb critical point (PAPER.md:151): started from all +1, |m| decays but has not vanished at L = 1024
+    assert 0 < abs(int(want[-1, 0])) < L * L
+
+
+def test_cfg5_packed_32768_whole_lattice_one_step():
+    """Every site of one full step at cfg 5's real size (2.1e9 site updates) against the oracle's row function over all
+    rows; the record against the oracle's sums of the (already verified) layers."""
+    w = workloads.config(5)
+    J, q, L = w.J[0], w.q[0], w.L
+    with shaken.Shaken(L, 1, w.seed, packed=True, max_records=8) as s:
+        s.init(w.init)
+        s.run(J, q, 2, 1)
+        sigma_k = s.get_spins(0)[0].copy()
+        t = s.step
+        s.run(J, q, 1, 1)
+        tau_new, sigma_new = s.get_spins(1)[0], s.get_spins(0)[0]
+        with ThreadPoolExecutor(rowsplit.n_threads()) as pool:
+            assert rowsplit.mismatching_rows(sigma_k, tau_new, w.seed, 0, J, q, t, 0, pool) == []
+            assert rowsplit.mismatching_rows(tau_new, sigma_new, w.seed, 0, J, q, t, 1, pool) == []
+        assert np.array_equal(s.observables()[-1, 0], so.measure(sigma_new, tau_new))
+
+
+@pytest.mark.skipif(host_memory_gb() < 48, reason="needs about 20 GB of host memory for three 65536^2 int8 layers")
+def test_maximum_lattice_side_65536_whole_lattice_one_step_int8():
+    """L = 65536 int8 (4.3e9 sites per layer): every row of both half-steps of a recorded step from an iid start."""
+    L, seed, J, q = 65536, 9, 0.44, 0.66
+    with shaken.Shaken(L, 1, seed, max_records=2) as s:
+        s.init(0)
+        sigma0 = s.get_spins(0)[0].copy()
+        s.run(J, q, 1, 1)
+        tau1 = s.get_spins(1)[0]
+        with ThreadPoolExecutor(rowsplit.n_threads()) as pool:
+            assert rowsplit.mismatching_rows(sigma0, tau1, seed, 0, J, q, 0, 0, pool) == []
+            del sigma0
+            sigma1 = s.get_spins(0)[0]
+            assert rowsplit.mismatching_rows(tau1, sigma1, seed, 0, J, q, 0, 1, pool) == []
+        rec = s.observables()[-1, 0]
+        assert rec[0] == int(sigma1.sum(dtype=np.int64)) and rec[1] == int(tau1.sum(dtype=np.int64))
+
+
+@pytest.mark.skipif(host_memory_gb() < 48, reason="needs about 22 GB of host memory")
+def test_chain_planes_beyond_4GiB_three_chains_of_49152():
+    """Three chains of 49152^2 int8 (2.4 GB per plane): chain 1 straddles the 4 GiB offset, chain 2 starts above it; one
+    recorded step with per-chain couplings, sampled row bands of chains 1 and 2 (incl. the row that contains byte offset
+    2^32, strip boundaries and the torus wrap) against the oracle, and M_sigma, M_tau of every chain by brute force."""
+    L, n, seed = 49152, 3, 13
+    J = np.array([0.44, 0.7, 0.3])
+    q = np.array([0.66, 0.7, 1.5])
+    with shaken.Shaken(L, n, seed, max_records=2) as s:
+        s.init(0)
+        sigma0 = s.get_spins(0).copy()
+        s.run_grid(J, q, 1, 1)
+        tau1 = s.get_spins(1)
+        row_4g = (2**32 - L * L) // L                 # row of chain 1 that holds byte offset 2^32 of the layer
+        for ch in (1, 2):
+            for r0, k in [(0, 2), (L - 2, 2), (row_4g - 1, 3), (221, 3), (30011, 1)]:
+                assert np.array_equal(so.half_step_rows(sigma0[ch], seed, ch, J[ch], q[ch], 0, 0, r0, k), tau1[ch, r0:r0 + k]), ("half0", ch, r0)
+        del sigma0
+        sigma1 = s.get_spins(0)
+        for ch in (1, 2):
+            for r0, k in [(0, 2), (L - 2, 2), (row_4g - 1, 3), (40001, 2)]:
+                assert np.array_equal(so.half_step_rows(tau1[ch], seed, ch, J[ch], q[ch], 0, 1, r0, k), sigma1[ch, r0:r0 + k]), ("half1", ch, r0)
+        rec = s.observables()[-1]
+        for ch in range(n):
+            assert rec[ch, 0] == int(sigma1[ch].sum(dtype=np.int64)) and rec[ch, 1] == int(tau1[ch].sum(dtype=np.int64))

@@ -298,16 +298,16 @@ def test_cfg1_full_length():
 
 @pytest.mark.parametrize("L,n_chains", [(16, 1), (48, 3), (64, 2), (128, 2)])
 def test_small_lattice_path_and_generic_kernels_both_match_oracle(L, n_chains):
-    """L <= 128 runs in the one-CTA-per-chain persistent kernel (kernel_small.cuh) under variant 0; every other
-    variant forces one of the generic strip kernels (include/shaken.h).  All must equal the oracle, records included,
-    also when a run is split and obs_every does not divide the split."""
+    """L <= 128 runs in the one-CTA-per-chain persistent kernel (kernel_small.cuh) under variant 0; variants 3 and 8
+    force the strip kernels (block tasks / per-warp task lists, include/shaken.h).  All must equal the oracle, records
+    included, also when a run is split and obs_every does not divide the split."""
     seed = 77 + L
     J = np.linspace(0.2, 0.9, n_chains)
     q = np.linspace(1.5, 0.1, n_chains)
     o = so.Oracle(L, n_chains, seed)
     o.init(0)
     o.run_grid(J, q, 11, 3)
-    for variant in (0, 1, 2, 3, 4, 5, 6, 7, 8, 9):
+    for variant in (0, 3, 8):
         with shaken.Shaken(L, n_chains, seed, max_records=8) as s:
             s.set_variant(variant)
             s.init(0)
@@ -316,7 +316,7 @@ def test_small_lattice_path_and_generic_kernels_both_match_oracle(L, n_chains):
             assert_same_state(s, o, f"L={L} variant={variant}")
 
 
-@pytest.mark.parametrize("variant", [0, 1, 2, 4, 5, 6, 7, 8, 9])
+@pytest.mark.parametrize("variant", [0, 3, 8])
 def test_every_int8_code_path_matches_oracle_on_a_ragged_lattice(variant):
     """L = 272: 17 vectors per row (ragged warp strip), several row blocks per chain, three chains with different
     couplings incl. a saturated table; records on some steps only, so launches with and without fused sums, the
@@ -333,6 +333,45 @@ def test_every_int8_code_path_matches_oracle_on_a_ragged_lattice(variant):
         s.run_grid(J, q, 5, 2)
         s.run_grid(J, q, 4, 2)
         assert_same_state(s, o, f"variant={variant}")
+
+
+@pytest.mark.parametrize("L,packed,variant", [(272, False, 0), (528, False, 3), (1056, True, 0), (64, False, 0)])
+def test_step_index_crossing_2_to_31_in_every_kernel_family(L, packed, variant):
+    """Global step index t0 = 2^31 - 2: g = 2t + half crosses 2^32 inside the run, so counter word 3 (g hi) changes
+    between two steps.  L = 272 takes the band kernel (device_half_step_keys), 528 with the strip switch the strip
+    kernels (make_step_keys on the host), 1056 the packed kernel, 64 the small-lattice kernel.  Oracle: same t0."""
+    seed, t0 = 19, 2**31 - 2
+    o = so.Oracle(L, 1, seed)
+    o.init(0)
+    o.step = t0
+    o.run(0.5, 0.8, 4, 1)
+    with shaken.Shaken(L, 1, seed, packed=packed, max_records=8) as s:
+        s.set_variant(variant)
+        s.init(0)
+        s.step = t0
+        s.run(0.5, 0.8, 3, 1)
+        s.run(0.5, 0.8, 1, 1)
+        assert s.step == t0 + 4
+        assert_same_state(s, o, f"L={L} packed={packed}")
+
+
+@pytest.mark.parametrize("L,n_chains", [(2048, 1), (1024, 4), (1488, 2)])
+def test_band_kernel_tall_bands_per_chain_tables_and_split_runs(L, n_chains):
+    """The band kernel's tall-band branch (more than three trips of vectors per band: one chain at L >= ~1792, or four
+    chains of 1024^2), with per-chain (J, q) tables, records on some steps only, and the run split over two shaken_run
+    calls in the middle of a recording interval (stamp continuity, the pending C_x, C_y of the last record)."""
+    seed = 3 + L
+    J = np.linspace(0.3, 0.9, n_chains)
+    q = np.linspace(1.2, 0.2, n_chains)
+    o = so.Oracle(L, n_chains, seed)
+    o.init(0)
+    o.run_grid(J, q, 7, 3)
+    with shaken.Shaken(L, n_chains, seed, max_records=4) as s:
+        s.init(0)
+        s.run_grid(J, q, 4, 3)
+        s.run_grid(J, q, 3, 3)
+        assert s.launch_count == 3, "init + one cooperative launch per run call expected"
+        assert_same_state(s, o, f"L={L} chains={n_chains}")
 
 
 # ----------------------------------------------------------------------------- coupled chains, coalescence (SURVEY 8(f) rank 1)
