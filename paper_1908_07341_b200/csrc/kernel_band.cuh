@@ -1,13 +1,20 @@
 // kernel_band.cuh -- mid-size lattices (128 < L <= 2048, few chains): a half-step is a microsecond of work, so one
 // launch per half-step is mostly launch latency (cfg 2: 4.9 us per launch for 0.8 us of arithmetic).  Here the whole
 // run is ONE cooperative launch.  Every CTA owns a band of rows of one chain and keeps both sublattices of the band in
-// shared memory; per half-step it needs exactly one row from a neighbouring band (eq. (14): the field
-// uses the down row in half 0, the up row in half 1), which the neighbour publishes through a small global buffer in
-// "data + stamp" form: every 64-bit store carries the spin word and the half-step stamp, so a reader that sees the
-// stamp has the data (no fence, no separate flag; see st_pair).  A CTA computes the row its neighbour waits for first, one word per
-// thread, and every word is published by the thread that computed it; one warp does no arithmetic and polls for the
-// row the CTA itself needs next.  There is no grid-wide barrier: only neighbouring
-// bands wait for each other, which is why all CTAs must be co-resident -- the cooperative launch guarantees it.
+// shared memory.  The fields of eq. (14) reach one row across a band edge in each half-step: the
+// down row in half 0, the up row in half 1.  Because a site's random word is a function of (seed, chain, step, half,
+// site) alone, a band can redraw the tau row ABOVE itself redundantly (from the sigma row above, which it receives, and
+// its own top sigma row), so bands exchange only sigma rows, ONCE per full step: after half-step 1 a band publishes its
+// bottom and top sigma rows, and in the next half-step 0 it needs the top row of the band below and the bottom row of
+// the band above.  One hand-over latency per step instead of two, at the price of one extra row of half-step 0.
+//
+// The hand-over goes through a small global buffer in "data + stamp" form: every 64-bit store carries a spin word and
+// the step's stamp, so a reader that sees the stamp has the data (no fence, no separate flag; see ld_pair / st_pairs2).
+// The thread that computes a vector of a boundary row polls for exactly the words it needs and the thread that computed
+// a published vector stores it itself: no staging warp, no barrier on the exchange path.  Work is ordered so that the
+// rows that wait for a neighbour come LAST in half-step 0 and the rows a neighbour waits for come FIRST in half-step 1:
+// the hand-over latency hides behind the interior rows.  There is no grid-wide barrier: only neighbouring bands wait
+// for each other, which is why all CTAs must be co-resident -- the cooperative launch guarantees it.
 // Site -> random word mapping, thresholds and rule are those of kernel_i8.cuh; only the schedule differs.
 #pragma once
 #include "kernels_common.cuh"
@@ -15,7 +22,7 @@
 namespace shaken {
 
 constexpr int BAND_THREADS = 512;
-constexpr int BAND_L_MAX = 2048;   // W = L/4 <= 512: a published row is at most 8 words per lane of the collecting warp
+constexpr int BAND_L_MAX = 2048;   // W = L/4 <= 512 words per row
 
 struct BandParams {
     uint8_t *sigma;          // [n_chains][L][L] int8
@@ -32,25 +39,37 @@ struct BandParams {
     StepKeys keys;           // only k0[], k1[] are used
     int bpc;                 // bands per chain
     int rows_per_band;
-    uint2 *xs;               // [2][n_bands][L/4] {word, stamp}: last sigma row of each band after half-step 1
-    uint2 *xt;               // [2][n_bands][L/4] {word, stamp}: first tau row of each band after half-step 0
-    uint32_t magicV;         // floor(2^32 / (L/16)) + 1: the same for vector indices c / (L/16)
-    uint32_t magicW;         // floor(2^32 / (L/4)) + 1: c / W == __umulhi(c, magicW) for the small c used here
-    uint32_t stamp0;         // stamps of this launch are stamp0 + 1 .. stamp0 + 2 n_steps (never seen before in xs, xt)
+    uint2 *xtop;             // [2][n_bands][L/4] {word, stamp}: TOP sigma row of each band after a full step (by parity of the step)
+    uint2 *xbot;             // [2][n_bands][L/4] {word, stamp}: BOTTOM sigma row of each band after a full step
+    uint32_t magicV;         // floor(2^32 / (L/16)) + 1: c / (L/16) == __umulhi(c, magicV) for the small c used here
+    uint32_t magicW;         // floor(2^32 / (L/4)) + 1: the same for word indices c / W
+    uint32_t stamp0;         // stamps of this launch are stamp0 + 1 .. stamp0 + n_steps (never seen before in xtop, xbot)
 };
 
-// A {word, stamp} pair crosses between CTAs as ONE naturally aligned 64-bit scalar access, relaxed at gpu scope on both
-// sides: the PTX memory model makes such an access single-copy atomic (a vector access would count as two scalar ones),
-// so a reader that sees the stamp of a half-step has the spin word written with it.  No fence, no flag.
+// dynamic shared memory: sigma rows r0-1 .. r1 (halo below, band, halo above) and tau rows r0 .. r1 (band, redundant row)
+__host__ __device__ inline size_t band_smem_bytes(int L, int rows_per_band) { return (size_t)(2 * rows_per_band + 3) * (size_t)(L / 4) * sizeof(uint32_t); }
+
+// A {word, stamp} pair crosses between CTAs as ONE naturally aligned 64-bit scalar, relaxed at gpu scope on both sides:
+// the PTX memory model makes such an access single-copy atomic (the elements of a vector access count as separate scalar
+// accesses, which is all that is needed: every pair validates itself), so a reader that sees the stamp of a step has
+// the spin word written with it.  No fence, no flag.
+__device__ __forceinline__ void ld_pairs2(const uint2 *p, uint2 &a, uint2 &b)
+{
+    unsigned long long x, y;
+    asm volatile("ld.relaxed.gpu.global.v2.u64 {%0, %1}, [%2];" : "=l"(x), "=l"(y) : "l"(p) : "memory");
+    a = make_uint2((uint32_t)x, (uint32_t)(x >> 32));
+    b = make_uint2((uint32_t)y, (uint32_t)(y >> 32));
+}
 __device__ __forceinline__ uint2 ld_pair(const uint2 *p)
 {
     unsigned long long v;
     asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
     return make_uint2((uint32_t)v, (uint32_t)(v >> 32));
 }
-__device__ __forceinline__ void st_pair(uint2 *p, uint32_t word, uint32_t stamp)
+__device__ __forceinline__ void st_pairs2(uint2 *p, uint32_t w0, uint32_t w1, uint32_t stamp)
 {
-    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" :: "l"(p), "l"(((unsigned long long)stamp << 32) | word) : "memory");
+    const unsigned long long s = (unsigned long long)stamp << 32;
+    asm volatile("st.relaxed.gpu.global.v2.u64 [%0], {%1, %2};" :: "l"(p), "l"(s | w0), "l"(s | w1) : "memory");
 }
 
 __global__ void __launch_bounds__(BAND_THREADS, 1) band_run_i8(const __grid_constant__ BandParams p)
@@ -62,26 +81,22 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) band_run_i8(const __grid_cons
     const int L = p.L, W = L >> 2;
     const int band = blockIdx.x, chain = band / p.bpc, k = band - chain * p.bpc;
     const int r0 = k * p.rows_per_band;
-    const int nr = min(L, r0 + p.rows_per_band) - r0;
-    const int down = chain * p.bpc + (k == 0 ? p.bpc - 1 : k - 1);
-    const int up = chain * p.bpc + (k == p.bpc - 1 ? 0 : k + 1);
+    const int nr = min(L, r0 + p.rows_per_band) - r0;                 // rows of this band (>= 1)
+    const int below = chain * p.bpc + (k == 0 ? p.bpc - 1 : k - 1);   // band that owns row r0 - 1
+    const int above = chain * p.bpc + (k == p.bpc - 1 ? 0 : k + 1);   // band that owns row r0 + nr
     const int nb = gridDim.x;
-    const int ncalls = nr * W;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t lane8 = (uint32_t)lane * 8u;
-    const bool duty_warp = warp == BAND_THREADS / 32 - 1;
-    constexpr int WORKERS = BAND_THREADS - 32;   // polls for the neighbour's row while the other warps compute
 
-    uint32_t *sg = smem;                          // sigma band [nr][W]
-    uint32_t *ta = smem + p.rows_per_band * W;    // tau band
-    uint32_t *hs = ta + p.rows_per_band * W;      // sigma row below the band
-    uint32_t *ht = hs + W;                        // tau row above the band
+    uint32_t *sg = smem;                          // sigma rows: index 0 = row r0-1 (halo), 1 .. nr = the band, nr+1 = row r0+nr (halo)
+    uint32_t *ta = smem + (p.rows_per_band + 2) * W;   // tau rows: index 0 .. nr-1 = the band, nr = row r0+nr (redrawn redundantly)
 
     const size_t plane = (size_t)L * L;
     uint32_t *gs = reinterpret_cast<uint32_t *>(p.sigma + (size_t)chain * plane);
     uint32_t *gt = reinterpret_cast<uint32_t *>(p.tau + (size_t)chain * plane);
-    for (int i = tid; i < ncalls; i += BAND_THREADS) { sg[i] = gs[(size_t)r0 * W + i]; ta[i] = gt[(size_t)r0 * W + i]; }
-    for (int i = tid; i < W; i += BAND_THREADS) hs[i] = gs[(size_t)(r0 == 0 ? L - 1 : r0 - 1) * W + i];
+    const int row_below = r0 == 0 ? L - 1 : r0 - 1, row_above = r0 + nr == L ? 0 : r0 + nr;
+    for (int i = tid; i < nr * W; i += BAND_THREADS) { sg[W + i] = gs[(size_t)r0 * W + i]; ta[i] = gt[(size_t)r0 * W + i]; }
+    for (int i = tid; i < W; i += BAND_THREADS) { sg[i] = gs[(size_t)row_below * W + i]; sg[(nr + 1) * W + i] = gs[(size_t)row_above * W + i]; }
     for (int t = tid; t < 64 * 32; t += BAND_THREADS) {
         const int e = t >> 5;
         uint32_t T2[2];
@@ -99,71 +114,31 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) band_run_i8(const __grid_cons
     uint32_t xa2 = 0, xb0 = 0;
     ChainKeys ck = {0u, 0u};
 
-    // one word (4 sites) of the new sublattice
-    auto update_word = [&](const uint32_t sw, const uint32_t hw, const uint32_t vw, const uint32_t n) -> uint32_t {
-        const uint32_t y = (hw & 0x40044004u) | (vw & ~0x40044004u);
-        const uint32_t z = ((sw & 0x20022002u) | (y & ~0x20022002u)) & 0xE00EE00Eu;
-        const uint32_t o01 = __dp4a(z, 0x00004080u, lane8), o23 = __dp4a(z, 0x40800000u, lane8);
-        const uint2 t01 = *reinterpret_cast<const uint2 *>(reinterpret_cast<const char *>(s_pair) + o01);
-        const uint2 t23 = *reinterpret_cast<const uint2 *>(reinterpret_cast<const char *>(s_pair) + o23);
-        uint32_t rw[4];
-        philox_site_words(n, p.keys, xa2, xb0, ck, rw);
-        uint32_t out = 0x01010101u;
-        out = add_if_not_less(out, rw[0], t01.x, 0xFEu);
-        out = add_if_not_less(out, rw[1], t01.y, 0xFEu << 8);
-        out = add_if_not_less(out, rw[2], t23.x, 0xFEu << 16);
-        out = add_if_not_less(out, rw[3], t23.y, 0xFEu << 24);
-        return out;
-    };
-
-    // One 16-byte vector (4 words = 16 sites = 4 Philox calls) per thread per trip, as in kernel_i8.cuh: the four
-    // independent chains interleave, the horizontal neighbours of three of the four words are in registers already.
-    // half 0: tau from sigma, rows ascending.  half 1: sigma from tau, rows walked from the last one down.
-    // `half` is a run-time value on purpose: one copy of this code serves both half-steps and every trip.
-    const int nvec = W >> 2, nvecs = nr * nvec;   // vectors per row, per band
-    auto update_vector = [&](const int half, const int c, uint2 *xmine, const uint32_t stamp) {
-        const uint32_t *src = half ? ta : sg;
-        uint32_t *dst = half ? sg : ta;
-        const uint32_t *halo = half ? ht : hs;
-        const int rr = (int)__umulhi((uint32_t)c, p.magicV), cv = c - rr * nvec;
-        const int r = half ? nr - 1 - rr : rr;
-        const int at = r * W + 4 * cv;
-        const uint4 s4 = *reinterpret_cast<const uint4 *>(src + at);
-        const bool edge = half ? r == nr - 1 : r == 0;
-        const uint4 v4 = *reinterpret_cast<const uint4 *>(edge ? halo + 4 * cv : src + (half ? at + W : at - W));
-        const int ce = half ? (cv == nvec - 1 ? 0 : 4 * cv + 4) : (cv == 0 ? W - 1 : 4 * cv - 1);
-        const uint32_t e = src[r * W + ce];
+    // one 16-byte vector (16 sites = 4 Philox calls, interleaved by the compiler) of the new sublattice:
+    // s4 = own words, v4 = vertical neighbours, e = the word holding the horizontal edge spin, n = Philox counter of word 0.
+    auto update_vector = [&](const int half, const uint4 s4, const uint4 v4, const uint32_t e, const uint32_t n) -> uint4 {
         const uint32_t w[4] = {s4.x, s4.y, s4.z, s4.w}, vw[4] = {v4.x, v4.y, v4.z, v4.w};
-        const uint32_t n = (uint32_t)(r0 + r) * (uint32_t)W + 4u * (uint32_t)cv;
         uint32_t o[4];
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
             const uint32_t hl = __funnelshift_l(j == 0 ? e : w[j - 1], w[j], 8);      // left neighbours (half 0)
             const uint32_t hr = __funnelshift_r(w[j], j == 3 ? e : w[j + 1], 8);      // right neighbours (half 1)
-            o[j] = update_word(w[j], half ? hr : hl, vw[j], n + (uint32_t)j);
+            const uint32_t hw = half ? hr : hl;
+            const uint32_t y = (hw & 0x40044004u) | (vw[j] & ~0x40044004u);
+            const uint32_t z = ((w[j] & 0x20022002u) | (y & ~0x20022002u)) & 0xE00EE00Eu;
+            const uint32_t o01 = __dp4a(z, 0x00004080u, lane8), o23 = __dp4a(z, 0x40800000u, lane8);
+            const uint2 t01 = *reinterpret_cast<const uint2 *>(reinterpret_cast<const char *>(s_pair) + o01);
+            const uint2 t23 = *reinterpret_cast<const uint2 *>(reinterpret_cast<const char *>(s_pair) + o23);
+            uint32_t rw[4];
+            philox_site_words(n + (uint32_t)j, p.keys, xa2, xb0, ck, rw);
+            uint32_t out = 0x01010101u;
+            out = add_if_not_less(out, rw[0], t01.x, 0xFEu);
+            out = add_if_not_less(out, rw[1], t01.y, 0xFEu << 8);
+            out = add_if_not_less(out, rw[2], t23.x, 0xFEu << 16);
+            out = add_if_not_less(out, rw[3], t23.y, 0xFEu << 24);
+            o[j] = out;
         }
-        *reinterpret_cast<uint4 *>(dst + at) = make_uint4(o[0], o[1], o[2], o[3]);
-        if (rr == 0) {                            // (tall bands only, see below) a vector of the row the neighbour waits for
-#pragma unroll
-            for (int j = 0; j < 4; ++j) st_pair(xmine + 4 * cv + j, o[j], stamp);
-        }
-    };
-
-    // The first row in walking order (first tau row in half 0, last sigma row in half 1) is the one the neighbouring band
-    // waits for and the only one that reads the incoming row: it is done one WORD per thread (a single Philox call, the
-    // shortest latency there is), ahead of the vectors, and each word leaves at once for the neighbour as a
-    // {word, stamp} pair -- no barrier on the critical path of the ring.
-    auto boundary_word = [&](const int half, const int cw, uint2 *xmine, const uint32_t stamp) {
-        const uint32_t *src = half ? ta : sg;
-        uint32_t *dst = half ? sg : ta;
-        const uint32_t *halo = half ? ht : hs;
-        const int r = half ? nr - 1 : 0, at = r * W + cw;
-        const uint32_t sw = src[at];
-        const uint32_t e = src[r * W + (half ? (cw == W - 1 ? 0 : cw + 1) : (cw == 0 ? W - 1 : cw - 1))];
-        const uint32_t hw = half ? __funnelshift_r(sw, e, 8) : __funnelshift_l(e, sw, 8);
-        const uint32_t out = update_word(sw, hw, halo[cw], (uint32_t)(r0 + r) * (uint32_t)W + (uint32_t)cw);
-        dst[at] = out;
-        st_pair(xmine + cw, out, stamp);
+        return make_uint4(o[0], o[1], o[2], o[3]);
     };
 
     // block-wide sums of up to six int partials into one record (int64 atomics: bands of a chain share the record)
@@ -182,90 +157,106 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) band_run_i8(const __grid_cons
         __syncthreads();
     };
 
-    // C_x, C_y of the record taken after the previous step: sigma is final, hs holds the sigma row below the band
+    // C_x, C_y of the record taken after the previous step: sigma is final, sg row 0 holds the new sigma row below the band
     auto bond_sums = [&](long long *dst) {
         int v[6] = {0, 0, 0, 0, 0, 0};
-        for (int c = tid; c < ncalls; c += BAND_THREADS) {
+        for (int c = tid; c < nr * W; c += BAND_THREADS) {
             const int r = (int)__umulhi((uint32_t)c, p.magicW), cw = c - r * W;
-            const uint32_t s0 = sg[c];
-            const uint32_t e = sg[r * W + (cw == 0 ? W - 1 : cw - 1)];
-            v[4] = __dp4a((int)s0, (int)__funnelshift_l(e, s0, 8), v[4]);             // sigma_x sigma_{x left}
-            v[5] = __dp4a((int)s0, (int)(r == 0 ? hs[cw] : sg[c - W]), v[5]);         // sigma_x sigma_{x down}
+            const uint32_t *row = sg + (r + 1) * W;
+            const uint32_t s0 = row[cw];
+            v[4] = __dp4a((int)s0, (int)__funnelshift_l(row[cw == 0 ? W - 1 : cw - 1], s0, 8), v[4]);   // sigma_x sigma_{x left}
+            v[5] = __dp4a((int)s0, (int)row[cw - W], v[5]);                                              // sigma_x sigma_{x down}
         }
         reduce_to(dst, v, 4, 2);
     };
 
-    // Receiving side of the exchange (polling warp only): copy the neighbour's published row into shared memory as soon
-    // as every word carries this half-step's stamp.
-    auto collect = [&](const uint2 *src, const uint32_t stamp, uint32_t *dst) {
-        // W <= 512: at most two rounds of 8 words per lane.  The loads are unconditional (indices past the row are
-        // clamped to its last word) and all eight are in flight together; a round is repeated until every word carries
-        // the stamp.  (A version with predicated loads compiled into a loop that was 3.7x slower.)
-        for (int i0 = 0; i0 < W; i0 += 256) {
-            uint2 v[8];
-            bool ok;
-            do {
-                ok = true;
-#pragma unroll
-                for (int j = 0; j < 8; ++j) v[j] = ld_pair(src + min(i0 + j * 32 + lane, W - 1));
-#pragma unroll
-                for (int j = 0; j < 8; ++j)
-                    if (v[j].y != stamp) ok = false;
-            } while (!ok);
-#pragma unroll
-            for (int j = 0; j < 8; ++j) {
-                const int i = i0 + j * 32 + lane;
-                if (i < W) dst[i] = v[j].x;
-            }
-        }
-    };
-
+    const int nvec = W >> 2;                      // vectors per row
+    const int n0 = (nr + 1) * nvec, n1 = nr * nvec;   // vectors of half-step 0 (band + redundant row) and of half-step 1
     long long *pending = nullptr;
     long long nrec = 0;
     // full steps until the next recorded one: a countdown instead of a 64-bit modulo per step
     long long until_rec = p.obs_every > 0 ? p.obs_every - (long long)(p.t0 % (unsigned long long)p.obs_every) : 0;
 #pragma unroll 1
-    for (long long h = 0; h < 2 * p.n_steps; ++h) {
-        const long long s = h >> 1;
-        const int half = (int)(h & 1);
+    for (long long s = 0; s < p.n_steps; ++s) {
         const unsigned long long t = p.t0 + (unsigned long long)s;
-        const int par = (int)(s & 1);
-        // half 0: tau <- sigma, field from the down and left neighbours (eq. (15)); hs is in place (loaded at the start,
-        // collected during the previous half-step 1 afterwards).  half 1: sigma <- tau, up and right neighbours (eq. (16)).
-        if (half == 0 && pending) { bond_sums(pending); pending = nullptr; }
-        device_half_step_keys(p.keys, 2ull * t + (unsigned long long)half, p.chain0 + (uint32_t)chain, xa2, xb0, ck);
+        // hand-over buffers: the rows published after step s-1 (parity (s-1) & 1) are read now
+        const uint32_t stamp_in = p.stamp0 + (uint32_t)s;
+        const uint2 *in_below = p.xtop + ((size_t)((s + 1) & 1) * nb + below) * W;   // top row of the band below = row r0-1
+        const uint2 *in_above = p.xbot + ((size_t)((s + 1) & 1) * nb + above) * W;   // bottom row of the band above = row r0+nr
 
-        // half 0 hands the first tau row to the band below, half 1 the last sigma row to the band above; the row this
-        // band needs next (tau above for half 1, sigma below for the next half 0 and for the bond sums) comes back the
-        // same way.  hs is not read during half-step 1, ht not during half-step 0.
-        const uint32_t stamp = p.stamp0 + (uint32_t)(h + 1);
-        uint2 *xmine = (half ? p.xs : p.xt) + ((size_t)par * nb + band) * W;
-        const uint2 *xnbr = (half ? p.xs : p.xt) + ((size_t)par * nb + (half ? down : up)) * W;
-        // The last warp does no arithmetic: it polls for the neighbour's row from the start of the half-step, so the
-        // handshake (one L2 round trip after the neighbour's first vectors are done) hides behind the other 15 warps.
-        if (duty_warp) collect(xnbr, stamp, half ? hs : ht);
-        else if (nvecs <= 3 * WORKERS) {
-            // short bands: the hand-over is the critical path, so the neighbour's row goes first, word by word
+        // ---- half-step 0: tau <- sigma, field from the down and left neighbours (eq. (15)); rows 0 .. nr of the tau array.
+        // Order: the interior rows first, then row 0 (needs the sigma row below the band), then row nr (needs the sigma
+        // row above the band): those two wait for the neighbours' rows of the previous step (none on the first step of a
+        // launch: the halo rows came from global memory).
+        device_half_step_keys(p.keys, 2ull * t, p.chain0 + (uint32_t)chain, xa2, xb0, ck);
 #pragma unroll 1
-            for (int cw = tid; cw < W; cw += WORKERS) boundary_word(half, cw, xmine, stamp);
+        for (int c = tid; c < n0; c += BAND_THREADS) {
+            const int kk = (int)__umulhi((uint32_t)c, p.magicV), cv = c - kk * nvec;
+            const int i = kk < nr - 1 ? kk + 1 : (kk == nr - 1 ? 0 : nr);      // tau row
+            const uint32_t *self = sg + (i + 1) * W, *downr = sg + i * W;
+            uint4 s4, v4;
+            uint32_t e;
+            if (s > 0 && i == 0) {
+                // vertical neighbours from the band below, straight from the hand-over buffer
+                uint2 a, b, c2, d;
+                do { ld_pairs2(in_below + 4 * cv, a, b); ld_pairs2(in_below + 4 * cv + 2, c2, d); }
+                while (a.y != stamp_in || b.y != stamp_in || c2.y != stamp_in || d.y != stamp_in);
+                v4 = make_uint4(a.x, b.x, c2.x, d.x);
+                *reinterpret_cast<uint4 *>(sg + 4 * cv) = v4;                  // kept for the bond sums of a recorded step
+                s4 = *reinterpret_cast<const uint4 *>(self + 4 * cv);
+                e = self[cv == 0 ? W - 1 : 4 * cv - 1];
+            } else if (s > 0 && i == nr) {
+                // the row above the band: own words and the left edge spin from the band above
+                uint2 a, b, c2, d, ee;
+                const uint2 *pe = in_above + (cv == 0 ? W - 1 : 4 * cv - 1);
+                do { ld_pairs2(in_above + 4 * cv, a, b); ld_pairs2(in_above + 4 * cv + 2, c2, d); ee = ld_pair(pe); }
+                while (a.y != stamp_in || b.y != stamp_in || c2.y != stamp_in || d.y != stamp_in || ee.y != stamp_in);
+                s4 = make_uint4(a.x, b.x, c2.x, d.x);
+                e = ee.x;
+                v4 = *reinterpret_cast<const uint4 *>(downr + 4 * cv);
+            } else {
+                s4 = *reinterpret_cast<const uint4 *>(self + 4 * cv);
+                v4 = *reinterpret_cast<const uint4 *>(downr + 4 * cv);
+                e = self[cv == 0 ? W - 1 : 4 * cv - 1];
+            }
+            int gr = r0 + i;
+            if (gr >= L) gr -= L;
+            const uint4 o = update_vector(0, s4, v4, e, (uint32_t)gr * (uint32_t)W + 4u * (uint32_t)cv);
+            *reinterpret_cast<uint4 *>(ta + i * W + 4 * cv) = o;
+        }
+        __syncthreads();
+        if (pending) { bond_sums(pending); pending = nullptr; }   // (two more barriers, only after a recorded step)
+
+        // ---- half-step 1: sigma <- tau, up and right neighbours (eq. (16)); rows 0 .. nr-1.  Order: the top row and the
+        // bottom row first -- the neighbours wait for them -- each vector published by the thread that computed it.
+        device_half_step_keys(p.keys, 2ull * t + 1ull, p.chain0 + (uint32_t)chain, xa2, xb0, ck);
+        const uint32_t stamp_out = p.stamp0 + (uint32_t)s + 1u;
+        uint2 *out_top = p.xtop + ((size_t)(s & 1) * nb + band) * W;
+        uint2 *out_bot = p.xbot + ((size_t)(s & 1) * nb + band) * W;
 #pragma unroll 1
-            for (int c = nvec + tid; c < nvecs; c += WORKERS) update_vector(half, c, xmine, stamp);   // rows 1 .. nr-1
-        } else {
-            // tall bands: several trips of vectors hide the hand-over anyway; the row is part of the first trip
-#pragma unroll 1
-            for (int c = tid; c < nvecs; c += WORKERS) update_vector(half, c, xmine, stamp);
+        for (int c = tid; c < n1; c += BAND_THREADS) {
+            const int kk = (int)__umulhi((uint32_t)c, p.magicV), cv = c - kk * nvec;
+            const int i = kk == 0 ? nr - 1 : (kk == 1 ? 0 : kk - 1);          // sigma row
+            const uint32_t *self = ta + i * W;
+            const uint4 s4 = *reinterpret_cast<const uint4 *>(self + 4 * cv);
+            const uint4 v4 = *reinterpret_cast<const uint4 *>(self + W + 4 * cv);
+            const uint32_t e = self[cv == nvec - 1 ? 0 : 4 * cv + 4];
+            const uint4 o = update_vector(1, s4, v4, e, (uint32_t)(r0 + i) * (uint32_t)W + 4u * (uint32_t)cv);
+            *reinterpret_cast<uint4 *>(sg + (i + 1) * W + 4 * cv) = o;
+            if (i == nr - 1) { st_pairs2(out_top + 4 * cv, o.x, o.y, stamp_out); st_pairs2(out_top + 4 * cv + 2, o.z, o.w, stamp_out); }
+            if (i == 0) { st_pairs2(out_bot + 4 * cv, o.x, o.y, stamp_out); st_pairs2(out_bot + 4 * cv + 2, o.z, o.w, stamp_out); }
         }
         __syncthreads();
 
-        // record (M_sigma, M_tau, E_J, E_q now; C_x, C_y at the start of the next half-step 0)
-        if (half == 1 && p.obs_every > 0 && --until_rec == 0) {
+        // record (M_sigma, M_tau, E_J, E_q now; C_x, C_y once the new sigma row below the band has arrived)
+        if (p.obs_every > 0 && --until_rec == 0) {
             until_rec = p.obs_every;
             long long *dst = p.rec + ((size_t)nrec * p.n_chains + chain) * 6;
             int v[6] = {0, 0, 0, 0, 0, 0};
-            for (int c = tid; c < ncalls; c += BAND_THREADS) {
+            for (int c = tid; c < nr * W; c += BAND_THREADS) {
                 const int r = (int)__umulhi((uint32_t)c, p.magicW), cw = c - r * W;
-                const uint32_t s0 = sg[c], t0w = ta[c];
-                const uint32_t tu = r == nr - 1 ? ht[cw] : ta[c + W];
+                const uint32_t s0 = sg[W + c], t0w = ta[c];
+                const uint32_t tu = ta[c + W];                                  // row nr of ta is the redrawn row above the band
                 const uint32_t tr = __funnelshift_r(t0w, ta[r * W + (cw == W - 1 ? 0 : cw + 1)], 8);
                 v[0] = __dp4a((int)s0, 0x01010101, v[0]);
                 v[1] = __dp4a((int)t0w, 0x01010101, v[1]);
@@ -278,8 +269,19 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) band_run_i8(const __grid_cons
             ++nrec;
         }
     }
-    if (pending) bond_sums(pending);              // hs already holds the final sigma row below the band
-    for (int i = tid; i < ncalls; i += BAND_THREADS) { gs[(size_t)r0 * W + i] = sg[i]; gt[(size_t)r0 * W + i] = ta[i]; }
+    if (pending) {
+        // the last step was recorded: fetch the final sigma row below the band (the neighbour published it after its last step)
+        const uint32_t stamp_in = p.stamp0 + (uint32_t)p.n_steps;
+        const uint2 *in_below = p.xtop + ((size_t)((p.n_steps + 1) & 1) * nb + below) * W;
+        for (int i = tid; i < W; i += BAND_THREADS) {
+            uint2 a;
+            do { a = ld_pair(in_below + i); } while (a.y != stamp_in);
+            sg[i] = a.x;
+        }
+        __syncthreads();
+        bond_sums(pending);
+    }
+    for (int i = tid; i < nr * W; i += BAND_THREADS) { gs[(size_t)r0 * W + i] = sg[W + i]; gt[(size_t)r0 * W + i] = ta[i]; }
 }
 
 } // namespace shaken

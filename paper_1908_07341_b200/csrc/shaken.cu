@@ -36,7 +36,7 @@ struct shaken_ctx {
     int64_t n_rec = 0;
     uint32_t *d_tab = nullptr;    // [n_chains][8] per-chain tables for shaken_run_grid
     unsigned long long *d_bad = nullptr;
-    uint2 *d_xch = nullptr;       // band path: exchange rows xs, xt ([2][n_bands][L/4] {word, stamp} each)
+    uint2 *d_xch = nullptr;       // band path: hand-over rows xtop, xbot ([2][n_bands][L/4] {word, stamp} each)
     size_t xch_bytes = 0;
     uint32_t xch_stamp = 0;       // last stamp written into d_xch
     int coop = -1;                // cooperative launch supported (-1: not queried yet)
@@ -591,7 +591,7 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
         const int rpb = (ctx->L + bpc - 1) / bpc;
         bpc = (ctx->L + rpb - 1) / rpb;
         const int W = ctx->L / 4;
-        const size_t smem = ((size_t)2 * rpb * W + 2 * (size_t)W) * sizeof(uint32_t);   // two band layers, two halo rows
+        const size_t smem = band_smem_bytes(ctx->L, rpb);       // two band layers, two sigma halo rows, the redundant tau row
         const int n_bands = bpc * ctx->n_chains;
         // worth it while a half-step is short next to a launch; measured against the strip kernels: 3.6x at 512^2, 2.5x at
         // 1024^2, 2.2x at 2048^2 (the largest band that fits shared memory)
@@ -611,7 +611,7 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
                 ctx->xch_stamp = 0xFFFFFFFFu;                            // forces the clearing below
             }
             // stamps must be new to the buffer: clear it when the 32-bit stamp space would wrap (or after allocation)
-            if ((uint64_t)ctx->xch_stamp + 2ull * (uint64_t)n_steps + 2ull >= 0xFFFFFFFFull) {
+            if ((uint64_t)ctx->xch_stamp + (uint64_t)n_steps + 2ull >= 0xFFFFFFFFull) {
                 if ((uint64_t)n_steps >= 0x7FFFFFF0ull) return fail(ctx, SHAKEN_EINVAL, "shaken_run: n_steps too large for one call");
                 CU(cudaMemsetAsync(ctx->d_xch, 0, ctx->xch_bytes, ctx->stream));
                 ctx->xch_stamp = 0;
@@ -632,12 +632,12 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
             make_step_keys(ctx->seed, 0, bp.keys);
             bp.bpc = bpc;
             bp.rows_per_band = rpb;
-            bp.xs = ctx->d_xch;
-            bp.xt = ctx->d_xch + xrow;
+            bp.xtop = ctx->d_xch;
+            bp.xbot = ctx->d_xch + xrow;
             bp.stamp0 = ctx->xch_stamp;
             bp.magicW = (uint32_t)(4294967296ull / (uint64_t)W) + 1u;
             bp.magicV = (uint32_t)(4294967296ull / (uint64_t)(W / 4)) + 1u;
-            ctx->xch_stamp += (uint32_t)(2 * n_steps);
+            ctx->xch_stamp += (uint32_t)n_steps;                         // one stamp per full step
             CU(cudaFuncSetAttribute(band_run_i8, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
             void *args[] = {&bp};
             // the bands wait for one another, so they must all be resident: a cooperative launch either guarantees
@@ -651,7 +651,7 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
                 return SHAKEN_OK;
             }
             cudaGetLastError();
-            ctx->xch_stamp -= (uint32_t)(2 * n_steps);
+            ctx->xch_stamp -= (uint32_t)n_steps;
             if (le != cudaErrorCooperativeLaunchTooLarge && le != cudaErrorLaunchOutOfResources && le != cudaErrorNotSupported)
                 return fail(ctx, SHAKEN_ECUDA, "band kernel launch: %s", cudaGetErrorString(le));
         }
