@@ -141,6 +141,34 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) band_run_i8(const __grid_cons
         return make_uint4(o[0], o[1], o[2], o[3]);
     };
 
+    // The same vector in two stages, for the rows that wait for a neighbour: a site's random word does not depend on any
+    // spin, so the Philox calls (85 % of the instructions) are made BEFORE the wait and only the table lookups and the
+    // compares are left for after it.
+    auto draw = [&](const uint32_t n, uint32_t (&R)[4][4]) {
+#pragma unroll
+        for (int j = 0; j < 4; ++j) philox_site_words(n + (uint32_t)j, p.keys, xa2, xb0, ck, R[j]);
+    };
+    auto apply0 = [&](const uint4 s4, const uint4 v4, const uint32_t e, const uint32_t (&R)[4][4]) -> uint4 {
+        const uint32_t w[4] = {s4.x, s4.y, s4.z, s4.w}, vw[4] = {v4.x, v4.y, v4.z, v4.w};
+        uint32_t o[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const uint32_t hw = __funnelshift_l(j == 0 ? e : w[j - 1], w[j], 8);      // left neighbours
+            const uint32_t y = (hw & 0x40044004u) | (vw[j] & ~0x40044004u);
+            const uint32_t z = ((w[j] & 0x20022002u) | (y & ~0x20022002u)) & 0xE00EE00Eu;
+            const uint32_t o01 = __dp4a(z, 0x00004080u, lane8), o23 = __dp4a(z, 0x40800000u, lane8);
+            const uint2 t01 = *reinterpret_cast<const uint2 *>(reinterpret_cast<const char *>(s_pair) + o01);
+            const uint2 t23 = *reinterpret_cast<const uint2 *>(reinterpret_cast<const char *>(s_pair) + o23);
+            uint32_t out = 0x01010101u;
+            out = add_if_not_less(out, R[j][0], t01.x, 0xFEu);
+            out = add_if_not_less(out, R[j][1], t01.y, 0xFEu << 8);
+            out = add_if_not_less(out, R[j][2], t23.x, 0xFEu << 16);
+            out = add_if_not_less(out, R[j][3], t23.y, 0xFEu << 24);
+            o[j] = out;
+        }
+        return make_uint4(o[0], o[1], o[2], o[3]);
+    };
+
     // block-wide sums of up to six int partials into one record (int64 atomics: bands of a chain share the record)
     auto reduce_to = [&](long long *dst, const int (&v)[6], const int first, const int count) {
 #pragma unroll
@@ -194,34 +222,33 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) band_run_i8(const __grid_cons
             const int kk = (int)__umulhi((uint32_t)c, p.magicV), cv = c - kk * nvec;
             const int i = kk < nr - 1 ? kk + 1 : (kk == nr - 1 ? 0 : nr);      // tau row
             const uint32_t *self = sg + (i + 1) * W, *downr = sg + i * W;
-            uint4 s4, v4;
-            uint32_t e;
+            int gr = r0 + i;
+            if (gr >= L) gr -= L;
+            const uint32_t n = (uint32_t)gr * (uint32_t)W + 4u * (uint32_t)cv;
+            uint4 o;
             if (s > 0 && i == 0) {
-                // vertical neighbours from the band below, straight from the hand-over buffer
+                // vertical neighbours from the band below, straight from the hand-over buffer; random words first
+                uint32_t R[4][4];
+                draw(n, R);
                 uint2 a, b, c2, d;
                 do { ld_pairs2(in_below + 4 * cv, a, b); ld_pairs2(in_below + 4 * cv + 2, c2, d); }
                 while (a.y != stamp_in || b.y != stamp_in || c2.y != stamp_in || d.y != stamp_in);
-                v4 = make_uint4(a.x, b.x, c2.x, d.x);
+                const uint4 v4 = make_uint4(a.x, b.x, c2.x, d.x);
                 *reinterpret_cast<uint4 *>(sg + 4 * cv) = v4;                  // kept for the bond sums of a recorded step
-                s4 = *reinterpret_cast<const uint4 *>(self + 4 * cv);
-                e = self[cv == 0 ? W - 1 : 4 * cv - 1];
+                o = apply0(*reinterpret_cast<const uint4 *>(self + 4 * cv), v4, self[cv == 0 ? W - 1 : 4 * cv - 1], R);
             } else if (s > 0 && i == nr) {
-                // the row above the band: own words and the left edge spin from the band above
+                // the row above the band: own words and the left edge spin from the band above; random words first
+                uint32_t R[4][4];
+                draw(n, R);
                 uint2 a, b, c2, d, ee;
                 const uint2 *pe = in_above + (cv == 0 ? W - 1 : 4 * cv - 1);
                 do { ld_pairs2(in_above + 4 * cv, a, b); ld_pairs2(in_above + 4 * cv + 2, c2, d); ee = ld_pair(pe); }
                 while (a.y != stamp_in || b.y != stamp_in || c2.y != stamp_in || d.y != stamp_in || ee.y != stamp_in);
-                s4 = make_uint4(a.x, b.x, c2.x, d.x);
-                e = ee.x;
-                v4 = *reinterpret_cast<const uint4 *>(downr + 4 * cv);
+                o = apply0(make_uint4(a.x, b.x, c2.x, d.x), *reinterpret_cast<const uint4 *>(downr + 4 * cv), ee.x, R);
             } else {
-                s4 = *reinterpret_cast<const uint4 *>(self + 4 * cv);
-                v4 = *reinterpret_cast<const uint4 *>(downr + 4 * cv);
-                e = self[cv == 0 ? W - 1 : 4 * cv - 1];
+                o = update_vector(0, *reinterpret_cast<const uint4 *>(self + 4 * cv), *reinterpret_cast<const uint4 *>(downr + 4 * cv),
+                                  self[cv == 0 ? W - 1 : 4 * cv - 1], n);
             }
-            int gr = r0 + i;
-            if (gr >= L) gr -= L;
-            const uint4 o = update_vector(0, s4, v4, e, (uint32_t)gr * (uint32_t)W + 4u * (uint32_t)cv);
             *reinterpret_cast<uint4 *>(ta + i * W + 4 * cv) = o;
         }
         __syncthreads();
