@@ -251,6 +251,14 @@ int shaken_philox_words(const uint32_t *ctr, const uint32_t *key, uint32_t *out,
  */
 int shaken_selftest_philox_rate(int32_t blocks_per_sm, int32_t iters, int32_t reps, double *sites_per_ns);
 
+/*
+ * shaken_test_band_hook: test hook for the one-launch band path (mid-size lattices).  what = 0: the
+ * stamp counter of the hand-over buffer is set to `value` (a value near 2^32 exercises the wrap-around clearing);
+ * what = 1: the next cooperative launch is treated as refused (value != 0), which exercises the fall-back to the
+ * per-half-step kernels.  Results never depend on either.  SHAKEN_EINVAL for another selector.
+ */
+int shaken_test_band_hook(shaken_ctx *ctx, int what, uint32_t value);
+
 /* Number of kernels this context has launched so far (half-steps, init, conversions, reductions). */
 int64_t shaken_launch_count(const shaken_ctx *ctx);
 

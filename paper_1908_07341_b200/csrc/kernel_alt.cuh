@@ -21,6 +21,7 @@
 
 #include "kernels_common.cuh"
 #include "kernel_small.cuh"
+#include "kernel_band.cuh"
 
 namespace shaken {
 
@@ -512,6 +513,168 @@ __global__ void __launch_bounds__(256) alt_small_i8(const __grid_constant__ Smal
         uint32_t *gs = reinterpret_cast<uint32_t *>(p.sigma + (size_t)(chain_first + m) * L * L);
         for (int i = tid; i < words; i += blockDim.x) gs[i] = smem[m * words + i];
     }
+}
+
+// Mid-size lattices (128 < L <= 2048, few chains): the whole run in ONE cooperative launch, row bands in shared memory,
+// as kernel_band.cuh does for the shaken dynamics (two launches per step are 6-9 us of launch latency for well under a
+// microsecond of work at 1024^2).  Here a redrawn site reads the rows above AND below, so a band keeps TWO halo rows on
+// either side and redraws, in half-step 0, also the nearest halo row on each side (redundantly: the random word of a site
+// is a function of the site), which makes the halo of half-step 1 valid without a hand-over in between.  Bands exchange
+// once per full step: after half-step 1 a band publishes its two bottom and its two top rows ({word, stamp} pairs, see
+// kernel_band.cuh) and collects the neighbours' rows at the start of the next step.  rows_per_band is even, so every
+// band has at least two rows.  BandParams: xtop / xbot hold [2][n_bands][2][L/4] pairs, utab / gtab the table A[0..4].
+__host__ __device__ inline size_t alt_band_smem_bytes(int L, int rows_per_band) { return (size_t)(rows_per_band + 4) * (size_t)(L / 4) * sizeof(uint32_t); }
+
+__global__ void __launch_bounds__(BAND_THREADS, 1) alt_band_i8(const __grid_constant__ BandParams p)
+{
+    extern __shared__ __align__(16) uint32_t smem[];
+    __shared__ __align__(256) uint32_t s_tab[ALT_TAB_WORDS];
+    __shared__ long long s_red[BAND_THREADS / 32][3];
+
+    const int L = p.L, W = L >> 2, nvec = W >> 2;
+    const int band = blockIdx.x, chain = band / p.bpc, k = band - chain * p.bpc;
+    const int r0 = k * p.rows_per_band;
+    const int nr = min(L, r0 + p.rows_per_band) - r0;                 // rows of this band (even, >= 2)
+    const int below = chain * p.bpc + (k == 0 ? p.bpc - 1 : k - 1);
+    const int above = chain * p.bpc + (k == p.bpc - 1 ? 0 : k + 1);
+    const int nb = gridDim.x;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    uint32_t *sg = smem;                          // row index j holds global row r0 - 2 + j (mod L), j = 0 .. nr + 3
+    uint32_t *gs = reinterpret_cast<uint32_t *>(p.sigma + (size_t)chain * L * L);
+    for (int i = tid; i < (nr + 4) * W; i += BAND_THREADS) {
+        const int j = (int)__umulhi((uint32_t)i, p.magicW), cw = i - j * W;
+        int gr = r0 - 2 + j;
+        gr = gr < 0 ? gr + L : (gr >= L ? gr - L : gr);
+        sg[i] = gs[(size_t)gr * W + cw];
+    }
+    if (tid < 8) s_tab[tid] = tid < 5 ? (p.gtab ? p.gtab[(size_t)chain * 8 + 4 - tid] : p.utab[4 - tid]) : 0u;   // entry i = A[4 - i]
+    __syncthreads();
+    const uint32_t tb = shared_addr(s_tab);
+
+    uint32_t xa2 = 0, xb0 = 0;
+    ChainKeys ck = {0u, 0u};
+    // one vector (16 sites, the 8 of the row's active parity redrawn) of row index j, in place
+    auto redraw = [&](const int half, const int j, const int v) -> uint4 {
+        int gr = r0 - 2 + j;
+        gr = gr < 0 ? gr + L : (gr >= L ? gr - L : gr);
+        uint32_t *row = sg + j * W;
+        const uint4 c4 = *reinterpret_cast<const uint4 *>(row + 4 * v);
+        const uint32_t cw[6] = {row[v == 0 ? W - 1 : 4 * v - 1], c4.x, c4.y, c4.z, c4.w, row[v + 1 == nvec ? 0 : 4 * v + 4]};
+        uint32_t fu[4], fd[4];
+        minus4(*reinterpret_cast<const uint4 *>(row + W + 4 * v), fu);
+        minus4(*reinterpret_cast<const uint4 *>(row - W + 4 * v), fd);
+        uint32_t rnd[8];
+        const uint32_t n0 = (uint32_t)gr * (uint32_t)(L >> 3) + 2u * (uint32_t)v;
+        philox_site_words(n0, p.keys, xa2, xb0, ck, rnd);
+        philox_site_words(n0 + 1u, p.keys, xa2, xb0, ck, rnd + 4);
+        int d0 = 0, d1 = 0, d2 = 0, d3 = 0;
+        const uint4 o = ((gr + half) & 1) ? alt_vector_i8<1, false>(cw, fu, fd, rnd, tb, d0, d1, d2, d3) : alt_vector_i8<0, false>(cw, fu, fd, rnd, tb, d0, d1, d2, d3);
+        *reinterpret_cast<uint4 *>(row + 4 * v) = o;
+        return o;
+    };
+    auto reduce_to = [&](long long *dst, const int (&v)[3], const int first, const int count, const int slot0) {
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            const int w = __reduce_add_sync(0xFFFFFFFFu, v[j]);
+            if (lane == 0) s_red[warp][j] = w;
+        }
+        __syncthreads();
+        if (tid < count) {
+            long long tot = 0;
+            for (int w = 0; w < BAND_THREADS / 32; ++w) tot += s_red[w][first + tid];
+            atomicAdd(reinterpret_cast<unsigned long long *>(dst + slot0 + (tid ? 3 + tid : 0)), (unsigned long long)tot);   // M, C_x, C_y sit at 0, 4, 5
+        }
+        __syncthreads();
+    };
+    // the part of C_y that waits for the neighbour: the band's bottom row against the neighbour's NEW top row (row index 1)
+    auto bond_y_edge = [&](long long *dst) {
+        int v[3] = {0, 0, 0};
+        for (int c = tid; c < W; c += BAND_THREADS) v[2] = __dp4a((int)sg[2 * W + c], (int)sg[W + c], v[2]);
+        reduce_to(dst, v, 2, 1, 5);
+    };
+    // neighbours' rows of the step just finished: row indices 0, 1 from the band below, nr + 2, nr + 3 from the band above
+    auto collect = [&](const long long s_done, const bool only_below) {
+        const uint32_t stamp_in = p.stamp0 + (uint32_t)s_done;
+        const uint2 *in_below = p.xtop + ((size_t)((s_done + 1) & 1) * nb + below) * 2 * W;
+        const uint2 *in_above = p.xbot + ((size_t)((s_done + 1) & 1) * nb + above) * 2 * W;
+        for (int i = tid; i < (only_below ? 2 : 4) * W; i += BAND_THREADS) {
+            const uint2 *src = i < 2 * W ? in_below + i : in_above + (i - 2 * W);
+            uint2 a;
+            do { a = ld_pair(src); } while (a.y != stamp_in);
+            sg[i < 2 * W ? i : (nr + 2) * W + (i - 2 * W)] = a.x;
+        }
+    };
+
+    long long *pending = nullptr;
+    long long nrec = 0;
+    long long until_rec = p.obs_every > 0 ? p.obs_every - (long long)(p.t0 % (unsigned long long)p.obs_every) : 0;
+#pragma unroll 1
+    for (long long s = 0; s < p.n_steps; ++s) {
+        const unsigned long long t = p.t0 + (unsigned long long)s;
+        // half-step 0: colour 0 of row indices 1 .. nr + 2 (the band and one halo row on either side).  First the rows
+        // that read only the band's own rows (indices 3 .. nr), then the neighbours' rows of the previous step are
+        // collected -- they were published early in the neighbours' half-step 1 and have had all that time to arrive --
+        // and the four rows next to them follow (indices 1, 2, nr + 1, nr + 2).
+        device_half_step_keys(p.keys, 2ull * t, p.chain0 + (uint32_t)chain, xa2, xb0, ck);
+#pragma unroll 1
+        for (int c = tid; c < (nr - 2) * nvec; c += BAND_THREADS) {
+            const int kk = (int)__umulhi((uint32_t)c, p.magicV);
+            redraw(0, 3 + kk, c - kk * nvec);
+        }
+        if (s > 0) collect(s, false);
+        __syncthreads();
+        if (pending) { bond_y_edge(pending); pending = nullptr; }
+#pragma unroll 1
+        for (int c = tid; c < 4 * nvec; c += BAND_THREADS) {
+            const int kk = (int)__umulhi((uint32_t)c, p.magicV);
+            redraw(0, kk < 2 ? 1 + kk : nr - 1 + kk, c - kk * nvec);
+        }
+        __syncthreads();
+        // half-step 1: colour 1 of the band's rows (indices 2 .. nr + 1); the two top rows and the two bottom rows first,
+        // each vector published by the thread that computed it
+        device_half_step_keys(p.keys, 2ull * t + 1ull, p.chain0 + (uint32_t)chain, xa2, xb0, ck);
+        const uint32_t stamp_out = p.stamp0 + (uint32_t)s + 1u;
+        uint2 *out_top = p.xtop + ((size_t)(s & 1) * nb + band) * 2 * W;   // rows r1-2, r1-1
+        uint2 *out_bot = p.xbot + ((size_t)(s & 1) * nb + band) * 2 * W;   // rows r0, r0+1
+#pragma unroll 1
+        for (int c = tid; c < nr * nvec; c += BAND_THREADS) {
+            const int kk = (int)__umulhi((uint32_t)c, p.magicV), v = c - kk * nvec;
+            const int j = kk == 0 ? nr + 1 : (kk == 1 ? nr : kk);              // row index: nr+1, nr, 2, 3, 4 .. nr-1
+            const uint4 o = redraw(1, j, v);
+            if (j >= nr) {
+                uint2 *x = out_top + (j - nr) * W + 4 * v;
+                st_pair(x, o.x, stamp_out); st_pair(x + 1, o.y, stamp_out); st_pair(x + 2, o.z, stamp_out); st_pair(x + 3, o.w, stamp_out);
+            }
+            if (j <= 3) {
+                uint2 *x = out_bot + (j - 2) * W + 4 * v;
+                st_pair(x, o.x, stamp_out); st_pair(x + 1, o.y, stamp_out); st_pair(x + 2, o.z, stamp_out); st_pair(x + 3, o.w, stamp_out);
+            }
+        }
+        __syncthreads();
+        // record (M, 0, 0, 0, C_x, C_y): M and C_x now, C_y once the neighbour's new top row has been collected
+        if (p.obs_every > 0 && --until_rec == 0) {
+            until_rec = p.obs_every;
+            long long *dst = p.rec + ((size_t)nrec * p.n_chains + chain) * 6;
+            int v[3] = {0, 0, 0};
+            for (int c = tid; c < nr * W; c += BAND_THREADS) {
+                const int r = (int)__umulhi((uint32_t)c, p.magicW), cw = c - r * W;
+                const uint32_t *row = sg + (2 + r) * W;
+                const uint32_t s0 = row[cw];
+                v[0] = __dp4a((int)s0, 0x01010101, v[0]);
+                v[1] = __dp4a((int)s0, (int)__funnelshift_r(s0, row[cw == W - 1 ? 0 : cw + 1], 8), v[1]);   // sigma_x sigma_{x right}
+                if (r > 0) v[2] = __dp4a((int)s0, (int)row[cw - W], v[2]);                                  // sigma_x sigma_{x down} inside the band
+            }
+            reduce_to(dst, v, 0, 3, 0);
+            pending = dst;
+            ++nrec;
+        }
+    }
+    if (pending) {
+        collect(p.n_steps, true);
+        __syncthreads();
+        bond_y_edge(pending);
+    }
+    for (int i = tid; i < nr * W; i += BAND_THREADS) gs[(size_t)r0 * W + i] = sg[2 * W + i];
 }
 
 } // namespace shaken

@@ -66,6 +66,10 @@ __device__ __forceinline__ uint2 ld_pair(const uint2 *p)
     asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
     return make_uint2((uint32_t)v, (uint32_t)(v >> 32));
 }
+__device__ __forceinline__ void st_pair(uint2 *p, uint32_t word, uint32_t stamp)
+{
+    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" :: "l"(p), "l"(((unsigned long long)stamp << 32) | word) : "memory");
+}
 __device__ __forceinline__ void st_pairs2(uint2 *p, uint32_t w0, uint32_t w1, uint32_t stamp)
 {
     const unsigned long long s = (unsigned long long)stamp << 32;

@@ -40,6 +40,8 @@ struct shaken_ctx {
     size_t xch_bytes = 0;
     uint32_t xch_stamp = 0;       // last stamp written into d_xch
     int coop = -1;                // cooperative launch supported (-1: not queried yet)
+    bool band_refused = false;    // test hook: never take the band path
+    bool band_refuse_next = false;   // test hook: treat the next cooperative launch as refused (exercises the fall-back)
     void *d_stage = nullptr;      // staging for packed <-> int8 conversion
     size_t stage_bytes = 0;
 
@@ -472,6 +474,96 @@ static int choose_rows_per_task(const shaken_ctx *ctx, int nseg, long long grid_
     return best;
 }
 
+// ---------------------------------------------------------------------------------------------------
+// Band path (kernel_band.cuh, kernel_alt.cuh: alt_band_i8): mid-size lattices, few chains -- the whole run in ONE
+// cooperative launch, row bands resident in shared memory.  Returns 0 when the run was launched (bookkeeping done),
+// 1 when the path does not apply or the cooperative launch was refused (the strip kernels do the job then), < 0 on error.
+// ---------------------------------------------------------------------------------------------------
+static int try_band_launch(shaken_ctx *ctx, bool alternate, const uint32_t *gtab, const uint32_t utab[8], int64_t n_steps, int64_t obs_every, int64_t n_new)
+{
+    if (ctx->packed || ctx->variant != 0 || ctx->group != 1 || ctx->L <= SMALL_L_MAX || ctx->L > BAND_L_MAX || ctx->n_chains > ctx->num_sms) return 1;
+    if (ctx->coop < 0) {
+        int dev = 0, v = 0;
+        CU(cudaGetDevice(&dev));
+        CU(cudaDeviceGetAttribute(&v, cudaDevAttrCooperativeLaunch, dev));
+        ctx->coop = v;
+    }
+    int bpc = ctx->num_sms / ctx->n_chains;
+    if (bpc > ctx->L) bpc = ctx->L;
+    int rpb = (ctx->L + bpc - 1) / bpc;
+    if (alternate) rpb += rpb & 1;                                    // even: every band has at least two rows (L is even)
+    bpc = (ctx->L + rpb - 1) / rpb;
+    const int W = ctx->L / 4;
+    const size_t smem = alternate ? alt_band_smem_bytes(ctx->L, rpb) : band_smem_bytes(ctx->L, rpb);
+    const int n_bands = bpc * ctx->n_chains;
+    // worth it while a half-step is short next to a launch; measured against the strip kernels: 3.6x at 512^2, 2.5x at
+    // 1024^2, 2.2x at 2048^2 (the largest band that fits shared memory)
+    const bool small_job = (double)ctx->n_chains * ctx->L * ctx->L <= 4.5e6;
+    if (!ctx->coop || !small_job || smem > 160 * 1024 || ctx->band_refused) return 1;
+    const int rows_out = alternate ? 2 : 1;                           // rows a band publishes per side and step
+    const size_t xrow = (size_t)2 * n_bands * rows_out * W;           // uint2 elements per hand-over array (two parities)
+    const size_t need = 2 * xrow * sizeof(uint2);
+    if (ctx->xch_bytes < need) {
+        cudaFree(ctx->d_xch);
+        ctx->d_xch = nullptr;
+        ctx->xch_bytes = 0;
+        if (cudaMalloc(&ctx->d_xch, need) != cudaSuccess) {
+            cudaGetLastError();
+            return fail(ctx, SHAKEN_ENOMEM, "cudaMalloc of %zu exchange bytes failed", need);
+        }
+        ctx->xch_bytes = need;
+        ctx->xch_stamp = 0xFFFFFFFFu;                                // forces the clearing below
+    }
+    // stamps must be new to the buffer: clear it when the 32-bit stamp space would wrap (or after allocation)
+    if ((uint64_t)ctx->xch_stamp + (uint64_t)n_steps + 2ull >= 0xFFFFFFFFull) {
+        if ((uint64_t)n_steps >= 0x7FFFFFF0ull) return fail(ctx, SHAKEN_EINVAL, "shaken_run: n_steps too large for one call");
+        CU(cudaMemsetAsync(ctx->d_xch, 0, ctx->xch_bytes, ctx->stream));
+        ctx->xch_stamp = 0;
+    }
+    BandParams bp;
+    memset(&bp, 0, sizeof(bp));
+    bp.sigma = (uint8_t *)ctx->d_sigma;
+    bp.tau = (uint8_t *)ctx->d_tau;
+    bp.L = ctx->L;
+    bp.n_chains = ctx->n_chains;
+    bp.chain0 = ctx->chain0;
+    bp.t0 = ctx->step;
+    bp.n_steps = n_steps;
+    bp.obs_every = obs_every;
+    bp.rec = ctx->d_rec ? ctx->d_rec + (size_t)ctx->n_rec * ctx->n_chains * SHAKEN_N_OBS : nullptr;
+    bp.gtab = gtab;
+    memcpy(bp.utab, utab, sizeof(bp.utab));
+    make_step_keys(ctx->seed, 0, bp.keys);
+    bp.bpc = bpc;
+    bp.rows_per_band = rpb;
+    bp.xtop = ctx->d_xch;
+    bp.xbot = ctx->d_xch + xrow;
+    bp.stamp0 = ctx->xch_stamp;
+    bp.magicW = (uint32_t)(4294967296ull / (uint64_t)W) + 1u;
+    bp.magicV = (uint32_t)(4294967296ull / (uint64_t)(W / 4)) + 1u;
+    ctx->xch_stamp += (uint32_t)n_steps;                             // one stamp per full step
+    const void *kernel = alternate ? (const void *)alt_band_i8 : (const void *)band_run_i8;
+    CU(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    void *args[] = {&bp};
+    // the bands wait for one another, so they must all be resident: a cooperative launch either guarantees
+    // that or fails up front (a smaller or shared GPU) -- then the strip kernels do the job
+    const cudaError_t le = ctx->band_refuse_next ? cudaErrorCooperativeLaunchTooLarge
+                                                 : cudaLaunchCooperativeKernel(kernel, dim3(n_bands), dim3(BAND_THREADS), args, smem, ctx->stream);
+    ctx->band_refuse_next = false;
+    if (le == cudaSuccess) {
+        ctx->launches++;
+        ctx->step += (uint64_t)n_steps;
+        ctx->n_rec += n_new;
+        if (!alternate) ctx->have_tau = true;
+        return 0;
+    }
+    cudaGetLastError();
+    ctx->xch_stamp -= (uint32_t)n_steps;
+    if (le != cudaErrorCooperativeLaunchTooLarge && le != cudaErrorLaunchOutOfResources && le != cudaErrorNotSupported)
+        return fail(ctx, SHAKEN_ECUDA, "band kernel launch: %s", cudaGetErrorString(le));
+    return 1;
+}
+
 static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool uniform, int64_t n_steps, int64_t obs_every)
 {
     if (n_steps < 0 || obs_every < 0) return fail(ctx, SHAKEN_EINVAL, "shaken_run: negative count");
@@ -579,82 +671,9 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
     }
 
     // band path: mid-size lattices, few chains -- the whole run in one cooperative launch (kernel_band.cuh)
-    if (!ctx->packed && ctx->variant == 0 && ctx->group == 1 && ctx->L > SMALL_L_MAX && ctx->L <= BAND_L_MAX && ctx->n_chains <= ctx->num_sms) {   // (small_path returned above)
-        if (ctx->coop < 0) {
-            int dev = 0, v = 0;
-            CU(cudaGetDevice(&dev));
-            CU(cudaDeviceGetAttribute(&v, cudaDevAttrCooperativeLaunch, dev));
-            ctx->coop = v;
-        }
-        int bpc = ctx->num_sms / ctx->n_chains;
-        if (bpc > ctx->L) bpc = ctx->L;
-        const int rpb = (ctx->L + bpc - 1) / bpc;
-        bpc = (ctx->L + rpb - 1) / rpb;
-        const int W = ctx->L / 4;
-        const size_t smem = band_smem_bytes(ctx->L, rpb);       // two band layers, two sigma halo rows, the redundant tau row
-        const int n_bands = bpc * ctx->n_chains;
-        // worth it while a half-step is short next to a launch; measured against the strip kernels: 3.6x at 512^2, 2.5x at
-        // 1024^2, 2.2x at 2048^2 (the largest band that fits shared memory)
-        const bool small_job = (double)ctx->n_chains * ctx->L * ctx->L <= 4.5e6;
-        if (ctx->coop && small_job && smem <= 160 * 1024) {
-            const size_t xrow = (size_t)2 * n_bands * W;                 // uint2 elements per exchange array
-            const size_t need = 2 * xrow * sizeof(uint2);
-            if (ctx->xch_bytes < need) {
-                cudaFree(ctx->d_xch);
-                ctx->d_xch = nullptr;
-                ctx->xch_bytes = 0;
-                if (cudaMalloc(&ctx->d_xch, need) != cudaSuccess) {
-                    cudaGetLastError();
-                    return fail(ctx, SHAKEN_ENOMEM, "cudaMalloc of %zu exchange bytes failed", need);
-                }
-                ctx->xch_bytes = need;
-                ctx->xch_stamp = 0xFFFFFFFFu;                            // forces the clearing below
-            }
-            // stamps must be new to the buffer: clear it when the 32-bit stamp space would wrap (or after allocation)
-            if ((uint64_t)ctx->xch_stamp + (uint64_t)n_steps + 2ull >= 0xFFFFFFFFull) {
-                if ((uint64_t)n_steps >= 0x7FFFFFF0ull) return fail(ctx, SHAKEN_EINVAL, "shaken_run: n_steps too large for one call");
-                CU(cudaMemsetAsync(ctx->d_xch, 0, ctx->xch_bytes, ctx->stream));
-                ctx->xch_stamp = 0;
-            }
-            BandParams bp;
-            memset(&bp, 0, sizeof(bp));
-            bp.sigma = (uint8_t *)ctx->d_sigma;
-            bp.tau = (uint8_t *)ctx->d_tau;
-            bp.L = ctx->L;
-            bp.n_chains = ctx->n_chains;
-            bp.chain0 = ctx->chain0;
-            bp.t0 = ctx->step;
-            bp.n_steps = n_steps;
-            bp.obs_every = obs_every;
-            bp.rec = ctx->d_rec ? ctx->d_rec + (size_t)ctx->n_rec * ctx->n_chains * SHAKEN_N_OBS : nullptr;
-            bp.gtab = p.gtab;
-            memcpy(bp.utab, p.utab, sizeof(bp.utab));
-            make_step_keys(ctx->seed, 0, bp.keys);
-            bp.bpc = bpc;
-            bp.rows_per_band = rpb;
-            bp.xtop = ctx->d_xch;
-            bp.xbot = ctx->d_xch + xrow;
-            bp.stamp0 = ctx->xch_stamp;
-            bp.magicW = (uint32_t)(4294967296ull / (uint64_t)W) + 1u;
-            bp.magicV = (uint32_t)(4294967296ull / (uint64_t)(W / 4)) + 1u;
-            ctx->xch_stamp += (uint32_t)n_steps;                         // one stamp per full step
-            CU(cudaFuncSetAttribute(band_run_i8, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-            void *args[] = {&bp};
-            // the bands wait for one another, so they must all be resident: a cooperative launch either guarantees
-            // that or fails up front (a smaller or shared GPU) -- then the strip kernels below do the job
-            const cudaError_t le = cudaLaunchCooperativeKernel((const void *)band_run_i8, dim3(n_bands), dim3(BAND_THREADS), args, smem, ctx->stream);
-            if (le == cudaSuccess) {
-                ctx->launches++;
-                ctx->step += (uint64_t)n_steps;
-                ctx->n_rec += n_new;
-                ctx->have_tau = true;
-                return SHAKEN_OK;
-            }
-            cudaGetLastError();
-            ctx->xch_stamp -= (uint32_t)n_steps;
-            if (le != cudaErrorCooperativeLaunchTooLarge && le != cudaErrorLaunchOutOfResources && le != cudaErrorNotSupported)
-                return fail(ctx, SHAKEN_ECUDA, "band kernel launch: %s", cudaGetErrorString(le));
-        }
+    {
+        const int br = try_band_launch(ctx, false, p.gtab, p.utab, n_steps, obs_every, n_new);
+        if (br <= 0) return br;                                       // 0: done, < 0: error, 1: not applicable / refused
     }
 
     const long long blocks_needed = ctx->perwarp ? (p.ntasks + I8_THREADS / 32 - 1) / (I8_THREADS / 32) : p.ntasks;
@@ -834,6 +853,12 @@ static int run_alt_impl(shaken_ctx *ctx, const double *J, bool uniform, int64_t 
         ctx->step += (uint64_t)n_steps;
         ctx->n_rec += n_new;
         return SHAKEN_OK;
+    }
+
+    // mid-size lattices, few chains: the whole run in one cooperative launch (kernel_alt.cuh: alt_band_i8)
+    {
+        const int br = try_band_launch(ctx, true, p.gtab, p.utab, n_steps, obs_every, n_new);
+        if (br <= 0) return br;
     }
 
     const int wpb = ALT_THREADS / 32;
@@ -1168,6 +1193,15 @@ extern "C" int shaken_selftest_philox_rate(int32_t blocks_per_sm, int32_t iters,
 // ---------------------------------------------------------------------------------------------------
 // test hook
 // ---------------------------------------------------------------------------------------------------
+extern "C" int shaken_test_band_hook(shaken_ctx *ctx, int what, uint32_t value)
+{
+    if (!ctx) return fail(nullptr, SHAKEN_EINVAL, "shaken_test_band_hook: ctx is NULL");
+    if (what == 0) ctx->xch_stamp = value;              // next band launch starts its stamps here (wrap handling)
+    else if (what == 1) ctx->band_refuse_next = value != 0;   // next cooperative launch counts as refused
+    else return fail(ctx, SHAKEN_EINVAL, "shaken_test_band_hook: unknown selector %d", what);
+    return SHAKEN_OK;
+}
+
 extern "C" int shaken_philox_words(const uint32_t *ctr, const uint32_t *key, uint32_t *out, int64_t n)
 {
     shaken_ctx *ctx = nullptr;

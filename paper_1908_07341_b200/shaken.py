@@ -56,6 +56,7 @@ SIGNATURES = {
     "shaken_launch_count": (C.c_int64, [_p]),
     "shaken_set_variant": (C.c_int, [_p, C.c_int]),
     "shaken_adopt_spins": (C.c_int, [_p]),
+    "shaken_test_band_hook": (C.c_int, [_p, C.c_int, C.c_uint32]),
     "shaken_moments": (C.c_int, [_p, C.c_int64, C.c_int64, C.c_int64, C.POINTER(C.c_double)]),
     "shaken_selftest_philox_rate": (C.c_int, [C.c_int32, C.c_int32, C.c_int32, C.POINTER(C.c_double)]),
     "shaken_last_error": (C.c_char_p, [_p]),
@@ -292,6 +293,9 @@ class Shaken:
         out = np.zeros((self.n_chains, e.size, 2), dtype=np.int64)
         self._ck(self._lib.shaken_diag_correlations(self._h, e.ctypes.data, e.size, out.ctypes.data))
         return out
+
+    def test_band_hook(self, what: int, value: int):
+        self._ck(self._lib.shaken_test_band_hook(self._h, int(what), int(value)))
 
     def adopt_spins(self):
         """Declare that the bound device buffers already hold valid spins (shaken_adopt_spins)."""

@@ -80,6 +80,62 @@ def test_alternate_batch_of_mid_size_chains_runs_in_the_one_cta_per_chain_path()
             assert np.array_equal(s.observables(), o.observables()), variant
 
 
+@pytest.mark.parametrize("L,n_chains", [(144, 1), (272, 3), (528, 1), (1024, 1), (2048, 1), (1024, 4)])
+def test_alternate_band_path_one_launch_per_run_matches_oracle(L, n_chains):
+    """128 < L <= 2048 with few chains: the whole shaken_run_alternate call is ONE cooperative launch (alt_band_i8: row
+    bands in shared memory, two halo rows per side, one hand-over per full step).  Per-chain couplings, records on some
+    steps only, the run split in the middle of a recording interval; the same run through the per-half-step kernels
+    (variant 3) must give the same bits."""
+    seed, steps = 500 + L, 9
+    J = np.linspace(0.25, 0.6, n_chains)
+    o = so.Oracle(L, n_chains, seed)
+    o.init(0)
+    o.run_alternate(J, steps, 2)
+    for variant in (0, 3):
+        with shaken.Shaken(L, n_chains, seed, max_records=steps) as s:
+            s.set_variant(variant)
+            s.init(0)
+            l0 = s.launch_count
+            s.run_alternate(J, 5, 2)
+            s.run_alternate(J, steps - 5, 2)
+            if variant == 0:
+                assert s.launch_count - l0 == 2, "one cooperative launch per run call expected"
+            assert s.step == o.step
+            assert np.array_equal(s.get_spins(0), o.get_spins(0)), f"sigma differs, variant {variant}"
+            assert np.array_equal(s.observables(), o.observables()), f"records differ, variant {variant}"
+
+
+@pytest.mark.parametrize("alternate", [False, True])
+def test_band_path_stamp_wrap_and_refused_cooperative_launch(alternate):
+    """Two corners of the one-launch band path, through the test hook: (i) the 32-bit stamp counter of the hand-over
+    buffer about to wrap -- the buffer is cleared and the stamps restart; (ii) a refused cooperative launch -- the same
+    call falls back to the per-half-step kernels.  Both in the middle of a run, results unchanged."""
+    L, seed = 528, 61
+    o = so.Oracle(L, 1, seed)
+    o.init(0)
+    if alternate:
+        o.run_alternate(0.44, 12, 3)
+    else:
+        o.run(0.5, 0.7, 12, 3)
+    with shaken.Shaken(L, 1, seed, max_records=8) as s:
+        run = (lambda n: s.run_alternate(0.44, n, 3)) if alternate else (lambda n: s.run(0.5, 0.7, n, 3))
+        s.init(0)
+        l0 = s.launch_count
+        run(4)                                          # band kernel, stamps 1 .. 4
+        assert s.launch_count - l0 == 1
+        s.test_band_hook(0, 2**32 - 4)                  # the next launch would need stamps beyond 2^32 - 1
+        run(3)
+        assert s.launch_count - l0 == 2
+        s.test_band_hook(1, 1)                          # refuse the next cooperative launch
+        l1 = s.launch_count
+        run(2)
+        assert s.launch_count - l1 >= 4, "per-half-step kernels expected after the refusal"
+        run(3)                                          # band kernel again
+        assert s.step == o.step
+        assert np.array_equal(s.get_spins(0), o.get_spins(0)) and np.array_equal(s.get_spins(1), o.get_spins(1))
+        assert np.array_equal(s.observables(), o.observables())
+
+
 def test_alternate_grid_of_couplings_resume_and_chain_offset():
     L, n_chains, seed = 80, 5, 41
     J = np.array([0.1, 0.3, 0.44, 0.6, 0.9])
