@@ -45,6 +45,8 @@ __global__ void __launch_bounds__(I8_THREADS, 1) half_step_i8(const __grid_const
     constexpr bool OBS = (FLAGS & F_OBS) != 0;
     constexpr bool BONDS = (FLAGS & F_BONDS) != 0;
     constexpr bool UPDATE = (FLAGS & F_NOUPDATE) == 0;
+    constexpr bool COAL = (FLAGS & F_COAL) != 0;            // compare the sigma read here with the group's first chain
+    static_assert(!(COAL && HALF == 1), "the coalescence test rides on half-step 0 (which reads sigma)");
     // carry the round-0 Philox product by additions (philox.cuh): measured +1.6 % on launches with sums (their IDP.4A load
     // the multiplier pipe further), -0.6 % on plain ones, so only the former do it
     constexpr bool PRODUCT = (FLAGS & (F_OBS | F_BONDS)) != 0;
@@ -90,6 +92,7 @@ __global__ void __launch_bounds__(I8_THREADS, 1) half_step_i8(const __grid_const
 
     let_next_kernel_launch();
     wait_for_previous_kernel();
+    if (HALF == 1) finalize_coalescence(p);
     const long long task0 = PERWARP ? (long long)blockIdx.x * WPB + warp : (long long)blockIdx.x;
     const long long task_step = PERWARP ? (long long)gridDim.x * WPB : (long long)gridDim.x;
     for (long long bt = task0; bt < p.ntasks; bt += task_step) {
@@ -168,6 +171,11 @@ __global__ void __launch_bounds__(I8_THREADS, 1) half_step_i8(const __grid_const
             const uint32_t pstep_hi = (uint32_t)((unsigned long long)pstep >> 32), pstep_lo = (uint32_t)pstep;
             uint32_t *const my_idx = &s_idx[0][EXTRACT == EXTRACT_SMEM ? threadIdx.x : 0];
             const uint32_t lane8 = (uint32_t)lane * 8u;
+            // coalescence test: members other than the first of a group that has not coalesced yet
+            const int member = COAL ? chain % p.group : 0;
+            const bool cmp = COAL && member != 0 && p.coal[chain / p.group] < 0;
+            const ptrdiff_t to_first = -(ptrdiff_t)member * (ptrdiff_t)plane - (ptrdiff_t)2 * stride;   // pc runs two rows ahead
+            uint32_t differs = 0;
 
 
             // one row: cq = this row, vq = vertical neighbour row, e = edge word; loads the next row into (nq, en)
@@ -176,6 +184,8 @@ __global__ void __launch_bounds__(I8_THREADS, 1) half_step_i8(const __grid_const
                     nq = ldg128(pc);                                  // pc, pe run AHEAD rows in front of the row in use
                     en = ldg32(pe);
                 }
+                uint4 first = cq;
+                if (COAL && cmp) first = ldg128(pc + to_first);       // the same vector of the group's first chain
                 const uint32_t w[4] = {cq.x, cq.y, cq.z, cq.w};
                 const uint32_t vw[4] = {vq.x, vq.y, vq.z, vq.w};
                 uint32_t hw[4], zw[4], ow[4];
@@ -244,6 +254,7 @@ __global__ void __launch_bounds__(I8_THREADS, 1) half_step_i8(const __grid_const
                     }
                 }
                 if (UPDATE) *reinterpret_cast<uint4 *>(pd) = make_uint4(ow[0], ow[1], ow[2], ow[3]);
+                if (COAL) differs |= (first.x ^ cq.x) | (first.y ^ cq.y) | (first.z ^ cq.z) | (first.w ^ cq.w);
                 pc += stride; pe += stride; pd += stride;
                 if constexpr (PRODUCT) add64(ph, pl, pstep_hi, pstep_lo);
                 else n += nstep;
@@ -262,6 +273,7 @@ __global__ void __launch_bounds__(I8_THREADS, 1) half_step_i8(const __grid_const
                 do_row(B3, B2, e3, B1, e1, i + 2 < rows); if (++i == rows) break;
                 do_row(B0, B3, e0, B2, e2, i + 2 < rows); if (++i == rows) break;
             }
+            if (COAL && differs != 0) p.diff[chain / p.group] = p.cstamp;   // every writer stores the same value
         }
     }
     if ((OBS || BONDS) && cur_chain >= 0) flush(cur_chain);

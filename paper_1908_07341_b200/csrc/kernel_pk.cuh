@@ -34,6 +34,7 @@ __global__ void __launch_bounds__(PK_THREADS, 1) half_step_pk(const __grid_const
     constexpr bool OBS = (FLAGS & F_OBS) != 0;
     constexpr bool BONDS = (FLAGS & F_BONDS) != 0;
     constexpr bool UPDATE = (FLAGS & F_NOUPDATE) == 0;
+    constexpr bool COAL = (FLAGS & F_COAL) != 0;            // compare the sigma read here with the group's first chain
     constexpr int WPB = PK_THREADS / 32;
     static_assert(!(BONDS && HALF == 1), "bond sums ride on half-step 0");
 
@@ -73,6 +74,7 @@ __global__ void __launch_bounds__(PK_THREADS, 1) half_step_pk(const __grid_const
 
     let_next_kernel_launch();
     wait_for_previous_kernel();
+    if (HALF == 1) finalize_coalescence(p);
     for (long long bt = blockIdx.x; bt < p.ntasks; bt += gridDim.x) {
         const int chain = (int)(bt / bpc);
         const int lt = (int)(bt % bpc) * WPB + warp;
@@ -125,6 +127,11 @@ __global__ void __launch_bounds__(PK_THREADS, 1) half_step_pk(const __grid_const
             uint32_t Yv[8];
             if (UPDATE) spread2(V, Yv);
             int a0 = 0, a1 = 0, a2 = 0;     // popcount partials of this task
+            // coalescence test: members other than the first of a group that has not coalesced yet
+            const int member = COAL ? chain % p.group : 0;
+            const bool cmp = COAL && member != 0 && p.coal[chain / p.group] < 0;
+            const ptrdiff_t to_first = -(ptrdiff_t)member * (ptrdiff_t)plane;
+            uint32_t differs = 0;
 
             for (int i = 0; i < rows; ++i) {
                 if (i + 2 < rows) {
@@ -132,6 +139,7 @@ __global__ void __launch_bounds__(PK_THREADS, 1) half_step_pk(const __grid_const
                     E2 = __ldg(pe + 2 * stride);
                 }
                 const uint32_t S = S0, e = E0;
+                if (COAL && cmp) differs |= S ^ __ldg(pc + to_first);   // the same word of the group's first chain
                 // horizontal neighbour plane: left (half 0) or right (half 1)
                 const uint32_t Hp = HALF == 0 ? ((S << 1) | (e >> 31)) : ((S >> 1) | (e << 31));
                 uint32_t out = 0;
@@ -189,6 +197,7 @@ __global__ void __launch_bounds__(PK_THREADS, 1) half_step_pk(const __grid_const
                 pc += stride; pe += stride; pd += stride;
                 add64(ph, pl, pstep_hi, pstep_lo);
             }
+            if (COAL && differs != 0) p.diff[chain / p.group] = p.cstamp;   // every writer stores the same value
             if (OBS || BONDS) {
                 const int ns = rows * 32;
                 if (HALF == 1) {

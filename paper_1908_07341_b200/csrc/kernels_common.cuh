@@ -22,7 +22,7 @@ namespace shaken {
 constexpr int I8_THREADS = 512;         // int8 half-step: one 512-thread block per SM, up to 128 registers per thread
 constexpr int MAX_ROWS_PER_TASK = 4096;   // int32 observable partials: 2 * 512 * rows per warp stay far below 2^31
 
-enum : int { F_OBS = 1, F_BONDS = 2, F_NOUPDATE = 4 };
+enum : int { F_OBS = 1, F_BONDS = 2, F_NOUPDATE = 4, F_COAL = 8 };
 
 struct StepParams {
     const void *src;        // sublattice that is read   (half 0: sigma, half 1: tau)
@@ -41,8 +41,28 @@ struct StepParams {
     uint32_t utab[8];       // one table for all chains (kernel parameters live in constant memory)
     long long *rec_cur;     // [n_chains][6] record of the step being computed (F_OBS) or nullptr
     long long *rec_prev;    // [n_chains][6] record whose C_x, C_y are still owed (F_BONDS) or nullptr
+    // coupled chains (group > 1), PAPER.md:234 T = min{n : X_n = Y_n}: half-step 0 launches with F_COAL compare the sigma
+    // they read (the state after `cstamp` full steps) of every member with the group's first chain and stamp diff[group]
+    // with cstamp where they differ; the half-step 1 launch that follows (do_fin, fin_stamp) turns "no difference stamped"
+    // into the coalescence time (do_fin).  coal: [n_groups] times, -1 = not yet; diff: [n_groups] stamps.
+    long long *coal;
+    unsigned long long *diff;
+    unsigned long long cstamp;
+    unsigned long long fin_stamp;
+    int do_fin;
     StepKeys keys;
 };
+
+// coalescence bookkeeping at the start of a half-step 1 launch (block 0 only; the half-step 0 launch that stamped the
+// differences has completed: wait_for_previous_kernel)
+__device__ __forceinline__ void finalize_coalescence(const StepParams &p)
+{
+    if (p.do_fin && blockIdx.x == 0) {
+        const long long ng = p.n_chains / p.group;
+        for (long long gi = threadIdx.x; gi < ng; gi += blockDim.x)
+            if (p.coal[gi] < 0 && p.diff[gi] != p.fin_stamp) p.coal[gi] = (long long)p.fin_stamp;
+    }
+}
 
 // counter word 1 of a chain: its own global index, or that of the first chain of its coupling group
 __device__ __forceinline__ uint32_t rng_chain(const StepParams &p, int chain) { return p.chain0 + (uint32_t)((chain / p.group) * p.group); }

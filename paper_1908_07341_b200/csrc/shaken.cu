@@ -681,6 +681,28 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
     const size_t rec_stride = (size_t)ctx->n_chains * SHAKEN_N_OBS;
 
     ctx->have_tau = true;           // half-step 0 redraws every tau from sigma alone
+    // coupled chains: the comparison of a step's sigma rides on the NEXT half-step 0 (which reads exactly that sigma), the
+    // bookkeeping on the half-step 1 after it; the last step of the call is closed by a read-only pass
+    const bool coupled = ctx->group > 1;
+    const long long ng = coupled ? ctx->n_chains / ctx->group : 0;
+    p.coal = coupled ? ctx->d_coal : nullptr;
+    p.diff = coupled ? reinterpret_cast<unsigned long long *>(ctx->d_coal + ng) : nullptr;
+    bool cmp_due = false;           // sigma has changed since it was last compared
+    auto half0 = [&](int flags) -> cudaError_t {
+        switch (flags) {
+            case 0: return launch_half<0, 0>(ctx, p, grid);
+            case F_OBS: return launch_half<0, F_OBS>(ctx, p, grid);
+            case F_BONDS: return launch_half<0, F_BONDS>(ctx, p, grid);
+            case F_OBS | F_BONDS: return launch_half<0, F_OBS | F_BONDS>(ctx, p, grid);
+            case F_COAL: return launch_half<0, F_COAL>(ctx, p, grid);
+            case F_COAL | F_OBS: return launch_half<0, F_COAL | F_OBS>(ctx, p, grid);
+            case F_COAL | F_BONDS: return launch_half<0, F_COAL | F_BONDS>(ctx, p, grid);
+            case F_COAL | F_OBS | F_BONDS: return launch_half<0, F_COAL | F_OBS | F_BONDS>(ctx, p, grid);
+            case F_NOUPDATE | F_BONDS: return launch_half<0, F_NOUPDATE | F_BONDS>(ctx, p, grid);
+            case F_NOUPDATE | F_COAL: return launch_half<0, F_NOUPDATE | F_COAL>(ctx, p, grid);
+            default: return launch_half<0, F_NOUPDATE | F_COAL | F_BONDS>(ctx, p, grid);
+        }
+    };
     long long *pending = nullptr;   // record that still lacks C_x, C_y
     for (int64_t s = 0; s < n_steps; ++s) {
         const uint64_t t = ctx->step;
@@ -692,47 +714,46 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
         p.dst = ctx->d_tau;
         p.rec_cur = cur;
         p.rec_prev = pending;
+        p.cstamp = p.fin_stamp = (unsigned long long)t;             // sigma as it stands is the state after t steps
+        p.do_fin = 0;
         make_step_keys(ctx->seed, 2 * t, p.keys);
-        if (rec && pending) e = launch_half<0, F_OBS | F_BONDS>(ctx, p, grid);
-        else if (rec) e = launch_half<0, F_OBS>(ctx, p, grid);
-        else if (pending) e = launch_half<0, F_BONDS>(ctx, p, grid);
-        else e = launch_half<0, 0>(ctx, p, grid);
+        e = half0((rec ? F_OBS : 0) | (pending ? F_BONDS : 0) | (cmp_due ? F_COAL : 0));
         if (e != cudaSuccess) return fail(ctx, SHAKEN_ECUDA, "half-step 0 launch: %s", cudaGetErrorString(e));
         pending = nullptr;
         // half-step 1: sigma <- tau  (eq. 16)
         p.src = ctx->d_tau;
         p.dst = ctx->d_sigma;
         p.rec_prev = nullptr;
+        p.do_fin = cmp_due ? 1 : 0;
         make_step_keys(ctx->seed, 2 * t + 1, p.keys);
         if (rec) e = launch_half<1, F_OBS>(ctx, p, grid);
         else e = launch_half<1, 0>(ctx, p, grid);
         if (e != cudaSuccess) return fail(ctx, SHAKEN_ECUDA, "half-step 1 launch: %s", cudaGetErrorString(e));
         ctx->launches += 2;
         ctx->step = t + 1;
-        if (ctx->group > 1) {
-            // sigma of every member against the first chain of its group, after every full step
-            const long long ng = ctx->n_chains / ctx->group;
-            const long long vpc = (long long)(shaken_spin_bytes(ctx) / 16) / ctx->n_chains;
-            unsigned long long *diff = reinterpret_cast<unsigned long long *>(ctx->d_coal + ng);
-            coalesce_compare<<<grid_for(ctx, ng * (ctx->group - 1) * vpc), 256, 0, ctx->stream>>>((const uint4 *)ctx->d_sigma, vpc, ctx->group, ng, ctx->d_coal, diff, (unsigned long long)ctx->step);
-            coalesce_finalize<<<grid_for(ctx, ng), 256, 0, ctx->stream>>>(ctx->d_coal, diff, ng, (unsigned long long)ctx->step);
-            CU(cudaGetLastError());
-            ctx->launches += 2;
-        }
+        cmp_due = coupled;
         if (rec) {
             pending = cur;
             ctx->n_rec++;
         }
     }
-    if (pending) {
-        // the last step was recorded: its sigma-layer bond sums are taken by a read-only pass over sigma
+    if (pending || cmp_due) {
+        // the last step: its sigma-layer bond sums (if it was recorded) and its comparison (coupled chains) are taken by
+        // a read-only pass over sigma
         p.src = ctx->d_sigma;
         p.dst = nullptr;
         p.rec_cur = nullptr;
         p.rec_prev = pending;
-        cudaError_t e = launch_half<0, F_BONDS | F_NOUPDATE>(ctx, p, grid);
-        if (e != cudaSuccess) return fail(ctx, SHAKEN_ECUDA, "bond-sum launch: %s", cudaGetErrorString(e));
+        p.cstamp = p.fin_stamp = (unsigned long long)ctx->step;
+        p.do_fin = 0;
+        cudaError_t e = half0(F_NOUPDATE | (pending ? F_BONDS : 0) | (cmp_due ? F_COAL : 0));
+        if (e != cudaSuccess) return fail(ctx, SHAKEN_ECUDA, "closing read-only launch: %s", cudaGetErrorString(e));
         ctx->launches++;
+        if (cmp_due) {
+            coalesce_finalize<<<grid_for(ctx, ng), 256, 0, ctx->stream>>>(ctx->d_coal, p.diff, ng, (unsigned long long)ctx->step);
+            CU(cudaGetLastError());
+            ctx->launches++;
+        }
     }
     return SHAKEN_OK;
 }
