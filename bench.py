@@ -55,6 +55,9 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-workloads", action="store_true", help="skip the short legs on the other four BASELINE.json workloads")
+    ap.add_argument("--slabs", action="store_true",
+                    help="N ranks share ONE lattice of the named single-chain int8 workload as row slabs (strong scaling; one sigma "
+                         "row each way per step by peer stores, DESIGN.md section 9) instead of running N replicas")
     ap.add_argument("--variant", type=int, default=0, choices=[0, 3, 8], help="code-path switch of shaken_set_variant (0 = automatic)")
     ap.add_argument("--cpu-multicore-leg", action="store_true", help=argparse.SUPPRESS)
     ap.add_argument("--dynamics", default="shaken", choices=["shaken", "alternate"],
@@ -270,8 +273,33 @@ def muls_per_site(w, alt):
     return (17.0 / w.obs_every + 18.0 * (1.0 - 1.0 / w.obs_every)) / 4.0
 
 
-def time_workload(shaken, torch, dist, w, K, W, dev, stream, rank, world, alt, variant=0, before_timed=None):
+def time_workload(shaken, torch, dist, w, K, W, dev, stream, rank, world, alt, variant=0, before_timed=None, slabs=False):
     """W warm-up steps, then K steps timed with CUDA events on the library's stream.  Returns (context, ms, launches, run)."""
+    if slabs:
+        from paper_1908_07341_b200 import parallel
+
+        s = parallel.open_slab(w.L, w.seed, world, rank, max_records=(K + W) // max(w.obs_every, 1) + 4 if w.obs_every else 0, stream=stream)
+        parallel.connect_slabs_ipc(s)
+
+        def run(n):
+            s.run(w.J[0], w.q[0], n, w.obs_every)
+
+        s.init(w.init)
+        run(W)
+        s.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+        if before_timed:
+            before_timed()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        l0 = s.launch_count
+        e0.record(stream)
+        run(K)
+        e1.record(stream)
+        e1.synchronize()
+        torch.cuda.synchronize(dev)
+        return s, e0.elapsed_time(e1), s.launch_count - l0, run
     s = shaken.Shaken(w.L, w.n_chains, w.seed, packed=w.packed, max_records=(K + W) // max(w.obs_every, 1) + 4 if w.obs_every else 1,
                       device=str(dev), stream=stream)
     s.set_chain_offset(rank * w.n_chains)
@@ -306,10 +334,10 @@ def time_workload(shaken, torch, dist, w, K, W, dev, stream, rank, world, alt, v
     return s, e0.elapsed_time(e1), s.launch_count - l0, run
 
 
-def rooflines(w, alt, ms, K, n_sms, sm_max_mhz, hbm_peak, philox_only):
+def rooflines(w, alt, ms, K, n_sms, sm_max_mhz, hbm_peak, philox_only, share=1.0):
     """HBM view (the metric's denominator), integer-multiplier view and the measured Philox-only ceiling of one workload."""
     bytes_per_update = 0.25 if w.packed else 2.0
-    sites_per_launch = w.n_chains * w.L * w.L
+    sites_per_launch = int(w.n_chains * w.L * w.L * share)   # share < 1: this rank's slab of a shared lattice
     if alt:
         bytes_per_update *= 2.0                            # in place on one array: read + write the array to redraw half of it
         sites_per_launch //= 2
@@ -351,29 +379,39 @@ def run_ours(args):
     uniform = len(set(w.J)) == 1 and len(set(w.q)) == 1
 
     sampler = ClockSampler(local_rank)
+    slabs = bool(args.slabs)
+    if slabs and (alt or w.packed or w.n_chains != 1):
+        raise SystemExit("bench.py --slabs: needs a single-chain int8 workload of the shaken dynamics (cfg4, cfg2, paper<L>)")
     s, ms, launches, run = time_workload(shaken, torch, dist, w, K, W, dev, stream, rank, world, alt, args.variant,
-                                         before_timed=sampler.start if rank == 0 else None)
-    if rank == 0:
-        # nvidia-smi needs ~50 ms per sample: keep the same launch sequence running right after the timed region
-        # until at least 1.5 s of load has been sampled (records are discarded; obs cadence unchanged)
-        t_end = time.perf_counter() + max(1.5 - ms * 1e-3, 0.0)
-        while time.perf_counter() < t_end:
-            s.clear_records()
-            run(K)
-            s.synchronize()
-        sampler.stop()
+                                         before_timed=sampler.start if rank == 0 else None, slabs=slabs)
     if world > 1:
         t = torch.tensor([ms], device=dev, dtype=torch.float64)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         ms = float(t.item())
+    # nvidia-smi needs ~50 ms per sample: keep the same launch sequence running right after the timed region until at
+    # least 1.5 s of load has been sampled (records are discarded; obs cadence unchanged).  Slabs of one lattice wait for
+    # each other, so there every rank repeats the run the same number of times; replicas are independent (rank 0 only).
+    reps = int(max(1.5 - ms * 1e-3, 0.0) / max(ms * 1e-3, 1e-6)) + 1
+    if rank == 0 or (slabs and world > 1):
+        for _ in range(reps):
+            s.clear_records()
+            run(K)
+            s.synchronize()
+    if rank == 0:
+        sampler.stop()
+    if world > 1:
         dist.barrier()
 
     updates_per_rank = (1.0 if alt else 2.0) * n_local * w.L * w.L * K   # alternate: a half-step redraws one colour
+    if slabs:
+        updates_per_rank /= world                          # strong scaling: the ranks share one lattice
     value = world * updates_per_rank / (ms * 1e6)
 
     # ------------------------------------------------------------------ e2e through the C ABI with host buffers
     e2e = None
-    if not args.no_e2e:
+    if not args.no_e2e and slabs:
+        e2e = {"unavailable": "the e2e leg is measured on the replica arm (a slab holds a part of the lattice)"}
+    elif not args.no_e2e:
         nsp = n_local * w.L * w.L
         h_sigma = torch.empty(nsp, dtype=torch.int8).pin_memory()
         h_out = torch.empty(nsp, dtype=torch.int8).pin_memory()
@@ -427,7 +465,7 @@ def run_ours(args):
     except Exception as e:                                 # the hook must never cost the bench line
         philox_only = None
         print("bench.py: philox-only hook failed: %r" % (e,), file=sys.stderr)
-    rl = rooflines(w, alt, ms, K, props.multi_processor_count, sm_max_mhz, hbm_peak, philox_only)
+    rl = rooflines(w, alt, ms, K, props.multi_processor_count, sm_max_mhz, hbm_peak, philox_only, 1.0 / world if slabs else 1.0)
     traffic, traffic_source = None, None
     tpath = os.path.join(ROOT, "profiles", "traffic.txt")
     if os.path.exists(tpath):
@@ -457,13 +495,14 @@ def run_ours(args):
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
-        "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "ms_per_step": ms / K, "higher_is_better": True, "scaling": "strong" if slabs else "weak", "vs_baseline": None,
         "dtype": "u32 bit-packed" if w.packed else "int8", "data": "synthetic",
         "config": {"workload": w.name, "dynamics": args.dynamics, "L": w.L, "n_chains_per_gpu": n_local, "J": w.J[0] if uniform else "grid",
                    "q": (w.q[0] if uniform else "grid") if not alt else None, "obs_every": w.obs_every, "init": w.init, "seed": w.seed,
                    "l2": "inputs larger than L2 (2 x %.0f MB per step)" % (shaken_bytes(w) / 1e6) if shaken_bytes(w) > 126e6
                          else "working set fits L2 (launch/latency-bound regime)",
-                   "parallelism": "replicas (independent chains, no collective)" if world > 1 else "single GPU"},
+                   "parallelism": ("row slabs of one lattice, one sigma row each way per step by peer stores" if slabs else
+                                   "replicas (independent chains, no collective)") if world > 1 or slabs else "single GPU"},
         "clocks": sampler.summary(),
         "e2e": e2e,
         "gpu_launches": int(launches),

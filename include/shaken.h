@@ -223,6 +223,42 @@ int64_t shaken_coalescence(shaken_ctx *ctx, int64_t *out, int64_t max_groups);
  */
 int shaken_diag_correlations(shaken_ctx *ctx, const int32_t *ells, int32_t n_ell, int64_t *out);
 
+/*
+ * Row-slab sharding of ONE lattice over several contexts / GPUs (second bullet).  The fields of eq. (14)
+ * reach one row across a slab edge per half-step; because a site's random word is a function of the
+ * GLOBAL site index, a slab redraws the tau row above itself redundantly and the slabs exchange only sigma rows, once per
+ * full step, by stores into the neighbours' "inbox" (peer memory over NVLink) -- results are bit-identical to the unsplit
+ * lattice for any partition.  int8 layout, one chain.
+ *
+ * shaken_create_slab: context for rows [row0, row0 + n_rows) of an L x L torus (n_rows >= 2; L as for shaken_create).
+ *   The context owns its device buffers (shaken_bind is not available; shaken_set_stream chooses the stream).
+ *   shaken_spin_bytes = n_rows * L; shaken_get_spins / shaken_set_spins move the slab's rows [n_rows][L];
+ *   shaken_init as usual (iid: the init-stream words of the slab's global sites).  Records hold the sums over the slab's
+ *   own sites and bonds (E_J, C_y: the bonds to the rows above / below the slab counted once, by the lower / upper slab's
+ *   partner as on the torus); the caller adds the records of all slabs.  The C_x, C_y of the LAST record of a run need
+ *   the neighbour's new row: they are completed by the next shaken_run or by shaken_observables (both wait for it).
+ *   shaken_run_grid works with its single chain; shaken_run_alternate, coupling and shaken_diag_correlations return
+ *   SHAKEN_ESTATE.
+ * shaken_slab_inbox: DEVICE pointer and size of this context's inbox ([2 sides][2 parities][L/4] {word, stamp} pairs),
+ *   for the neighbours to store into.
+ * shaken_slab_connect: the inboxes of the rank below (owner of row row0 - 1) and above (owner of row row0 + n_rows),
+ *   DEVICE pointers valid on this device (the same process: any peer-enabled allocation; for a single slab both are
+ *   its own inbox).  shaken_slab_ipc_export / shaken_slab_ipc_connect do the same across processes with CUDA IPC
+ *   handles (64 bytes each, HOST memory; exchange them with any host-side transport, e.g. torch.distributed).
+ * shaken_slab_exchange: publish the slab's current edge rows now if they have not been (shaken_run does it itself; an
+ *   explicit call lets a driver that advances several slabs ONE AFTER THE OTHER on one device publish all of them before
+ *   any of them waits).  Every rank must make the same sequence of run / exchange calls: exchanges are counted.
+ * shaken_run on a slab: per step one hand-over (publish, wait for the neighbours' rows, redraw tau row n_rows) and the two
+ *   half-step launches of the strip kernels.  SHAKEN_ESTATE if not connected.
+ */
+int shaken_create_slab(shaken_ctx **out, int32_t L, int32_t row0, int32_t n_rows, uint64_t seed);
+int shaken_set_stream(shaken_ctx *ctx, void *cuda_stream);
+int shaken_slab_inbox(shaken_ctx *ctx, void **d_inbox, size_t *bytes);
+int shaken_slab_connect(shaken_ctx *ctx, void *d_inbox_below, void *d_inbox_above);
+int shaken_slab_ipc_export(shaken_ctx *ctx, void *handle64);
+int shaken_slab_ipc_connect(shaken_ctx *ctx, const void *below_handle64, const void *above_handle64);
+int shaken_slab_exchange(shaken_ctx *ctx);
+
 /* Wait until everything enqueued by this context has finished. */
 int shaken_synchronize(shaken_ctx *ctx);
 

@@ -65,6 +65,7 @@ __global__ void __launch_bounds__(I8_THREADS, 1) half_step_i8(const __grid_const
     const int L = p.L;
     const int L4 = L >> 2;
     const int R = p.rows_per_task;
+    const int NR = p.slab_rows ? p.slab_rows : L;                   // rows this launch redraws
     const size_t plane = (size_t)L * (size_t)L;
     const int tpc = p.nrb * p.nseg;                                  // warp tasks per chain
     const int bpc = (tpc + WPB - 1) / WPB;                           // block tasks per chain
@@ -146,14 +147,15 @@ __global__ void __launch_bounds__(I8_THREADS, 1) half_step_i8(const __grid_const
         if (lt < tpc && cv < p.nvec) {
             const int c0 = cv * 16;
             const int r_first = rb * R;
-            const int r_last = min(L, r_first + R) - 1;
+            const int r_last = min(NR, r_first + R) - 1;
             const int rows = r_last - r_first + 1;
             const uint8_t *sbase = reinterpret_cast<const uint8_t *>(p.src) + (size_t)chain * plane;
             uint8_t *dbase = reinterpret_cast<uint8_t *>(p.dst) + (size_t)chain * plane;
 
             const int dir = HALF ? -1 : +1;
             int r = HALF ? r_last : r_first;
-            const int rh = HALF ? (r_last + 1 == L ? 0 : r_last + 1) : (r_first == 0 ? L - 1 : r_first - 1);
+            // row of the vertical neighbours of the strip's first row: wraps on a torus, never in a slab (rows -1 and NR exist)
+            const int rh = HALF ? (r_last + 1 == NR && !p.slab_rows ? 0 : r_last + 1) : (r_first == 0 && !p.slab_rows ? L - 1 : r_first - 1);
             const int ce = HALF ? (c0 + 16 == L ? 0 : c0 + 16) : (c0 == 0 ? L - 4 : c0 - 4);
 
             // running pointers (one 64-bit add each per row; no multiplies on the FMA pipe inside the loop)
@@ -163,7 +165,7 @@ __global__ void __launch_bounds__(I8_THREADS, 1) half_step_i8(const __grid_const
             uint8_t *pd = dbase + (size_t)r * L + c0;
             // Philox counter word 0 of the lane's first call in the row is n = r * L/4 + 4 cv; only its product with M0 is
             // needed, and that is carried from call to call and from row to row by 64-bit additions (philox.cuh)
-            uint32_t n = (uint32_t)r * (uint32_t)L4 + (uint32_t)cv * 4u;
+            uint32_t n = ((uint32_t)r + p.row0) * (uint32_t)L4 + (uint32_t)cv * 4u;
             const uint32_t nstep = (uint32_t)(dir * L4);
             uint32_t ph, pl;
             mul_wide(PHILOX_M0, n, ph, pl);
@@ -262,7 +264,7 @@ __global__ void __launch_bounds__(I8_THREADS, 1) half_step_i8(const __grid_const
 
             // four row buffers rotate roles (vertical neighbour / current / two prefetched rows) without register moves:
             // the row loaded while row i is computed is row i + 2
-            uint4 B0 = ldg128(sbase + (size_t)rh * L + c0), B1 = ldg128(pc), B2 = B1, B3 = B1;
+            uint4 B0 = ldg128(sbase + (ptrdiff_t)rh * L + c0), B1 = ldg128(pc), B2 = B1, B3 = B1;
             uint32_t e0 = 0, e1 = ldg32(pe), e2 = 0, e3 = 0;
             pc += stride; pe += stride;
             if (rows > 1) { B2 = ldg128(pc); e2 = ldg32(pe); }

@@ -7,6 +7,7 @@
 #include "kernel_small.cuh"
 #include "kernel_band.cuh"
 #include "kernel_alt.cuh"
+#include "kernel_slab.cuh"
 
 namespace shaken {
 
@@ -16,7 +17,8 @@ namespace shaken {
 
 // iid start: spin = +1 iff init-stream word < 2^31; counter = (site>>2, chain, which, 0xFFFFFFFF).
 // One thread per Philox call (4 sites) per sublattice.  packed: 8 calls per word handled by one thread.
-__global__ void init_iid_i8(uint8_t *sigma, uint8_t *tau, int n_chains, uint32_t chain0, long long calls_per_chain, uint32_t k0, uint32_t k1)
+// n_offset: Philox counter word 0 of the first call (a slab of one lattice starts at row0 * L / 4, a whole torus at 0)
+__global__ void init_iid_i8(uint8_t *sigma, uint8_t *tau, int n_chains, uint32_t chain0, long long calls_per_chain, uint32_t k0, uint32_t k1, uint32_t n_offset)
 {
     const long long total = (long long)n_chains * calls_per_chain;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
@@ -25,7 +27,7 @@ __global__ void init_iid_i8(uint8_t *sigma, uint8_t *tau, int n_chains, uint32_t
 #pragma unroll
         for (int which = 0; which < 2; ++which) {
             uint32_t w[4];
-            philox4x32_10(n, chain, (uint32_t)which, 0xFFFFFFFFu, k0, k1, w);
+            philox4x32_10(n + n_offset, chain, (uint32_t)which, 0xFFFFFFFFu, k0, k1, w);
             uint32_t out = 0;
 #pragma unroll
             for (int b = 0; b < 4; ++b) out |= (w[b] < 0x80000000u ? 0x01u : 0xFFu) << (8 * b);

@@ -37,6 +37,10 @@ struct StepParams {
     int nseg;               // warp-wide strips per row = ceil(nvec / 32)
     int nrb;                // row blocks = ceil(L / rows_per_task)
     long long ntasks;       // n_chains * nrb * nseg
+    int slab_rows;          // 0: a whole L x L torus.  > 0: a SLAB of one lattice (row-slab sharding, kernel_slab.cuh): this
+                            // many rows are redrawn; src / dst point at the slab's row 0 and the arrays hold the rows just
+                            // below (index -1) and above (index slab_rows) as well, so vertical neighbours never wrap
+    uint32_t row0;          // global index of the slab's row 0 (enters the Philox counter); 0 for a whole torus
     const uint32_t *gtab;   // per-chain tables [n_chains][8] in global memory, or nullptr: use utab
     uint32_t utab[8];       // one table for all chains (kernel parameters live in constant memory)
     long long *rec_cur;     // [n_chains][6] record of the step being computed (F_OBS) or nullptr

@@ -55,6 +55,17 @@ struct shaken_ctx {
     long long *d_coal = nullptr;  // [n_chains / group] coalescence times, -1 = not yet; followed by the difference stamps
     bool perwarp = false;         // strip kernels: per-warp task lists for this run (many small chains)
     int64_t launches = 0;
+    // row-slab sharding of one lattice (shaken_create_slab; kernel_slab.cuh)
+    bool slab = false;
+    int n_rows = 0;               // rows of this slab
+    uint32_t row0 = 0;            // global index of its row 0
+    void *d_sigma_alloc = nullptr, *d_tau_alloc = nullptr;   // allocations (sigma: rows -1 .. n_rows, tau: rows 0 .. n_rows)
+    uint2 *d_inbox = nullptr;     // [2 sides][2 parities][L/4] {word, stamp}
+    uint2 *peer_below = nullptr, *peer_above = nullptr;      // the neighbours' inboxes (peer-mapped device pointers)
+    void *ipc_below = nullptr, *ipc_above = nullptr;         // ... when opened from IPC handles (closed on destroy)
+    uint32_t xstamp = 0;          // exchanges done (every rank counts the same)
+    bool published = false;       // the current sigma edge rows are in the neighbours' inboxes
+    long long *slab_pending = nullptr;   // record whose C_x, C_y wait for the neighbour's row (closed lazily)
     char err[512] = {0};
 };
 
@@ -145,7 +156,13 @@ extern "C" int shaken_destroy(shaken_ctx *ctx)
 {
     if (!ctx) return SHAKEN_OK;
     if (ctx->have_sigma || ctx->have_tau || ctx->d_rec || ctx->d_tab) cudaStreamSynchronize(ctx->stream);
-    if (ctx->own_spins) { cudaFree(ctx->d_sigma); cudaFree(ctx->d_tau); }
+    if (ctx->slab) {
+        if (ctx->ipc_below) cudaIpcCloseMemHandle(ctx->ipc_below);
+        if (ctx->ipc_above && ctx->ipc_above != ctx->ipc_below) cudaIpcCloseMemHandle(ctx->ipc_above);
+        cudaFree(ctx->d_sigma_alloc);
+        cudaFree(ctx->d_tau_alloc);
+        cudaFree(ctx->d_inbox);
+    } else if (ctx->own_spins) { cudaFree(ctx->d_sigma); cudaFree(ctx->d_tau); }
     if (ctx->own_rec) cudaFree(ctx->d_rec);
     cudaFree(ctx->d_tab);
     cudaFree(ctx->d_bad);
@@ -159,6 +176,7 @@ extern "C" int shaken_destroy(shaken_ctx *ctx)
 extern "C" size_t shaken_spin_bytes(const shaken_ctx *ctx)
 {
     if (!ctx) return 0;
+    if (ctx->slab) return (size_t)ctx->n_rows * (size_t)ctx->L;
     const size_t n = (size_t)ctx->n_chains * (size_t)ctx->L * (size_t)ctx->L;
     return ctx->packed ? n / 8 : n;
 }
@@ -185,6 +203,24 @@ static int ensure_spins(shaken_ctx *ctx)
     int rc = ensure_device(ctx);
     if (rc) return rc;
     if (ctx->d_sigma && ctx->d_tau) return SHAKEN_OK;
+    if (ctx->slab) {
+        // sigma holds rows -1 .. n_rows, tau rows 0 .. n_rows (the halo rows live in the arrays, kernel_slab.cuh)
+        const size_t row = (size_t)ctx->L, sb = (size_t)(ctx->n_rows + 2) * row, tb = (size_t)(ctx->n_rows + 1) * row;
+        void *a = nullptr, *b = nullptr;
+        if (cudaMalloc(&a, sb) != cudaSuccess || cudaMalloc(&b, tb) != cudaSuccess) {
+            cudaFree(a);
+            cudaGetLastError();
+            return fail(ctx, SHAKEN_ENOMEM, "cudaMalloc of %zu + %zu slab bytes failed", sb, tb);
+        }
+        ctx->d_sigma_alloc = a;
+        ctx->d_tau_alloc = b;
+        ctx->d_sigma = (uint8_t *)a + row;
+        ctx->d_tau = b;
+        ctx->own_spins = true;
+        CU(cudaMemsetAsync(a, 0x01, sb, ctx->stream));
+        CU(cudaMemsetAsync(b, 0x01, tb, ctx->stream));
+        return SHAKEN_OK;
+    }
     const size_t nb = shaken_spin_bytes(ctx);
     void *a = nullptr, *b = nullptr;
     if (cudaMalloc(&a, nb) != cudaSuccess || cudaMalloc(&b, nb) != cudaSuccess) {
@@ -204,6 +240,7 @@ static int ensure_spins(shaken_ctx *ctx)
 extern "C" int shaken_bind(shaken_ctx *ctx, void *d_sigma, void *d_tau, void *d_records, size_t rec_bytes, void *cuda_stream)
 {
     if (!ctx) return fail(nullptr, SHAKEN_EINVAL, "shaken_bind: ctx is NULL");
+    if (ctx->slab) return fail(ctx, SHAKEN_ESTATE, "shaken_bind: a slab context owns its buffers (use shaken_set_stream)");
     if (!d_sigma || !d_tau || ((uintptr_t)d_sigma & 15) || ((uintptr_t)d_tau & 15) || d_sigma == d_tau)
         return fail(ctx, SHAKEN_EINVAL, "shaken_bind: sigma/tau must be distinct, non-NULL, 16-byte aligned device pointers");
     if ((d_records == nullptr) != (rec_bytes == 0) || ((uintptr_t)d_records & 7))
@@ -267,6 +304,7 @@ extern "C" int shaken_clear_records(shaken_ctx *ctx)
     if (ctx->d_rec && ctx->n_rec > 0)
         CU(cudaMemsetAsync(ctx->d_rec, 0, (size_t)ctx->n_rec * shaken_record_bytes(ctx), ctx->stream));
     ctx->n_rec = 0;
+    ctx->slab_pending = nullptr;   // (a slab's last record may still have been waiting for its bond sums)
     return SHAKEN_OK;
 }
 
@@ -365,6 +403,8 @@ extern "C" int64_t shaken_coalescence(shaken_ctx *ctx, int64_t *out, int64_t max
     return n;
 }
 
+static int slab_close_record(shaken_ctx *ctx);
+
 static int grid_for(const shaken_ctx *ctx, long long work_items, int per_thread_items = 1)
 {
     long long blocks = (work_items + (long long)256 * per_thread_items - 1) / ((long long)256 * per_thread_items);
@@ -382,18 +422,21 @@ extern "C" int shaken_init(shaken_ctx *ctx, int mode)
     if (!ctx) return fail(nullptr, SHAKEN_EINVAL, "shaken_init: ctx is NULL");
     if (mode != SHAKEN_INIT_UP && mode != SHAKEN_INIT_DOWN && mode != SHAKEN_INIT_IID && mode != SHAKEN_INIT_SANDWICH)
         return fail(ctx, SHAKEN_EINVAL, "shaken_init: mode %d is not +1, -1, 0 or 2", mode);
+    if (ctx->slab && mode == SHAKEN_INIT_SANDWICH) return fail(ctx, SHAKEN_EINVAL, "shaken_init: a slab context holds one chain");
     int rc = ensure_spins(ctx);
     if (rc) return rc;
     const size_t nb = shaken_spin_bytes(ctx);
+    ctx->published = false;
+    ctx->slab_pending = nullptr;
     if (mode == SHAKEN_INIT_IID) {
         const uint32_t k0 = (uint32_t)ctx->seed, k1 = (uint32_t)(ctx->seed >> 32);
-        const long long sites = (long long)ctx->L * ctx->L;
+        const long long sites = (long long)ctx->L * (ctx->slab ? ctx->n_rows : ctx->L);
         if (ctx->packed) {
             const long long wpc = sites / 32;
             init_iid_pk<<<grid_for(ctx, wpc * ctx->n_chains), 256, 0, ctx->stream>>>((uint32_t *)ctx->d_sigma, (uint32_t *)ctx->d_tau, ctx->n_chains, ctx->chain0, wpc, k0, k1);
         } else {
             const long long cpc = sites / 4;
-            init_iid_i8<<<grid_for(ctx, cpc * ctx->n_chains), 256, 0, ctx->stream>>>((uint8_t *)ctx->d_sigma, (uint8_t *)ctx->d_tau, ctx->n_chains, ctx->chain0, cpc, k0, k1);
+            init_iid_i8<<<grid_for(ctx, cpc * ctx->n_chains), 256, 0, ctx->stream>>>((uint8_t *)ctx->d_sigma, (uint8_t *)ctx->d_tau, ctx->n_chains, ctx->chain0, cpc, k0, k1, ctx->slab ? ctx->row0 * (uint32_t)(ctx->L / 4) : 0u);
         }
         ctx->launches++;
         CU(cudaGetLastError());
@@ -449,6 +492,7 @@ static cudaError_t launch_half(const shaken_ctx *ctx, const StepParams &p, int g
 
 static int choose_rows_per_task(const shaken_ctx *ctx, int nseg, long long grid_cap, int wpb, double *score_out = nullptr)
 {
+    const int NR = ctx->slab ? ctx->n_rows : ctx->L;      // rows a launch redraws
     // Strip height R.  Tall strips amortise the halo row and the unprefetched loads at a strip's start; the persistent
     // grid walks block tasks (8 warp strips of one chain) round-robin, so the last wave should be full and so should
     // the warps of a block task.  Maximise
@@ -456,16 +500,16 @@ static int choose_rows_per_task(const shaken_ctx *ctx, int nseg, long long grid_
     // fill = ntasks / (grid * waves), warp_use = strips per chain / (8 * block tasks per chain), machine = grid / cap.
     int best = 4;
     double best_score = -1.0;
-    const int Rmax = ctx->L < MAX_ROWS_PER_TASK ? ctx->L : MAX_ROWS_PER_TASK;
-    for (int R = Rmax; R >= 4; --R) {
-        const long long nrb = (ctx->L + R - 1) / R;
+    const int Rmax = NR < MAX_ROWS_PER_TASK ? NR : MAX_ROWS_PER_TASK;
+    for (int R = Rmax; R >= (NR < 4 ? 1 : 4); --R) {
+        const long long nrb = (NR + R - 1) / R;
         const long long tpc = nrb * nseg;
         const long long bpc = (tpc + wpb - 1) / wpb;
         const long long ntasks = (long long)ctx->n_chains * bpc;
         const long long grid = ntasks < grid_cap ? ntasks : grid_cap;
         const long long waves = (ntasks + grid - 1) / grid;
         const double fill = (double)ntasks / (double)(grid * waves);
-        const double warp_use = (double)ctx->L / (double)(nrb * R) * (double)tpc / (double)(bpc * wpb);
+        const double warp_use = (double)NR / (double)(nrb * R) * (double)tpc / (double)(bpc * wpb);
         const double machine = (double)grid / (double)grid_cap;
         const double score = fill * warp_use * machine * ((double)R / ((double)R + 3.0));
         if (score > best_score + 1e-9) { best_score = score; best = R; }
@@ -564,6 +608,244 @@ static int try_band_launch(shaken_ctx *ctx, bool alternate, const uint32_t *gtab
     return 1;
 }
 
+// ---------------------------------------------------------------------------------------------------
+// Row-slab sharding of one lattice (second bullet; kernel_slab.cuh)
+// ---------------------------------------------------------------------------------------------------
+extern "C" int shaken_create_slab(shaken_ctx **out, int32_t L, int32_t row0, int32_t n_rows, uint64_t seed)
+{
+    if (!out) return fail(nullptr, SHAKEN_EINVAL, "shaken_create_slab: out is NULL");
+    *out = nullptr;
+    if (L < 16 || L > 65536 || L % 16 != 0) return fail(nullptr, SHAKEN_EINVAL, "shaken_create_slab: L=%d must be a multiple of 16 in [16, 65536]", L);
+    if (row0 < 0 || n_rows < 2 || row0 + n_rows > L)
+        return fail(nullptr, SHAKEN_EINVAL, "shaken_create_slab: rows [%d, %d) must lie in [0, L) and be at least two", row0, row0 + n_rows);
+    shaken_ctx *c = new (std::nothrow) shaken_ctx();
+    if (!c) return fail(nullptr, SHAKEN_ENOMEM, "shaken_create_slab: out of host memory");
+    c->L = L;
+    c->n_chains = 1;
+    c->seed = seed;
+    c->flags = SHAKEN_INT8;
+    c->slab = true;
+    c->row0 = (uint32_t)row0;
+    c->n_rows = n_rows;
+    *out = c;
+    return SHAKEN_OK;
+}
+
+extern "C" int shaken_set_stream(shaken_ctx *ctx, void *cuda_stream)
+{
+    if (!ctx) return fail(nullptr, SHAKEN_EINVAL, "shaken_set_stream: ctx is NULL");
+    if (ctx->d_sigma || ctx->d_rec) CU(cudaStreamSynchronize(ctx->stream));
+    ctx->stream = (cudaStream_t)cuda_stream;
+    return SHAKEN_OK;
+}
+
+static int slab_ensure_inbox(shaken_ctx *ctx)
+{
+    if (ctx->d_inbox) return SHAKEN_OK;
+    const size_t bytes = (size_t)4 * (ctx->L / 4) * sizeof(uint2);
+    if (cudaMalloc(&ctx->d_inbox, bytes) != cudaSuccess) {
+        cudaGetLastError();
+        return fail(ctx, SHAKEN_ENOMEM, "cudaMalloc of the slab inbox failed");
+    }
+    CU(cudaMemset(ctx->d_inbox, 0, bytes));            // stamp 0 is never used by an exchange
+    return SHAKEN_OK;
+}
+
+extern "C" int shaken_slab_inbox(shaken_ctx *ctx, void **d_inbox, size_t *bytes)
+{
+    if (!ctx || !ctx->slab || !d_inbox) return fail(ctx, SHAKEN_EINVAL, "shaken_slab_inbox: not a slab context or NULL argument");
+    int rc = slab_ensure_inbox(ctx);
+    if (rc) return rc;
+    *d_inbox = ctx->d_inbox;
+    if (bytes) *bytes = (size_t)4 * (ctx->L / 4) * sizeof(uint2);
+    return SHAKEN_OK;
+}
+
+extern "C" int shaken_slab_connect(shaken_ctx *ctx, void *d_inbox_below, void *d_inbox_above)
+{
+    if (!ctx || !ctx->slab || !d_inbox_below || !d_inbox_above) return fail(ctx, SHAKEN_EINVAL, "shaken_slab_connect: not a slab context or NULL argument");
+    int rc = slab_ensure_inbox(ctx);
+    if (rc) return rc;
+    ctx->peer_below = (uint2 *)d_inbox_below;
+    ctx->peer_above = (uint2 *)d_inbox_above;
+    ctx->published = false;
+    return SHAKEN_OK;
+}
+
+extern "C" int shaken_slab_ipc_export(shaken_ctx *ctx, void *handle64)
+{
+    if (!ctx || !ctx->slab || !handle64) return fail(ctx, SHAKEN_EINVAL, "shaken_slab_ipc_export: not a slab context or NULL argument");
+    static_assert(sizeof(cudaIpcMemHandle_t) == 64, "IPC handle size");
+    int rc = slab_ensure_inbox(ctx);
+    if (rc) return rc;
+    cudaIpcMemHandle_t h;
+    CU(cudaIpcGetMemHandle(&h, ctx->d_inbox));
+    memcpy(handle64, &h, 64);
+    return SHAKEN_OK;
+}
+
+extern "C" int shaken_slab_ipc_connect(shaken_ctx *ctx, const void *below_handle64, const void *above_handle64)
+{
+    if (!ctx || !ctx->slab || !below_handle64 || !above_handle64) return fail(ctx, SHAKEN_EINVAL, "shaken_slab_ipc_connect: not a slab context or NULL argument");
+    cudaIpcMemHandle_t hb, ha;
+    memcpy(&hb, below_handle64, 64);
+    memcpy(&ha, above_handle64, 64);
+    void *pb = nullptr, *pa = nullptr;
+    CU(cudaIpcOpenMemHandle(&pb, hb, cudaIpcMemLazyEnablePeerAccess));
+    if (memcmp(&hb, &ha, 64) == 0) pa = pb;             // two ranks: the same neighbour on both sides
+    else CU(cudaIpcOpenMemHandle(&pa, ha, cudaIpcMemLazyEnablePeerAccess));
+    ctx->ipc_below = pb;
+    ctx->ipc_above = pa;
+    return shaken_slab_connect(ctx, pb, pa);
+}
+
+static void slab_params(shaken_ctx *ctx, SlabParams &sp, double J, double q, uint64_t t)
+{
+    memset(&sp, 0, sizeof(sp));
+    sp.sigma = (uint8_t *)ctx->d_sigma;
+    sp.tau = (uint8_t *)ctx->d_tau;
+    sp.L = ctx->L;
+    sp.n_rows = ctx->n_rows;
+    sp.row0 = ctx->row0;
+    sp.chain = ctx->chain0;
+    sp.inbox = ctx->d_inbox;
+    sp.to_below = ctx->peer_below;
+    sp.to_above = ctx->peer_above;
+    sp.stamp = ctx->xstamp;
+    kernel_table(J, q, sp.utab);
+    make_step_keys(ctx->seed, 2 * t, sp.keys);
+}
+
+static int slab_grid(const shaken_ctx *ctx, int items)
+{
+    int g = (items + SLAB_THREADS - 1) / SLAB_THREADS;
+    return g < 1 ? 1 : (g > ctx->num_sms ? ctx->num_sms : g);
+}
+
+// store this slab's bottom and top sigma rows into the neighbours' inboxes (a new exchange: every rank counts alike)
+static int slab_publish_now(shaken_ctx *ctx)
+{
+    if (ctx->xstamp == 0xFFFFFFFFu) return fail(ctx, SHAKEN_ESTATE, "slab exchange counter exhausted (2^32 - 1 exchanges)");
+    ctx->xstamp++;
+    SlabParams sp;
+    slab_params(ctx, sp, 0.0, 0.0, 0);
+    slab_publish<<<slab_grid(ctx, ctx->L / 4), SLAB_THREADS, 0, ctx->stream>>>(sp);
+    CU(cudaGetLastError());
+    ctx->launches++;
+    ctx->published = true;
+    return SHAKEN_OK;
+}
+
+extern "C" int shaken_slab_exchange(shaken_ctx *ctx)
+{
+    if (!ctx || !ctx->slab) return fail(ctx, SHAKEN_EINVAL, "shaken_slab_exchange: not a slab context");
+    if (!ctx->peer_below || !ctx->peer_above) return fail(ctx, SHAKEN_ESTATE, "shaken_slab_exchange: not connected (shaken_slab_connect)");
+    if (!ctx->have_sigma) return fail(ctx, SHAKEN_ESTATE, "shaken_slab_exchange: no sigma yet");
+    int rc = ensure_device(ctx);
+    if (rc) return rc;
+    return ctx->published ? SHAKEN_OK : slab_publish_now(ctx);
+}
+
+// the record of the last step of a run still lacks C_x, C_y: they need the neighbour's new row below this slab
+static int slab_close_record(shaken_ctx *ctx)
+{
+    if (!ctx->published) { int rc = slab_publish_now(ctx); if (rc) return rc; }
+    SlabParams sp;
+    slab_params(ctx, sp, 0.0, 0.0, 0);
+    sp.redraw = 0;
+    slab_edge<<<slab_grid(ctx, ctx->L / 16), SLAB_THREADS, 0, ctx->stream>>>(sp);
+    CU(cudaGetLastError());
+    StepParams p;
+    memset(&p, 0, sizeof(p));
+    p.L = ctx->L;
+    p.nvec = ctx->L / 16;
+    p.n_chains = 1;
+    p.chain0 = ctx->chain0;
+    p.group = 1;
+    p.nseg = (p.nvec + 31) / 32;
+    p.slab_rows = ctx->n_rows;
+    p.row0 = ctx->row0;
+    p.rows_per_task = choose_rows_per_task(ctx, p.nseg, ctx->num_sms, I8_THREADS / 32);
+    p.nrb = (ctx->n_rows + p.rows_per_task - 1) / p.rows_per_task;
+    p.ntasks = ((long long)p.nrb * p.nseg + I8_THREADS / 32 - 1) / (I8_THREADS / 32);
+    p.src = ctx->d_sigma;
+    p.rec_prev = ctx->slab_pending;
+    ctx->perwarp = false;
+    const int grid = (int)(p.ntasks < ctx->num_sms ? p.ntasks : ctx->num_sms);
+    cudaError_t e = launch_half<0, F_BONDS | F_NOUPDATE>(ctx, p, grid);
+    if (e != cudaSuccess) return fail(ctx, SHAKEN_ECUDA, "slab bond-sum launch: %s", cudaGetErrorString(e));
+    ctx->launches += 2;
+    ctx->slab_pending = nullptr;
+    return SHAKEN_OK;
+}
+
+static int run_slab(shaken_ctx *ctx, double J, double q, int64_t n_steps, int64_t obs_every)
+{
+    if (!ctx->peer_below || !ctx->peer_above) return fail(ctx, SHAKEN_ESTATE, "shaken_run: slab not connected (shaken_slab_connect)");
+    StepParams p;
+    memset(&p, 0, sizeof(p));
+    p.L = ctx->L;
+    p.nvec = ctx->L / 16;
+    p.n_chains = 1;
+    p.chain0 = ctx->chain0;
+    p.group = 1;
+    p.nseg = (p.nvec + 31) / 32;
+    p.slab_rows = ctx->n_rows;
+    p.row0 = ctx->row0;
+    const int wpb = I8_THREADS / 32;
+    p.rows_per_task = choose_rows_per_task(ctx, p.nseg, ctx->num_sms, wpb);
+    p.nrb = (ctx->n_rows + p.rows_per_task - 1) / p.rows_per_task;
+    p.ntasks = ((long long)p.nrb * p.nseg + wpb - 1) / wpb;
+    kernel_table(J, q, p.utab);
+    ctx->perwarp = false;
+    const int grid = (int)(p.ntasks < ctx->num_sms ? p.ntasks : ctx->num_sms);
+    const size_t rec_stride = SHAKEN_N_OBS;
+    ctx->have_tau = true;
+    long long *pending = ctx->slab_pending;             // a record of an earlier call that still lacks C_x, C_y
+    ctx->slab_pending = nullptr;
+    for (int64_t s = 0; s < n_steps; ++s) {
+        const uint64_t t = ctx->step;
+        const bool rec = obs_every > 0 && (t + 1) % (uint64_t)obs_every == 0;
+        long long *cur = rec ? ctx->d_rec + (size_t)ctx->n_rec * rec_stride : nullptr;
+        // hand-over: the neighbours' edge rows of the current sigma into the arrays, tau row n_rows redrawn from them
+        if (!ctx->published) { int rc = slab_publish_now(ctx); if (rc) return rc; }
+        SlabParams sp;
+        slab_params(ctx, sp, J, q, t);
+        sp.redraw = 1;
+        slab_edge<<<slab_grid(ctx, ctx->L / 16), SLAB_THREADS, 0, ctx->stream>>>(sp);
+        CU(cudaGetLastError());
+        cudaError_t e;
+        p.src = ctx->d_sigma;
+        p.dst = ctx->d_tau;
+        p.rec_cur = cur;
+        p.rec_prev = pending;
+        make_step_keys(ctx->seed, 2 * t, p.keys);
+        if (rec && pending) e = launch_half<0, F_OBS | F_BONDS>(ctx, p, grid);
+        else if (rec) e = launch_half<0, F_OBS>(ctx, p, grid);
+        else if (pending) e = launch_half<0, F_BONDS>(ctx, p, grid);
+        else e = launch_half<0, 0>(ctx, p, grid);
+        if (e != cudaSuccess) return fail(ctx, SHAKEN_ECUDA, "slab half-step 0 launch: %s", cudaGetErrorString(e));
+        pending = nullptr;
+        p.src = ctx->d_tau;
+        p.dst = ctx->d_sigma;
+        p.rec_prev = nullptr;
+        make_step_keys(ctx->seed, 2 * t + 1, p.keys);
+        if (rec) e = launch_half<1, F_OBS>(ctx, p, grid);
+        else e = launch_half<1, 0>(ctx, p, grid);
+        if (e != cudaSuccess) return fail(ctx, SHAKEN_ECUDA, "slab half-step 1 launch: %s", cudaGetErrorString(e));
+        ctx->launches += 3;
+        ctx->step = t + 1;
+        ctx->published = false;
+        { int rc = slab_publish_now(ctx); if (rc) return rc; }     // the neighbours' next half-step 0 waits for these rows
+        if (rec) {
+            pending = cur;
+            ctx->n_rec++;
+        }
+    }
+    ctx->slab_pending = pending;                        // closed by the next run or by shaken_observables
+    return SHAKEN_OK;
+}
+
 static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool uniform, int64_t n_steps, int64_t obs_every)
 {
     if (n_steps < 0 || obs_every < 0) return fail(ctx, SHAKEN_EINVAL, "shaken_run: negative count");
@@ -582,6 +864,7 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
         rc = grow_records(ctx, ctx->n_rec + n_new);
         if (rc) return rc;
     }
+    if (ctx->slab) return run_slab(ctx, J[0], q[0], n_steps, obs_every);
 
     StepParams p;
     memset(&p, 0, sizeof(p));
@@ -787,6 +1070,7 @@ static int run_alt_impl(shaken_ctx *ctx, const double *J, bool uniform, int64_t 
     const int nJ = uniform ? 1 : ctx->n_chains;
     for (int i = 0; i < nJ; ++i)
         if (!isfinite(J[i])) return fail(ctx, SHAKEN_EINVAL, "shaken_run_alternate: non-finite coupling for chain %d", i);
+    if (ctx->slab) return fail(ctx, SHAKEN_ESTATE, "shaken_run_alternate: not available on a slab context");
     if (!ctx->have_sigma || !ctx->d_sigma) return fail(ctx, SHAKEN_ESTATE, "shaken_run_alternate: no sigma yet (call shaken_init, shaken_set_spins or shaken_adopt_spins)");
     int rc = ensure_device(ctx);
     if (rc) return rc;
@@ -943,6 +1227,10 @@ extern "C" int shaken_run_alternate_grid(shaken_ctx *ctx, const double *J, int64
 extern "C" int64_t shaken_observables(shaken_ctx *ctx, int64_t *out, int64_t max_records)
 {
     if (!ctx || max_records < 0) return fail(ctx, SHAKEN_EINVAL, "shaken_observables: bad argument");
+    if (ctx->slab && ctx->slab_pending) {
+        const int rc = slab_close_record(ctx);
+        if (rc) return rc;
+    }
     const int64_t n = ctx->n_rec < max_records ? ctx->n_rec : max_records;
     if (n > 0) {
         if (!out) return fail(ctx, SHAKEN_EINVAL, "shaken_observables: out is NULL");
@@ -977,7 +1265,7 @@ extern "C" int shaken_get_spins(shaken_ctx *ctx, int which, int8_t *host)
     if (!ctx || !host || (which != 0 && which != 1)) return fail(ctx, SHAKEN_EINVAL, "shaken_get_spins: bad argument");
     if (!(which ? ctx->have_tau : ctx->have_sigma) || !ctx->d_sigma)
         return fail(ctx, SHAKEN_ESTATE, "shaken_get_spins: %s has no defined content yet", which ? "tau" : "sigma");
-    const size_t n = (size_t)ctx->n_chains * ctx->L * ctx->L;
+    const size_t n = ctx->slab ? shaken_spin_bytes(ctx) : (size_t)ctx->n_chains * ctx->L * ctx->L;
     const void *src = which ? ctx->d_tau : ctx->d_sigma;
     if (!ctx->packed) {
         CU(cudaMemcpyAsync(host, src, n, cudaMemcpyDeviceToHost, ctx->stream));
@@ -1003,8 +1291,15 @@ extern "C" int shaken_set_spins(shaken_ctx *ctx, int which, const int8_t *host)
     if (!ctx || !host || (which != 0 && which != 1)) return fail(ctx, SHAKEN_EINVAL, "shaken_set_spins: bad argument");
     int rc = ensure_spins(ctx);
     if (rc) return rc;
-    const size_t n = (size_t)ctx->n_chains * ctx->L * ctx->L;
+    const size_t n = ctx->slab ? shaken_spin_bytes(ctx) : (size_t)ctx->n_chains * ctx->L * ctx->L;
     void *dst = which ? ctx->d_tau : ctx->d_sigma;
+    if (which == 0) {
+        if (ctx->slab && ctx->slab_pending) {            // the last record's C_x, C_y are sums over the sigma about to be replaced
+            rc = slab_close_record(ctx);
+            if (rc) return rc;
+        }
+        ctx->published = false;
+    }
     CU(cudaMemsetAsync(ctx->d_bad, 0, sizeof(unsigned long long), ctx->stream));
     if (!ctx->packed) {
         CU(cudaMemcpyAsync(dst, host, n, cudaMemcpyHostToDevice, ctx->stream));
@@ -1060,6 +1355,7 @@ extern "C" int shaken_adopt_spins(shaken_ctx *ctx)
 extern "C" int shaken_diag_correlations(shaken_ctx *ctx, const int32_t *ells, int32_t n_ell, int64_t *out)
 {
     if (!ctx || !ells || !out || n_ell < 1) return fail(ctx, SHAKEN_EINVAL, "shaken_diag_correlations: bad argument");
+    if (ctx->slab) return fail(ctx, SHAKEN_ESTATE, "shaken_diag_correlations: not available on a slab context");
     if (!ctx->have_sigma || !ctx->d_sigma) return fail(ctx, SHAKEN_ESTATE, "shaken_diag_correlations: no sigma yet");
     for (int e = 0; e < n_ell; ++e)
         if (ells[e] < 0) return fail(ctx, SHAKEN_EINVAL, "shaken_diag_correlations: negative distance");

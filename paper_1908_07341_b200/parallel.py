@@ -1,4 +1,4 @@
-"""Sharding a batch of chains over ranks.
+"""Sharding over ranks: a batch of chains by chains, one large lattice by row slabs.
 
 Chains are independent units, so the path shards with NO data-path collective: rank r owns a contiguous range of
 global chain indices and tells its context ``shaken_set_chain_offset(first)``, which makes local chain c draw the
@@ -71,3 +71,62 @@ def gather_records(local: np.ndarray, n_chains: int, group=None, device=None) ->
         f, c = chain_shard(n_chains, world, r)
         out[:, f:f + c] = part[:, :c].cpu().numpy()
     return out
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# Row slabs of ONE lattice (second bullet).  Rank r owns a contiguous block of rows; per full step it sends
+# its bottom sigma row to the rank below and its top sigma row to the rank above (one exchange, 2 x L bytes) -- the tau row
+# just above a slab is redrawn redundantly by that slab, which the counter-based generator makes bit-identical.  On GPUs
+# the rows travel by peer stores inside libshaken's kernels (kernel_slab.cuh); this module only does the index
+# arithmetic, the exchange of the IPC handles and the final sum of the per-slab int64 records.
+# ---------------------------------------------------------------------------------------------------------------------
+def slab_shard(L: int, world: int, rank: int) -> Tuple[int, int]:
+    """(row0, n_rows) of rank ``rank``: contiguous, balanced, at least two rows each (the library's minimum)."""
+    if world < 1 or not 0 <= rank < world or L < 2 * world:
+        raise ValueError("bad slab request: every rank needs at least two rows")
+    base, extra = divmod(L, world)
+    row0 = rank * base + min(rank, extra)
+    return row0, base + (1 if rank < extra else 0)
+
+
+def slab_neighbours(world: int, rank: int) -> Tuple[int, int]:
+    """(rank below, rank above) on the torus: the owners of row row0 - 1 and of row row0 + n_rows."""
+    return (rank - 1) % world, (rank + 1) % world
+
+
+def open_slab(L: int, seed: int, world: int, rank: int, **kw):
+    """This rank's slab context of an L x L lattice split over ``world`` ranks."""
+    from . import shaken
+
+    row0, n_rows = slab_shard(L, world, rank)
+    return shaken.ShakenSlab(L, row0, n_rows, seed, **kw)
+
+
+def connect_slabs_ipc(slab, group=None):
+    """Exchange the CUDA IPC handles of the slabs' inboxes over torch.distributed (one process per GPU) and connect every
+    slab to its two neighbours.  With a single rank the slab is its own neighbour on both sides (no IPC needed)."""
+    import torch.distributed as dist
+
+    world = dist.get_world_size(group) if dist.is_initialized() else 1
+    rank = dist.get_rank(group) if dist.is_initialized() else 0
+    if world == 1:
+        ptr = slab.inbox()
+        slab.connect(ptr, ptr)
+        return
+    handles = [None] * world
+    dist.all_gather_object(handles, slab.ipc_export(), group=group)
+    below, above = slab_neighbours(world, rank)
+    slab.ipc_connect(handles[below], handles[above])
+
+
+def sum_slab_records(local: np.ndarray, group=None, device=None) -> np.ndarray:
+    """The records of the whole lattice: the element-wise sum of the per-slab records ``[n_rec, 1, 6]`` (int64)."""
+    import torch
+    import torch.distributed as dist
+
+    t = torch.from_numpy(np.ascontiguousarray(local, dtype=np.int64).copy())
+    if device is not None:
+        t = t.to(device)
+    if dist.is_initialized() and dist.get_world_size(group) > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.SUM, group=group)
+    return t.cpu().numpy()

@@ -56,6 +56,13 @@ SIGNATURES = {
     "shaken_launch_count": (C.c_int64, [_p]),
     "shaken_set_variant": (C.c_int, [_p, C.c_int]),
     "shaken_adopt_spins": (C.c_int, [_p]),
+    "shaken_create_slab": (C.c_int, [C.POINTER(_p), C.c_int32, C.c_int32, C.c_int32, C.c_uint64]),
+    "shaken_set_stream": (C.c_int, [_p, _p]),
+    "shaken_slab_inbox": (C.c_int, [_p, C.POINTER(_p), C.POINTER(C.c_size_t)]),
+    "shaken_slab_connect": (C.c_int, [_p, _p, _p]),
+    "shaken_slab_ipc_export": (C.c_int, [_p, _p]),
+    "shaken_slab_ipc_connect": (C.c_int, [_p, _p, _p]),
+    "shaken_slab_exchange": (C.c_int, [_p]),
     "shaken_test_band_hook": (C.c_int, [_p, C.c_int, C.c_uint32]),
     "shaken_moments": (C.c_int, [_p, C.c_int64, C.c_int64, C.c_int64, C.POINTER(C.c_double)]),
     "shaken_selftest_philox_rate": (C.c_int, [C.c_int32, C.c_int32, C.c_int32, C.POINTER(C.c_double)]),
@@ -310,6 +317,55 @@ class Shaken:
 
     def set_variant(self, v: int):
         self._ck(self._lib.shaken_set_variant(self._h, int(v)))
+
+
+class ShakenSlab(Shaken):
+    """Rows [row0, row0 + n_rows) of one L x L lattice (shaken_create_slab): one slab of a row-slab sharded run.  The
+    library owns the device buffers; spins move as [n_rows, L] arrays; records are the slab's partial sums."""
+
+    def __init__(self, L: int, row0: int, n_rows: int, seed: int = 0, max_records: int = 0, stream=None):
+        self.L, self.n_chains, self.seed, self.packed = int(L), 1, int(seed), False
+        self.row0, self.n_rows = int(row0), int(n_rows)
+        self._h = _p()
+        self._lib = lib()
+        self._tensors = None
+        rc = self._lib.shaken_create_slab(C.byref(self._h), self.L, self.row0, self.n_rows, self.seed & (2**64 - 1))
+        if rc:
+            self._h = _p()
+            raise ShakenError(rc, self._lib.shaken_last_error(None).decode())
+        if stream is not None:
+            self._ck(self._lib.shaken_set_stream(self._h, stream.cuda_stream))
+            self._tensors = (None, None, None, stream)          # keeps the stream alive
+        if max_records:
+            self._ck(self._lib.shaken_reserve_records(self._h, int(max_records)))
+
+    @property
+    def n_sites(self) -> int:
+        return self.n_rows * self.L
+
+    def get_spins(self, which: int, out: Optional[np.ndarray] = None) -> np.ndarray:
+        if out is None:
+            out = np.empty((self.n_rows, self.L), dtype=np.int8)
+        return super().get_spins(which, out)
+
+    def inbox(self) -> int:
+        ptr, nb = _p(), C.c_size_t()
+        self._ck(self._lib.shaken_slab_inbox(self._h, C.byref(ptr), C.byref(nb)))
+        return int(ptr.value)
+
+    def connect(self, below_inbox: int, above_inbox: int):
+        self._ck(self._lib.shaken_slab_connect(self._h, _p(below_inbox), _p(above_inbox)))
+
+    def ipc_export(self) -> bytes:
+        buf = C.create_string_buffer(64)
+        self._ck(self._lib.shaken_slab_ipc_export(self._h, buf))
+        return buf.raw
+
+    def ipc_connect(self, below_handle: bytes, above_handle: bytes):
+        self._ck(self._lib.shaken_slab_ipc_connect(self._h, C.c_char_p(below_handle), C.c_char_p(above_handle)))
+
+    def exchange(self):
+        self._ck(self._lib.shaken_slab_exchange(self._h))
 
 
 # ---------------------------------------------------------------------- (a9) derived statistics, host side

@@ -1,0 +1,124 @@
+"""Parity (``-m gpu``) of row-slab sharding (second bullet; include/shaken.h shaken_create_slab): ONE lattice
+split into slabs of rows, every slab its own libshaken context, the slabs exchanging one sigma row each way per full
+step through their inboxes.  Only one GPU is available, so the slabs live on the same device and are advanced ONE AFTER
+THE OTHER on the same stream (all publish, then each runs a step): no kernel ever waits for a kernel that has not been
+launched.  The kernels, the halo logic, the stamps and the per-slab records are exactly those of a multi-GPU run; only
+the transport (peer stores over NVLink, IPC handles) is not exercised.  Expected values: the oracle's unsplit lattice."""
+import numpy as np
+import pytest
+
+from oracle import shaken_oracle as so
+from paper_1908_07341_b200 import parallel, shaken
+
+pytestmark = pytest.mark.gpu
+
+
+def open_ring(L, seed, bounds, max_records):
+    slabs = [shaken.ShakenSlab(L, r0, r1 - r0, seed, max_records=max_records) for r0, r1 in zip(bounds[:-1], bounds[1:])]
+    n = len(slabs)
+    for k, s in enumerate(slabs):
+        s.connect(slabs[(k - 1) % n].inbox(), slabs[(k + 1) % n].inbox())
+    return slabs
+
+
+@pytest.mark.parametrize("L,bounds", [(64, [0, 64]), (64, [0, 32, 64]), (272, [0, 100, 102, 272]), (528, [0, 176, 352, 528]),
+                                      (1056, [0, 2, 530, 1056])])
+def test_slabs_of_one_lattice_match_the_unsplit_oracle(L, bounds):
+    seed, steps, J, q = 7 + L, 7, 0.55, 0.8
+    o = so.Oracle(L, 1, seed)
+    o.init(0)
+    o.run(J, q, steps, 2)
+    slabs = open_ring(L, seed, bounds, steps)
+    try:
+        for s in slabs:
+            s.init(0)
+        for t in range(steps):
+            for s in slabs:
+                s.exchange()                      # all slabs publish before any of them waits
+            for s in slabs:
+                s.run(J, q, 1, 2)
+        sigma = np.vstack([s.get_spins(0) for s in slabs])
+        tau = np.vstack([s.get_spins(1) for s in slabs])
+        assert np.array_equal(sigma, o.get_spins(0)[0]), "sigma differs"
+        assert np.array_equal(tau, o.get_spins(1)[0]), "tau differs"
+        rec = sum(s.observables() for s in slabs)
+        assert np.array_equal(rec, o.observables()), "summed records differ"
+        assert all(s.step == steps for s in slabs)
+    finally:
+        for s in slabs:
+            s.close()
+
+
+def test_single_slab_runs_many_steps_per_call_and_resumes():
+    """One slab covering the whole lattice is its own neighbour: shaken_run(n) then needs no driver in between (each step
+    publishes to itself), records every step, run split in two calls, set_spins in between."""
+    L, seed, J, q = 528, 99, 0.7, 0.3
+    o = so.Oracle(L, 1, seed)
+    o.init(1)
+    o.run(J, q, 9, 1)
+    s = shaken.ShakenSlab(L, 0, L, seed, max_records=16)
+    try:
+        ptr = s.inbox()
+        s.connect(ptr, ptr)
+        s.init(1)
+        s.run(J, q, 4, 1)
+        mid = s.get_spins(0).copy()
+        s.set_spins(0, mid)                       # forgets the published rows: the next run publishes again
+        s.run(J, q, 5, 1)
+        assert np.array_equal(s.get_spins(0), o.get_spins(0)[0]) and np.array_equal(s.get_spins(1), o.get_spins(1)[0])
+        assert np.array_equal(s.observables(), o.observables())
+    finally:
+        s.close()
+
+
+def test_slab_argument_and_state_errors():
+    lib = shaken.lib()
+    with pytest.raises(shaken.ShakenError):
+        shaken.ShakenSlab(64, 0, 1, 1)            # fewer than two rows
+    with pytest.raises(shaken.ShakenError):
+        shaken.ShakenSlab(64, 60, 8, 1)           # beyond the lattice
+    s = shaken.ShakenSlab(64, 0, 32, 1)
+    try:
+        s.init(1)
+        with pytest.raises(shaken.ShakenError) as e:
+            s.run(0.5, 0.5, 1, 0)                 # not connected
+        assert e.value.code == shaken.ESTATE
+        with pytest.raises(shaken.ShakenError):
+            s.run_alternate(0.4, 1, 0)
+        assert parallel.slab_shard(64, 2, 1) == (32, 32)
+    finally:
+        s.close()
+
+
+def _device_count():
+    try:
+        import torch
+
+        return torch.cuda.device_count()
+    except Exception:
+        return 0
+
+
+@pytest.mark.skipif(_device_count() < 2, reason="needs two GPUs (the N > 1 arm of bench.py under torchrun)")
+@pytest.mark.parametrize("extra", [[], ["--slabs"]])
+def test_bench_two_ranks_under_torchrun(extra):
+    """The N > 1 arm of bench.py exactly as the driver launches it: replicas (weak scaling, no collective) and row slabs
+    of one lattice (strong scaling, peer stores through CUDA IPC inboxes)."""
+    import json
+    import os
+    import socket
+    import subprocess
+    import sys
+
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.join(root, "bench.py"), "--gpus", "2", "--steps", "3", "--warmup", "3",
+           "--no-cpu-baseline", "--workload", "paper4096"] + extra
+    out = subprocess.run(cmd, capture_output=True, text=True, timeout=600, cwd=root)
+    assert out.returncode == 0, out.stderr[-2000:]
+    line = json.loads([ln for ln in out.stdout.splitlines() if ln.startswith("{")][-1])
+    assert line["n_gpus"] == 2 and line["value"] > 0
+    assert line["scaling"] == ("strong" if extra else "weak")
