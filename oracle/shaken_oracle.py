@@ -7,7 +7,7 @@ The arithmetic lives in the C file (which cites PAPER.md passage by passage); th
 marshals arguments and, in :func:`derived_stats`, turns int64 records into the double-precision
 quantities of PAPER.md:194 (mean and variance of the magnetisation m, eq. 17 :196) plus
 <|m|>, <m^2>, <m^4> and the Binder cumulant named by BASELINE.json, using exact Python integers and
-ONE final division each.
+ONE final division each (pinned by hand-computed records in tests/test_oracle_stats.py).
 """
 from __future__ import annotations
 
