@@ -175,7 +175,8 @@ __global__ void __launch_bounds__(I8_THREADS, 1) half_step_i8(const __grid_const
             const uint32_t lane8 = (uint32_t)lane * 8u;
             // coalescence test: members other than the first of a group that has not coalesced yet
             const int member = COAL ? chain % p.group : 0;
-            const bool cmp = COAL && member != 0 && p.coal[chain / p.group] < 0;
+            // (not yet coalesced, and no difference of this step on record yet: one is enough)
+            const bool cmp = COAL && member != 0 && p.coal[chain / p.group] < 0 && __ldcg(p.diff + chain / p.group) != p.cstamp;
             const ptrdiff_t to_first = -(ptrdiff_t)member * (ptrdiff_t)plane - (ptrdiff_t)2 * stride;   // pc runs two rows ahead
             uint32_t differs = 0;
 

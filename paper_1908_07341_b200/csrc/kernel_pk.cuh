@@ -129,7 +129,8 @@ __global__ void __launch_bounds__(PK_THREADS, 1) half_step_pk(const __grid_const
             int a0 = 0, a1 = 0, a2 = 0;     // popcount partials of this task
             // coalescence test: members other than the first of a group that has not coalesced yet
             const int member = COAL ? chain % p.group : 0;
-            const bool cmp = COAL && member != 0 && p.coal[chain / p.group] < 0;
+            // (not yet coalesced, and no difference of this step on record yet: one is enough)
+            const bool cmp = COAL && member != 0 && p.coal[chain / p.group] < 0 && __ldcg(p.diff + chain / p.group) != p.cstamp;
             const ptrdiff_t to_first = -(ptrdiff_t)member * (ptrdiff_t)plane;
             uint32_t differs = 0;
 

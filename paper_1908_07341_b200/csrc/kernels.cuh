@@ -142,6 +142,7 @@ __global__ void coalesce_compare(const uint4 *sigma, long long vec_per_chain, in
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
         const long long gi = i / per_group, rest = i - gi * per_group;
         if (coal[gi] >= 0) continue;
+        if (__ldcg(diff + gi) == stamp) continue;          // a difference of this step is already on record: nothing left to find
         const long long m = 1 + rest / vec_per_chain, v = rest % vec_per_chain;
         const uint4 a = sigma[(gi * group) * vec_per_chain + v], b = sigma[(gi * group + m) * vec_per_chain + v];
         if (a.x != b.x || a.y != b.y || a.z != b.z || a.w != b.w) diff[gi] = stamp;

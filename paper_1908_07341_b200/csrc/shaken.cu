@@ -464,7 +464,7 @@ extern "C" int shaken_init(shaken_ctx *ctx, int mode)
 // ---------------------------------------------------------------------------------------------------
 // launch with programmatic stream serialization (see kernels_common.cuh: wait_for_previous_kernel)
 template <typename K, typename P>
-static void launch_pdl(K kernel, int grid, int threads, cudaStream_t stream, const P &p)
+static cudaError_t launch_pdl(K kernel, int grid, int threads, cudaStream_t stream, const P &p)
 {
     cudaLaunchConfig_t cfg;
     memset(&cfg, 0, sizeof(cfg));
@@ -476,7 +476,7 @@ static void launch_pdl(K kernel, int grid, int threads, cudaStream_t stream, con
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    cudaLaunchKernelEx(&cfg, kernel, p);
+    return cudaLaunchKernelEx(&cfg, kernel, p);
 }
 
 template <int HALF, int FLAGS>
@@ -484,10 +484,11 @@ static cudaError_t launch_half(const shaken_ctx *ctx, const StepParams &p, int g
 {
     // int8: block tasks (one threshold table per block; plain half-steps use the paired lookup) or per-warp task
     // lists (kernel_i8.cuh); results are identical
-    if (ctx->packed) launch_pdl(half_step_pk<HALF, FLAGS>, grid, PK_THREADS, ctx->stream, p);
-    else if (ctx->perwarp) launch_pdl(half_step_i8<HALF, FLAGS, true>, grid, I8_THREADS, ctx->stream, p);
-    else launch_pdl(half_step_i8<HALF, FLAGS, false>, grid, I8_THREADS, ctx->stream, p);
-    return cudaGetLastError();
+    cudaError_t e;
+    if (ctx->packed) e = launch_pdl(half_step_pk<HALF, FLAGS>, grid, PK_THREADS, ctx->stream, p);
+    else if (ctx->perwarp) e = launch_pdl(half_step_i8<HALF, FLAGS, true>, grid, I8_THREADS, ctx->stream, p);
+    else e = launch_pdl(half_step_i8<HALF, FLAGS, false>, grid, I8_THREADS, ctx->stream, p);
+    return e != cudaSuccess ? e : cudaGetLastError();
 }
 
 static int choose_rows_per_task(const shaken_ctx *ctx, int nseg, long long grid_cap, int wpb, double *score_out = nullptr)
@@ -1176,22 +1177,25 @@ static int run_alt_impl(shaken_ctx *ctx, const double *J, bool uniform, int64_t 
         const uint64_t t = ctx->step;
         const bool rec = obs_every > 0 && (t + 1) % (uint64_t)obs_every == 0;
         p.rec = nullptr;
+        cudaError_t le;
         make_step_keys(ctx->seed, 2 * t, p.keys);
-        if (ctx->packed) launch_pdl(alt_half<0, false, true>, grid, ALT_THREADS, ctx->stream, p);
-        else if (strips) launch_pdl(alt_strip_i8<0, false>, grid, ALT_THREADS, ctx->stream, p);
-        else launch_pdl(alt_half<0, false, false>, grid, ALT_THREADS, ctx->stream, p);
+        if (ctx->packed) le = launch_pdl(alt_half<0, false, true>, grid, ALT_THREADS, ctx->stream, p);
+        else if (strips) le = launch_pdl(alt_strip_i8<0, false>, grid, ALT_THREADS, ctx->stream, p);
+        else le = launch_pdl(alt_half<0, false, false>, grid, ALT_THREADS, ctx->stream, p);
+        if (le != cudaSuccess) return fail(ctx, SHAKEN_ECUDA, "alternate half-step 0 launch: %s", cudaGetErrorString(le));
         make_step_keys(ctx->seed, 2 * t + 1, p.keys);
         if (rec) {
             p.rec = ctx->d_rec + (size_t)ctx->n_rec * rec_stride;
-            if (ctx->packed) launch_pdl(alt_half<1, true, true>, grid, ALT_THREADS, ctx->stream, p);
-            else if (strips) launch_pdl(alt_strip_i8<1, true>, grid, ALT_THREADS, ctx->stream, p);
-            else launch_pdl(alt_half<1, true, false>, grid, ALT_THREADS, ctx->stream, p);
+            if (ctx->packed) le = launch_pdl(alt_half<1, true, true>, grid, ALT_THREADS, ctx->stream, p);
+            else if (strips) le = launch_pdl(alt_strip_i8<1, true>, grid, ALT_THREADS, ctx->stream, p);
+            else le = launch_pdl(alt_half<1, true, false>, grid, ALT_THREADS, ctx->stream, p);
             ctx->n_rec++;
         } else {
-            if (ctx->packed) launch_pdl(alt_half<1, false, true>, grid, ALT_THREADS, ctx->stream, p);
-            else if (strips) launch_pdl(alt_strip_i8<1, false>, grid, ALT_THREADS, ctx->stream, p);
-            else launch_pdl(alt_half<1, false, false>, grid, ALT_THREADS, ctx->stream, p);
+            if (ctx->packed) le = launch_pdl(alt_half<1, false, true>, grid, ALT_THREADS, ctx->stream, p);
+            else if (strips) le = launch_pdl(alt_strip_i8<1, false>, grid, ALT_THREADS, ctx->stream, p);
+            else le = launch_pdl(alt_half<1, false, false>, grid, ALT_THREADS, ctx->stream, p);
         }
+        if (le != cudaSuccess) return fail(ctx, SHAKEN_ECUDA, "alternate half-step 1 launch: %s", cudaGetErrorString(le));
         CU(cudaGetLastError());
         ctx->launches += 2;
         ctx->step = t + 1;
