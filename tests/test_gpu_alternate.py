@@ -80,7 +80,7 @@ def test_alternate_batch_of_mid_size_chains_runs_in_the_one_cta_per_chain_path()
             assert np.array_equal(s.observables(), o.observables()), variant
 
 
-@pytest.mark.parametrize("L,n_chains", [(144, 1), (272, 3), (528, 1), (1024, 1), (2048, 1), (1024, 4)])
+@pytest.mark.parametrize("L,n_chains", [(144, 1), (160, 74), (272, 3), (304, 37), (528, 1), (784, 2), (1024, 1), (2048, 1), (1024, 4)])
 def test_alternate_band_path_one_launch_per_run_matches_oracle(L, n_chains):
     """128 < L <= 2048 with few chains: the whole shaken_run_alternate call is ONE cooperative launch (alt_band_i8: row
     bands in shared memory, two halo rows per side, one hand-over per full step).  Per-chain couplings, records on some

@@ -374,6 +374,28 @@ def test_band_kernel_tall_bands_per_chain_tables_and_split_runs(L, n_chains):
         assert_same_state(s, o, f"L={L} chains={n_chains}")
 
 
+@pytest.mark.parametrize("L,n_chains,steps,obs", [(144, 1, 9, 1), (144, 5, 6, 2), (160, 148, 3, 1), (272, 2, 11, 3), (400, 3, 7, 0),
+                                                 (784, 1, 8, 1), (1040, 2, 5, 2), (1536, 1, 4, 1), (2048, 1, 3, 1), (304, 37, 4, 1)])
+def test_band_kernel_sweep_of_shapes_matches_oracle(L, n_chains, steps, obs):
+    """The one-launch band path over the shapes it serves: 9 to 128 vectors per row, one-row bands (148 chains), bands of
+    28 rows, a ragged last band, several chains with their own couplings, every record cadence; each run split in two."""
+    if n_chains * L * L > 4.5e6:
+        pytest.skip("beyond the band path")
+    seed = 1000 + L + n_chains
+    J = np.linspace(0.35, 0.75, n_chains)
+    q = np.linspace(0.9, 0.3, n_chains)
+    o = so.Oracle(L, n_chains, seed)
+    o.init(0)
+    o.run_grid(J, q, steps, obs)
+    with shaken.Shaken(L, n_chains, seed, max_records=steps) as s:
+        s.init(0)
+        l0 = s.launch_count
+        s.run_grid(J, q, steps // 2, obs)
+        s.run_grid(J, q, steps - steps // 2, obs)
+        assert s.launch_count - l0 == 2, "one cooperative launch per run call expected"
+        assert_same_state(s, o, f"L={L} chains={n_chains}")
+
+
 # ----------------------------------------------------------------------------- coupled chains, coalescence (SURVEY 8(f) rank 1)
 @pytest.mark.parametrize("packed,variant", [(False, 0), (False, 3), (True, 0)])
 def test_coupled_chains_and_coalescence_times_match_oracle(packed, variant):
