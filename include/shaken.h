@@ -204,9 +204,11 @@ int shaken_set_chain_offset(shaken_ctx *ctx, uint32_t first_chain);
  *   random numbers": all draw the words of the group's first chain (counter word 1 = first_chain + (c / group) * group).
  *   group >= 1 must divide n_chains; 1 (default) uncouples.  Couplings J, q are still per chain (give the members of a
  *   group the same values for the paper's experiment).  Forgets coalescence times.  Errors: SHAKEN_EINVAL, SHAKEN_ENOMEM.
- * While group > 1, after EVERY full step the sigma layers of each group's members are compared on the device; the
- *   coalescence time T = min{n : X_n = Y_n} of a group is the number of full steps done (global step counter) when they
- *   were first all equal.  shaken_init resets the times to -1.
+ * While group > 1 the sigma layers of each group's members are compared on the device after EVERY full step (fused into
+ *   the half-step kernels: the comparison of a step rides on the launches of the next one, a read-only pass closes a
+ *   run call, so the times are complete when shaken_run's work has finished); the coalescence time T = min{n : X_n = Y_n}
+ *   of a group is the number of full steps done (global step counter) when they were first all equal.  shaken_init
+ *   resets the times to -1.
  * shaken_coalescence: copy min(n_chains / group, max_groups) times to out (HOST int64, -1 = not yet); returns the
  *   count (0 when uncoupled) or a negative error code.  Synchronises the stream.
  */

@@ -40,7 +40,6 @@ struct shaken_ctx {
     size_t xch_bytes = 0;
     uint32_t xch_stamp = 0;       // last stamp written into d_xch
     int coop = -1;                // cooperative launch supported (-1: not queried yet)
-    bool band_refused = false;    // test hook: never take the band path
     bool band_refuse_next = false;   // test hook: treat the next cooperative launch as refused (exercises the fall-back)
     void *d_stage = nullptr;      // staging for packed <-> int8 conversion
     size_t stage_bytes = 0;
@@ -544,7 +543,7 @@ static int try_band_launch(shaken_ctx *ctx, bool alternate, const uint32_t *gtab
     // worth it while a half-step is short next to a launch; measured against the strip kernels: 3.6x at 512^2, 2.5x at
     // 1024^2, 2.2x at 2048^2 (the largest band that fits shared memory)
     const bool small_job = (double)ctx->n_chains * ctx->L * ctx->L <= 4.5e6;
-    if (!ctx->coop || !small_job || smem > 160 * 1024 || ctx->band_refused) return 1;
+    if (!ctx->coop || !small_job || smem > 160 * 1024) return 1;
     const int rows_out = alternate ? 2 : 1;                           // rows a band publishes per side and step
     const size_t xrow = (size_t)2 * n_bands * rows_out * W;           // uint2 elements per hand-over array (two parities)
     const size_t need = 2 * xrow * sizeof(uint2);
@@ -694,7 +693,11 @@ extern "C" int shaken_slab_ipc_connect(shaken_ctx *ctx, const void *below_handle
     void *pb = nullptr, *pa = nullptr;
     CU(cudaIpcOpenMemHandle(&pb, hb, cudaIpcMemLazyEnablePeerAccess));
     if (memcmp(&hb, &ha, 64) == 0) pa = pb;             // two ranks: the same neighbour on both sides
-    else CU(cudaIpcOpenMemHandle(&pa, ha, cudaIpcMemLazyEnablePeerAccess));
+    else if (cudaIpcOpenMemHandle(&pa, ha, cudaIpcMemLazyEnablePeerAccess) != cudaSuccess) {
+        const cudaError_t e = cudaGetLastError();
+        cudaIpcCloseMemHandle(pb);
+        return fail(ctx, SHAKEN_ECUDA, "cudaIpcOpenMemHandle (rank above): %s", cudaGetErrorString(e));
+    }
     ctx->ipc_below = pb;
     ctx->ipc_above = pa;
     return shaken_slab_connect(ctx, pb, pa);
