@@ -67,7 +67,7 @@ __global__ void __launch_bounds__(I8_THREADS, 1) half_step_i8(const __grid_const
     const int R = p.rows_per_task;
     const int NR = p.slab_rows ? p.slab_rows : L;                   // rows this launch redraws
     const size_t plane = (size_t)L * (size_t)L;
-    const int tpc = p.nrb * p.nseg;                                  // warp tasks per chain
+    const int tpc = p.nrb * p.nseg;                                  // warp tasks per chain (block tasks)
     const int bpc = (tpc + WPB - 1) / WPB;                           // block tasks per chain
 
     int cur_chain = -1;
@@ -97,8 +97,25 @@ __global__ void __launch_bounds__(I8_THREADS, 1) half_step_i8(const __grid_const
     const long long task0 = PERWARP ? (long long)blockIdx.x * WPB + warp : (long long)blockIdx.x;
     const long long task_step = PERWARP ? (long long)gridDim.x * WPB : (long long)gridDim.x;
     for (long long bt = task0; bt < p.ntasks; bt += task_step) {
-        const int chain = (int)(bt / (PERWARP ? tpc : bpc));
-        const int lt = PERWARP ? (int)(bt % tpc) : (int)(bt % bpc) * WPB + warp;   // this warp's task inside the chain
+      // PERWARP: task bt is a RANGE of p.range_len consecutive strip-rows g = ((chain * nseg + seg) * NR + row) -- the same
+      // number for every warp, so the launch is one full wave whatever the chain size -- walked piece by piece (a piece
+      // ends where the column strip ends).  Otherwise one piece: strip lt of the block's chain, rows rb * R ...
+      long long g = PERWARP ? bt * (long long)p.range_len : 0;
+      const long long g_end = PERWARP ? min(g + (long long)p.range_len, p.rows_total) : 1;
+      do {
+        int chain, lt, pr_first = 0, pr_rows = 0;
+        if (PERWARP) {
+            const long long cs = g / NR;
+            pr_first = (int)(g - cs * NR);
+            pr_rows = (int)min((long long)(NR - pr_first), g_end - g);
+            chain = (int)(cs / p.nseg);
+            lt = (int)(cs - (long long)chain * p.nseg);                 // the column segment
+            g += pr_rows;
+        } else {
+            chain = (int)(bt / bpc);
+            lt = (int)(bt % bpc) * WPB + warp;                          // this warp's task inside the chain
+            g = g_end;
+        }
         if (PERWARP && chain != cur_chain) {                          // warp-uniform
             if ((OBS || BONDS) && cur_chain >= 0) flush(cur_chain);
             cur_chain = chain;
@@ -141,13 +158,13 @@ __global__ void __launch_bounds__(I8_THREADS, 1) half_step_i8(const __grid_const
                 __syncthreads();
             }
         }
-        const int seg = lt % p.nseg;
+        const int seg = PERWARP ? lt : lt % p.nseg;
         const int rb = lt / p.nseg;
         const int cv = seg * 32 + lane;
-        if (lt < tpc && cv < p.nvec) {
+        if ((PERWARP || lt < tpc) && cv < p.nvec) {
             const int c0 = cv * 16;
-            const int r_first = rb * R;
-            const int r_last = min(NR, r_first + R) - 1;
+            const int r_first = PERWARP ? pr_first : rb * R;
+            const int r_last = PERWARP ? pr_first + pr_rows - 1 : min(NR, r_first + R) - 1;
             const int rows = r_last - r_first + 1;
             const uint8_t *sbase = reinterpret_cast<const uint8_t *>(p.src) + (size_t)chain * plane;
             uint8_t *dbase = reinterpret_cast<uint8_t *>(p.dst) + (size_t)chain * plane;
@@ -278,6 +295,7 @@ __global__ void __launch_bounds__(I8_THREADS, 1) half_step_i8(const __grid_const
             }
             if (COAL && differs != 0) p.diff[chain / p.group] = p.cstamp;   // every writer stores the same value
         }
+      } while (PERWARP && g < g_end);
     }
     if ((OBS || BONDS) && cur_chain >= 0) flush(cur_chain);
 }

@@ -36,7 +36,9 @@ struct StepParams {
     int rows_per_task;
     int nseg;               // warp-wide strips per row = ceil(nvec / 32)
     int nrb;                // row blocks = ceil(L / rows_per_task)
-    long long ntasks;       // n_chains * nrb * nseg
+    long long ntasks;       // block tasks: n_chains * ceil(nrb * nseg / warps per block); per-warp lists: number of ranges
+    long long rows_total;   // per-warp lists: n_chains * nseg * rows = strip-rows in the launch
+    int range_len;          // per-warp lists: strip-rows per range (<= MAX_ROWS_PER_TASK)
     int slab_rows;          // 0: a whole L x L torus.  > 0: a SLAB of one lattice (row-slab sharding, kernel_slab.cuh): this
                             // many rows are redrawn; src / dst point at the slab's row 0 and the arrays hold the rows just
                             // below (index -1) and above (index slab_rows) as well, so vertical neighbours never wrap

@@ -883,22 +883,34 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
     const long long cap = (long long)ctx->num_sms * resident;
     double score_block = 0.0;
     p.rows_per_task = choose_rows_per_task(ctx, p.nseg, cap, wpb, &score_block);
-    // many small chains: per-warp task lists (kernel_i8.cuh PER_WARP) balance at warp granularity with tall strips;
-    // they cannot use the paired lookup, which is worth ~5 % on launches without fused sums
-    ctx->perwarp = false;
-    if (!ctx->packed && (ctx->variant == SHAKEN_VARIANT_PERWARP || ctx->n_chains > 1)) {
-        double score_pw = 0.0;
-        const int Rpw = choose_rows_per_task(ctx, p.nseg, cap * wpb, 1, &score_pw);
-        const bool mostly_plain = obs_every == 0 || obs_every > 4;
-        if (ctx->variant == SHAKEN_VARIANT_PERWARP || score_pw * (mostly_plain ? 0.95 : 1.0) > score_block + 0.02) {
-            ctx->perwarp = true;
-            p.rows_per_task = Rpw;
-            wpb = 1;                                       // p.ntasks counts warp strips
-        }
-    }
     p.nrb = (ctx->L + p.rows_per_task - 1) / p.rows_per_task;
     // block tasks: wpb consecutive warp strips of one chain
     p.ntasks = (long long)ctx->n_chains * (((long long)p.nrb * p.nseg + wpb - 1) / wpb);
+    // many small chains: per-warp task lists (kernel_i8.cuh PERWARP).  Every warp gets a RANGE of the same number of
+    // consecutive strip-rows (a strip-row = one row of one 32-vector column strip of one chain), so the launch is one full
+    // wave whatever the chain size; a range is walked piece by piece, each piece paying the halo row and the two
+    // unprefetched rows of a strip start.  They cannot use the paired lookup, which is worth ~5 % on plain launches.
+    ctx->perwarp = false;
+    if (!ctx->packed && (ctx->variant == SHAKEN_VARIANT_PERWARP || ctx->n_chains > 1)) {
+        const long long S = (long long)ctx->n_chains * p.nseg * ctx->L;              // strip-rows per launch
+        const long long warps = cap * wpb;
+        long long waves = (S + warps * MAX_ROWS_PER_TASK - 1) / (warps * MAX_ROWS_PER_TASK);
+        long long n_ranges = warps * waves;
+        if (n_ranges > S) n_ranges = S;
+        const long long len = (S + n_ranges - 1) / n_ranges;
+        n_ranges = (S + len - 1) / len;
+        const long long waves_r = (n_ranges + warps - 1) / warps;
+        const double fill = (double)S / (double)(waves_r * warps * len);
+        const double pieces = 1.0 + (double)len / (double)ctx->L;                     // strip starts per range, on average
+        const double score_pw = fill * (double)len / ((double)len + 3.0 * pieces);
+        const bool mostly_plain = obs_every == 0 || obs_every > 4;
+        if (ctx->variant == SHAKEN_VARIANT_PERWARP || score_pw * (mostly_plain ? 0.95 : 1.0) > score_block + 0.02) {
+            ctx->perwarp = true;
+            p.rows_total = S;
+            p.range_len = (int)len;
+            p.ntasks = n_ranges;
+        }
+    }
 
     if (uniform) {
         kernel_table(J[0], q[0], p.utab);
@@ -963,7 +975,7 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
         if (br <= 0) return br;                                       // 0: done, < 0: error, 1: not applicable / refused
     }
 
-    const long long blocks_needed = ctx->perwarp ? (p.ntasks + I8_THREADS / 32 - 1) / (I8_THREADS / 32) : p.ntasks;
+    const long long blocks_needed = ctx->perwarp ? (p.ntasks + I8_THREADS / 32 - 1) / (I8_THREADS / 32) : p.ntasks;   // (ranges / warps per block)
     const int grid = (int)(blocks_needed < cap ? blocks_needed : cap);
     const size_t rec_stride = (size_t)ctx->n_chains * SHAKEN_N_OBS;
 
