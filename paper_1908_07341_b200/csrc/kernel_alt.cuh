@@ -529,7 +529,7 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) alt_band_i8(const __grid_cons
 {
     extern __shared__ __align__(16) uint32_t smem[];
     __shared__ __align__(256) uint32_t s_tab[ALT_TAB_WORDS];
-    __shared__ long long s_red[BAND_THREADS / 32][3];
+    __shared__ int s_acc[3];                      // the band's partial sums (M, C_x, C_y) of the record in progress
 
     const int L = p.L, W = L >> 2, nvec = W >> 2;
     const int band = blockIdx.x, chain = band / p.bpc, k = band - chain * p.bpc;
@@ -548,13 +548,15 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) alt_band_i8(const __grid_cons
         sg[i] = gs[(size_t)gr * W + cw];
     }
     if (tid < 8) s_tab[tid] = tid < 5 ? (p.gtab ? p.gtab[(size_t)chain * 8 + 4 - tid] : p.utab[4 - tid]) : 0u;   // entry i = A[4 - i]
+    if (tid < 3) s_acc[tid] = 0;
     __syncthreads();
     const uint32_t tb = shared_addr(s_tab);
 
     uint32_t xa2 = 0, xb0 = 0;
     ChainKeys ck = {0u, 0u};
     // one vector (16 sites, the 8 of the row's active parity redrawn) of row index j, in place
-    auto redraw = [&](const int half, const int j, const int v) -> uint4 {
+    int accM = 0, a1 = 0, ah = 0, av = 0;         // partial sums of a recorded step (see alt_vector_i8)
+    auto redraw = [&](const int half, const int j, const int v, const bool sums) -> uint4 {
         int gr = r0 - 2 + j;
         gr = gr < 0 ? gr + L : (gr >= L ? gr - L : gr);
         uint32_t *row = sg + j * W;
@@ -567,37 +569,18 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) alt_band_i8(const __grid_cons
         const uint32_t n0 = (uint32_t)gr * (uint32_t)(L >> 3) + 2u * (uint32_t)v;
         philox_site_words(n0, p.keys, xa2, xb0, ck, rnd);
         philox_site_words(n0 + 1u, p.keys, xa2, xb0, ck, rnd + 4);
-        int d0 = 0, d1 = 0, d2 = 0, d3 = 0;
-        const uint4 o = ((gr + half) & 1) ? alt_vector_i8<1, false>(cw, fu, fd, rnd, tb, d0, d1, d2, d3) : alt_vector_i8<0, false>(cw, fu, fd, rnd, tb, d0, d1, d2, d3);
+        uint4 o;
+        if (sums) o = ((gr + half) & 1) ? alt_vector_i8<1, true>(cw, fu, fd, rnd, tb, accM, a1, ah, av) : alt_vector_i8<0, true>(cw, fu, fd, rnd, tb, accM, a1, ah, av);
+        else o = ((gr + half) & 1) ? alt_vector_i8<1, false>(cw, fu, fd, rnd, tb, accM, a1, ah, av) : alt_vector_i8<0, false>(cw, fu, fd, rnd, tb, accM, a1, ah, av);
         *reinterpret_cast<uint4 *>(row + 4 * v) = o;
         return o;
     };
-    auto reduce_to = [&](long long *dst, const int (&v)[3], const int first, const int count, const int slot0) {
-#pragma unroll
-        for (int j = 0; j < 3; ++j) {
-            const int w = __reduce_add_sync(0xFFFFFFFFu, v[j]);
-            if (lane == 0) s_red[warp][j] = w;
-        }
-        __syncthreads();
-        if (tid < count) {
-            long long tot = 0;
-            for (int w = 0; w < BAND_THREADS / 32; ++w) tot += s_red[w][first + tid];
-            atomicAdd(reinterpret_cast<unsigned long long *>(dst + slot0 + (tid ? 3 + tid : 0)), (unsigned long long)tot);   // M, C_x, C_y sit at 0, 4, 5
-        }
-        __syncthreads();
-    };
-    // the part of C_y that waits for the neighbour: the band's bottom row against the neighbour's NEW top row (row index 1)
-    auto bond_y_edge = [&](long long *dst) {
-        int v[3] = {0, 0, 0};
-        for (int c = tid; c < W; c += BAND_THREADS) v[2] = __dp4a((int)sg[2 * W + c], (int)sg[W + c], v[2]);
-        reduce_to(dst, v, 2, 1, 5);
-    };
     // neighbours' rows of the step just finished: row indices 0, 1 from the band below, nr + 2, nr + 3 from the band above
-    auto collect = [&](const long long s_done, const bool only_below) {
+    auto collect = [&](const long long s_done) {
         const uint32_t stamp_in = p.stamp0 + (uint32_t)s_done;
         const uint2 *in_below = p.xtop + ((size_t)((s_done + 1) & 1) * nb + below) * 2 * W;
         const uint2 *in_above = p.xbot + ((size_t)((s_done + 1) & 1) * nb + above) * 2 * W;
-        for (int i = tid; i < (only_below ? 2 : 4) * W; i += BAND_THREADS) {
+        for (int i = tid; i < 4 * W; i += BAND_THREADS) {
             const uint2 *src = i < 2 * W ? in_below + i : in_above + (i - 2 * W);
             uint2 a;
             do { a = ld_pair(src); } while (a.y != stamp_in);
@@ -605,12 +588,13 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) alt_band_i8(const __grid_cons
         }
     };
 
-    long long *pending = nullptr;
     long long nrec = 0;
     long long until_rec = p.obs_every > 0 ? p.obs_every - (long long)(p.t0 % (unsigned long long)p.obs_every) : 0;
 #pragma unroll 1
     for (long long s = 0; s < p.n_steps; ++s) {
         const unsigned long long t = p.t0 + (unsigned long long)s;
+        const bool rec = p.obs_every > 0 && --until_rec == 0;            // block-uniform
+        if (rec) until_rec = p.obs_every;
         // half-step 0: colour 0 of row indices 1 .. nr + 2 (the band and one halo row on either side).  First the rows
         // that read only the band's own rows (indices 3 .. nr), then the neighbours' rows of the previous step are
         // collected -- they were published early in the neighbours' half-step 1 and have had all that time to arrive --
@@ -619,19 +603,21 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) alt_band_i8(const __grid_cons
 #pragma unroll 1
         for (int c = tid; c < (nr - 2) * nvec; c += BAND_THREADS) {
             const int kk = (int)__umulhi((uint32_t)c, p.magicV);
-            redraw(0, 3 + kk, c - kk * nvec);
+            redraw(0, 3 + kk, c - kk * nvec, false);
         }
-        if (s > 0) collect(s, false);
+        if (s > 0) collect(s);
         __syncthreads();
-        if (pending) { bond_y_edge(pending); pending = nullptr; }
 #pragma unroll 1
         for (int c = tid; c < 4 * nvec; c += BAND_THREADS) {
             const int kk = (int)__umulhi((uint32_t)c, p.magicV);
-            redraw(0, kk < 2 ? 1 + kk : nr - 1 + kk, c - kk * nvec);
+            redraw(0, kk < 2 ? 1 + kk : nr - 1 + kk, c - kk * nvec, false);
         }
         __syncthreads();
         // half-step 1: colour 1 of the band's rows (indices 2 .. nr + 1); the two top rows and the two bottom rows first,
-        // each vector published by the thread that computed it
+        // each vector published by the thread that computed it.  On a recorded step the sums are fused in: every bond of
+        // the lattice joins a site redrawn here to a passive one (final since half-step 0, also in the halo rows), so
+        // M = sum of the stored vectors, C_x = sum_{x redrawn} s_x (left + right), C_y = sum_{x redrawn} s_x (up + down),
+        // each bond counted once, by the band that owns its redrawn end -- no neighbour row is waited for.
         device_half_step_keys(p.keys, 2ull * t + 1ull, p.chain0 + (uint32_t)chain, xa2, xb0, ck);
         const uint32_t stamp_out = p.stamp0 + (uint32_t)s + 1u;
         uint2 *out_top = p.xtop + ((size_t)(s & 1) * nb + band) * 2 * W;   // rows r1-2, r1-1
@@ -640,7 +626,7 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) alt_band_i8(const __grid_cons
         for (int c = tid; c < nr * nvec; c += BAND_THREADS) {
             const int kk = (int)__umulhi((uint32_t)c, p.magicV), v = c - kk * nvec;
             const int j = kk == 0 ? nr + 1 : (kk == 1 ? nr : kk);              // row index: nr+1, nr, 2, 3, 4 .. nr-1
-            const uint4 o = redraw(1, j, v);
+            const uint4 o = redraw(1, j, v, rec);
             if (j >= nr) {
                 uint2 *x = out_top + (j - nr) * W + 4 * v;
                 st_pair(x, o.x, stamp_out); st_pair(x + 1, o.y, stamp_out); st_pair(x + 2, o.z, stamp_out); st_pair(x + 3, o.w, stamp_out);
@@ -650,29 +636,22 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) alt_band_i8(const __grid_cons
                 st_pair(x, o.x, stamp_out); st_pair(x + 1, o.y, stamp_out); st_pair(x + 2, o.z, stamp_out); st_pair(x + 3, o.w, stamp_out);
             }
         }
+        if (rec) {
+            // s * (l + r) = s * (2 - 2 * minus) per site: ah, av hold 4 * minus, so they are multiples of 4 (see alt_half)
+            const int w0 = __reduce_add_sync(0xFFFFFFFFu, accM), w1 = __reduce_add_sync(0xFFFFFFFFu, 2 * a1 - ah / 2),
+                      w2 = __reduce_add_sync(0xFFFFFFFFu, 2 * a1 - av / 2);
+            if (lane == 0) { atomicAdd(&s_acc[0], w0); atomicAdd(&s_acc[1], w1); atomicAdd(&s_acc[2], w2); }
+            accM = a1 = ah = av = 0;
+        }
         __syncthreads();
-        // record (M, 0, 0, 0, C_x, C_y): M and C_x now, C_y once the neighbour's new top row has been collected
-        if (p.obs_every > 0 && --until_rec == 0) {
-            until_rec = p.obs_every;
-            long long *dst = p.rec + ((size_t)nrec * p.n_chains + chain) * 6;
-            int v[3] = {0, 0, 0};
-            for (int c = tid; c < nr * W; c += BAND_THREADS) {
-                const int r = (int)__umulhi((uint32_t)c, p.magicW), cw = c - r * W;
-                const uint32_t *row = sg + (2 + r) * W;
-                const uint32_t s0 = row[cw];
-                v[0] = __dp4a((int)s0, 0x01010101, v[0]);
-                v[1] = __dp4a((int)s0, (int)__funnelshift_r(s0, row[cw == W - 1 ? 0 : cw + 1], 8), v[1]);   // sigma_x sigma_{x right}
-                if (r > 0) v[2] = __dp4a((int)s0, (int)row[cw - W], v[2]);                                  // sigma_x sigma_{x down} inside the band
+        if (rec) {
+            if (tid < 3) {
+                long long *dst = p.rec + ((size_t)nrec * p.n_chains + chain) * 6;
+                atomicAdd(reinterpret_cast<unsigned long long *>(dst + (tid ? 3 + tid : 0)), (unsigned long long)(long long)s_acc[tid]);   // M, C_x, C_y at 0, 4, 5
+                s_acc[tid] = 0;                   // next written after at least one more block barrier
             }
-            reduce_to(dst, v, 0, 3, 0);
-            pending = dst;
             ++nrec;
         }
-    }
-    if (pending) {
-        collect(p.n_steps, true);
-        __syncthreads();
-        bond_y_edge(pending);
     }
     for (int i = tid; i < nr * W; i += BAND_THREADS) gs[(size_t)r0 * W + i] = sg[2 * W + i];
 }

@@ -17,6 +17,8 @@
 // for each other, which is why all CTAs must be co-resident -- the cooperative launch guarantees it.
 // Site -> random word mapping, thresholds and rule are those of kernel_i8.cuh; only the schedule differs.
 #pragma once
+#include <type_traits>
+
 #include "kernels_common.cuh"
 
 namespace shaken {
@@ -81,6 +83,7 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) band_run_i8(const __grid_cons
     extern __shared__ __align__(16) uint32_t smem[];
     __shared__ uint2 s_pair[64][32];              // paired thresholds, lane-replicated (see kernel_i8.cuh)
     __shared__ long long s_red[BAND_THREADS / 32][6];
+    __shared__ int s_acc[6];                      // the band's partial sums of the record in progress
 
     const int L = p.L, W = L >> 2;
     const int band = blockIdx.x, chain = band / p.bpc, k = band - chain * p.bpc;
@@ -113,6 +116,7 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) band_run_i8(const __grid_cons
         }
         s_pair[e][t & 31] = make_uint2(T2[0], T2[1]);
     }
+    if (tid < 6) s_acc[tid] = 0;
     __syncthreads();
 
     uint32_t xa2 = 0, xb0 = 0;
@@ -208,9 +212,28 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) band_run_i8(const __grid_cons
     long long nrec = 0;
     // full steps until the next recorded one: a countdown instead of a 64-bit modulo per step
     long long until_rec = p.obs_every > 0 ? p.obs_every - (long long)(p.t0 % (unsigned long long)p.obs_every) : 0;
+    // The sums of a recorded step are taken where their operands are in registers anyway: M_sigma, M_tau, E_J, E_q in the
+    // half-step 1 that produces the recorded sigma, C_x and C_y in the NEXT half-step 0, which reads that sigma together
+    // with its left and down neighbours (incl. the neighbour band's new row).  Per-thread int partials -> warp sum ->
+    // shared-memory atomics; after the block barrier that ends the half-step anyway, six threads add the band's totals to
+    // the record (int64 atomics: the bands of a chain share it).  No extra pass, no extra barrier.
+    auto add_partials = [&](const int (&v)[6], const int first, const int count) {
+        for (int j = first; j < first + count; ++j) {
+            const int w = __reduce_add_sync(0xFFFFFFFFu, v[j]);
+            if (lane == 0 && w != 0) atomicAdd(&s_acc[j], w);
+        }
+    };
+    auto flush_partials = [&](long long *dst, const int first, const int count) {     // right after a block barrier
+        if (tid >= first && tid < first + count) {
+            atomicAdd(reinterpret_cast<unsigned long long *>(dst + tid), (unsigned long long)(long long)s_acc[tid]);
+            s_acc[tid] = 0;                       // next written after at least one more block barrier
+        }
+    };
 #pragma unroll 1
     for (long long s = 0; s < p.n_steps; ++s) {
         const unsigned long long t = p.t0 + (unsigned long long)s;
+        const bool rec = p.obs_every > 0 && --until_rec == 0;                        // block-uniform
+        if (rec) until_rec = p.obs_every;
         // hand-over buffers: the rows published after step s-1 (parity (s-1) & 1) are read now
         const uint32_t stamp_in = p.stamp0 + (uint32_t)s;
         const uint2 *in_below = p.xtop + ((size_t)((s + 1) & 1) * nb + below) * W;   // top row of the band below = row r0-1
@@ -221,6 +244,7 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) band_run_i8(const __grid_cons
         // row above the band): those two wait for the neighbours' rows of the previous step (none on the first step of a
         // launch: the halo rows came from global memory).
         device_half_step_keys(p.keys, 2ull * t, p.chain0 + (uint32_t)chain, xa2, xb0, ck);
+        int v[6] = {0, 0, 0, 0, 0, 0};
 #pragma unroll 1
         for (int c = tid; c < n0; c += BAND_THREADS) {
             const int kk = (int)__umulhi((uint32_t)c, p.magicV), cv = c - kk * nvec;
@@ -229,7 +253,8 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) band_run_i8(const __grid_cons
             int gr = r0 + i;
             if (gr >= L) gr -= L;
             const uint32_t n = (uint32_t)gr * (uint32_t)W + 4u * (uint32_t)cv;
-            uint4 o;
+            uint4 o, s4, v4;
+            uint32_t e;
             if (s > 0 && i == 0) {
                 // vertical neighbours from the band below, straight from the hand-over buffer; random words first
                 uint32_t R[4][4];
@@ -237,9 +262,11 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) band_run_i8(const __grid_cons
                 uint2 a, b, c2, d;
                 do { ld_pairs2(in_below + 4 * cv, a, b); ld_pairs2(in_below + 4 * cv + 2, c2, d); }
                 while (a.y != stamp_in || b.y != stamp_in || c2.y != stamp_in || d.y != stamp_in);
-                const uint4 v4 = make_uint4(a.x, b.x, c2.x, d.x);
-                *reinterpret_cast<uint4 *>(sg + 4 * cv) = v4;                  // kept for the bond sums of a recorded step
-                o = apply0(*reinterpret_cast<const uint4 *>(self + 4 * cv), v4, self[cv == 0 ? W - 1 : 4 * cv - 1], R);
+                v4 = make_uint4(a.x, b.x, c2.x, d.x);
+                *reinterpret_cast<uint4 *>(sg + 4 * cv) = v4;                  // (row index 0 of sg mirrors the row below the band)
+                s4 = *reinterpret_cast<const uint4 *>(self + 4 * cv);
+                e = self[cv == 0 ? W - 1 : 4 * cv - 1];
+                o = apply0(s4, v4, e, R);
             } else if (s > 0 && i == nr) {
                 // the row above the band: own words and the left edge spin from the band above; random words first
                 uint32_t R[4][4];
@@ -248,15 +275,30 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) band_run_i8(const __grid_cons
                 const uint2 *pe = in_above + (cv == 0 ? W - 1 : 4 * cv - 1);
                 do { ld_pairs2(in_above + 4 * cv, a, b); ld_pairs2(in_above + 4 * cv + 2, c2, d); ee = ld_pair(pe); }
                 while (a.y != stamp_in || b.y != stamp_in || c2.y != stamp_in || d.y != stamp_in || ee.y != stamp_in);
-                o = apply0(make_uint4(a.x, b.x, c2.x, d.x), *reinterpret_cast<const uint4 *>(downr + 4 * cv), ee.x, R);
+                s4 = make_uint4(a.x, b.x, c2.x, d.x);
+                v4 = *reinterpret_cast<const uint4 *>(downr + 4 * cv);
+                e = ee.x;
+                o = apply0(s4, v4, e, R);
             } else {
-                o = update_vector(0, *reinterpret_cast<const uint4 *>(self + 4 * cv), *reinterpret_cast<const uint4 *>(downr + 4 * cv),
-                                  self[cv == 0 ? W - 1 : 4 * cv - 1], n);
+                s4 = *reinterpret_cast<const uint4 *>(self + 4 * cv);
+                v4 = *reinterpret_cast<const uint4 *>(downr + 4 * cv);
+                e = self[cv == 0 ? W - 1 : 4 * cv - 1];
+                o = update_vector(0, s4, v4, e, n);
             }
             *reinterpret_cast<uint4 *>(ta + i * W + 4 * cv) = o;
+            if (__builtin_expect(pending != nullptr, 0) && i < nr) {
+                // C_x, C_y of the record taken after the previous step: sigma_x sigma_{x left}, sigma_x sigma_{x down}
+                const uint32_t w[4] = {s4.x, s4.y, s4.z, s4.w}, dw[4] = {v4.x, v4.y, v4.z, v4.w};
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    v[4] = __dp4a((int)w[j], (int)__funnelshift_l(j == 0 ? e : w[j - 1], w[j], 8), v[4]);
+                    v[5] = __dp4a((int)w[j], (int)dw[j], v[5]);
+                }
+            }
         }
+        if (pending) add_partials(v, 4, 2);
         __syncthreads();
-        if (pending) { bond_sums(pending); pending = nullptr; }   // (two more barriers, only after a recorded step)
+        if (pending) { flush_partials(pending, 4, 2); pending = nullptr; }
 
         // ---- half-step 1: sigma <- tau, up and right neighbours (eq. (16)); rows 0 .. nr-1.  Order: the top row and the
         // bottom row first -- the neighbours wait for them -- each vector published by the thread that computed it.
@@ -276,26 +318,24 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) band_run_i8(const __grid_cons
             *reinterpret_cast<uint4 *>(sg + (i + 1) * W + 4 * cv) = o;
             if (i == nr - 1) { st_pairs2(out_top + 4 * cv, o.x, o.y, stamp_out); st_pairs2(out_top + 4 * cv + 2, o.z, o.w, stamp_out); }
             if (i == 0) { st_pairs2(out_bot + 4 * cv, o.x, o.y, stamp_out); st_pairs2(out_bot + 4 * cv + 2, o.z, o.w, stamp_out); }
-        }
-        __syncthreads();
-
-        // record (M_sigma, M_tau, E_J, E_q now; C_x, C_y once the new sigma row below the band has arrived)
-        if (p.obs_every > 0 && --until_rec == 0) {
-            until_rec = p.obs_every;
-            long long *dst = p.rec + ((size_t)nrec * p.n_chains + chain) * 6;
-            int v[6] = {0, 0, 0, 0, 0, 0};
-            for (int c = tid; c < nr * W; c += BAND_THREADS) {
-                const int r = (int)__umulhi((uint32_t)c, p.magicW), cw = c - r * W;
-                const uint32_t s0 = sg[W + c], t0w = ta[c];
-                const uint32_t tu = ta[c + W];                                  // row nr of ta is the redrawn row above the band
-                const uint32_t tr = __funnelshift_r(t0w, ta[r * W + (cw == W - 1 ? 0 : cw + 1)], 8);
-                v[0] = __dp4a((int)s0, 0x01010101, v[0]);
-                v[1] = __dp4a((int)t0w, 0x01010101, v[1]);
-                v[2] = __dp4a((int)s0, (int)tu, v[2]);
-                v[2] = __dp4a((int)s0, (int)tr, v[2]);
-                v[3] = __dp4a((int)s0, (int)t0w, v[3]);
+            if (__builtin_expect(rec, 0)) {
+                // M_sigma, M_tau, E_J = sigma'_x (tau_{x up} + tau_{x right}), E_q = sigma'_x tau_x  (row nr of ta is the redrawn row above the band)
+                const uint32_t ow[4] = {o.x, o.y, o.z, o.w}, tw[4] = {s4.x, s4.y, s4.z, s4.w}, uw[4] = {v4.x, v4.y, v4.z, v4.w};
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    v[0] = __dp4a((int)ow[j], 0x01010101, v[0]);
+                    v[1] = __dp4a((int)tw[j], 0x01010101, v[1]);
+                    v[2] = __dp4a((int)ow[j], (int)uw[j], v[2]);
+                    v[2] = __dp4a((int)ow[j], (int)__funnelshift_r(tw[j], j == 3 ? e : tw[j + 1], 8), v[2]);
+                    v[3] = __dp4a((int)ow[j], (int)tw[j], v[3]);
+                }
             }
-            reduce_to(dst, v, 0, 4);
+        }
+        if (rec) add_partials(v, 0, 4);
+        __syncthreads();
+        if (rec) {
+            long long *dst = p.rec + ((size_t)nrec * p.n_chains + chain) * 6;
+            flush_partials(dst, 0, 4);
             pending = dst;
             ++nrec;
         }
