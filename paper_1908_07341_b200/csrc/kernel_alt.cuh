@@ -538,7 +538,7 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) alt_band_i8(const __grid_cons
     const int below = chain * p.bpc + (k == 0 ? p.bpc - 1 : k - 1);
     const int above = chain * p.bpc + (k == p.bpc - 1 ? 0 : k + 1);
     const int nb = gridDim.x;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int tid = threadIdx.x, lane = tid & 31;
     uint32_t *sg = smem;                          // row index j holds global row r0 - 2 + j (mod L), j = 0 .. nr + 3
     uint32_t *gs = reinterpret_cast<uint32_t *>(p.sigma + (size_t)chain * L * L);
     for (int i = tid; i < (nr + 4) * W; i += BAND_THREADS) {
