@@ -5,6 +5,7 @@
 #include "kernel_i8.cuh"
 #include "kernel_pk.cuh"
 #include "kernel_small.cuh"
+#include "kernel_cluster.cuh"
 #include "kernel_band.cuh"
 #include "kernel_alt.cuh"
 #include "kernel_slab.cuh"

@@ -40,6 +40,7 @@ struct shaken_ctx {
     size_t xch_bytes = 0;
     uint32_t xch_stamp = 0;       // last stamp written into d_xch
     int coop = -1;                // cooperative launch supported (-1: not queried yet)
+    bool no_cluster = false;      // a cluster launch failed once: small chains stay on one SM each
     bool band_refuse_next = false;   // test hook: treat the next cooperative launch as refused (exercises the fall-back)
     void *d_stage = nullptr;      // staging for packed <-> int8 conversion
     size_t stage_bytes = 0;
@@ -934,6 +935,52 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
     const bool small_path = !ctx->packed && ctx->variant == 0 && ctx->group <= SMALL_GROUP_MAX &&
                             small_smem_bytes(ctx->L, ctx->group) <= 200 * 1024 &&
                             (ctx->L <= SMALL_L_MAX || (ctx->L <= SMALL_L_BATCH_MAX && 2 * (ctx->n_chains / ctx->group) >= ctx->num_sms));
+    // A few small chains: one chain per CLUSTER of 8 SMs (kernel_cluster.cuh) instead of one per SM -- rows in the shared
+    // memory of 8 CTAs, the neighbour's row read through distributed shared memory, a cluster barrier per half-step.
+    const bool cluster_path = small_path && ctx->group == 1 && ctx->L >= 32 && ctx->L <= SMALL_L_MAX && !ctx->no_cluster &&
+                              (long long)ctx->n_chains * CLUSTER_CTAS <= ctx->num_sms;
+    if (cluster_path) {
+        SmallParams sp;
+        memset(&sp, 0, sizeof(sp));
+        sp.sigma = (uint8_t *)ctx->d_sigma;
+        sp.tau = (uint8_t *)ctx->d_tau;
+        sp.L = ctx->L;
+        sp.n_chains = ctx->n_chains;
+        sp.group = 1;
+        sp.chain0 = ctx->chain0;
+        sp.t0 = ctx->step;
+        sp.n_steps = n_steps;
+        sp.obs_every = obs_every;
+        sp.rec = ctx->d_rec ? ctx->d_rec + (size_t)ctx->n_rec * ctx->n_chains * SHAKEN_N_OBS : nullptr;
+        sp.gtab = p.gtab;
+        memcpy(sp.utab, p.utab, sizeof(sp.utab));
+        make_step_keys(ctx->seed, 0, sp.keys);
+        const int nwords = (ctx->L / CLUSTER_CTAS) * (ctx->L / 4);
+        const int threads = nwords >= 512 ? 512 : ((nwords + 31) / 32) * 32;
+        cudaLaunchConfig_t cfg;
+        memset(&cfg, 0, sizeof(cfg));
+        cfg.gridDim = dim3((unsigned)(ctx->n_chains * CLUSTER_CTAS));
+        cfg.blockDim = dim3((unsigned)threads);
+        cfg.dynamicSmemBytes = cluster_smem_bytes(ctx->L);
+        cfg.stream = ctx->stream;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = CLUSTER_CTAS;
+        attr[0].val.clusterDim.y = 1;
+        attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        const cudaError_t le = cudaLaunchKernelEx(&cfg, cluster_run_i8, sp);
+        if (le == cudaSuccess) {
+            ctx->launches++;
+            ctx->step += (uint64_t)n_steps;
+            ctx->n_rec += n_new;
+            ctx->have_tau = true;
+            return SHAKEN_OK;
+        }
+        cudaGetLastError();
+        ctx->no_cluster = true;                   // (a device or partition that cannot co-schedule the cluster: one chain per SM instead)
+    }
     if (small_path) {
         SmallParams sp;
         memset(&sp, 0, sizeof(sp));

@@ -316,6 +316,29 @@ def test_small_lattice_path_and_generic_kernels_both_match_oracle(L, n_chains):
             assert_same_state(s, o, f"L={L} variant={variant}")
 
 
+@pytest.mark.parametrize("L,n_chains", [(32, 1), (64, 1), (80, 3), (128, 1), (128, 18), (64, 19)])
+def test_cluster_path_for_few_small_chains_and_one_sm_path_for_many(L, n_chains):
+    """Up to 18 small chains (L >= 32) run one chain per CLUSTER of 8 SMs (kernel_cluster.cuh: rows in the shared memory of 8
+    CTAs, neighbour rows through distributed shared memory, fused sums); from 19 chains on one chain per SM
+    (kernel_small.cuh).  Per-chain couplings, records on some steps only and on every step, split runs, a record on the very
+    last step of a call (its C_x, C_y are closed from the final sigma)."""
+    seed = 300 + L + n_chains
+    J = np.linspace(0.3, 0.8, n_chains)
+    q = np.linspace(1.1, 0.2, n_chains)
+    for obs in (1, 3):
+        o = so.Oracle(L, n_chains, seed)
+        o.init(0)
+        o.run_grid(J, q, 12, obs)
+        with shaken.Shaken(L, n_chains, seed, max_records=16) as s:
+            s.init(0)
+            l0 = s.launch_count
+            s.run_grid(J, q, 5, obs)
+            s.run_grid(J, q, 4, obs)
+            s.run_grid(J, q, 3, obs)
+            assert s.launch_count - l0 == 3
+            assert_same_state(s, o, f"L={L} chains={n_chains} obs={obs}")
+
+
 @pytest.mark.parametrize("variant", [0, 3, 8])
 def test_every_int8_code_path_matches_oracle_on_a_ragged_lattice(variant):
     """L = 272: 17 vectors per row (ragged warp strip), several row blocks per chain, three chains with different
