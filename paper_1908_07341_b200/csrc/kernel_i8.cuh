@@ -2,7 +2,7 @@
 //
 // Spins are bytes 0x01 (+1) / 0xFF (-1): bit 0 is always 1 and every bit 1..7 of a byte is the "minus" flag m.
 //
-// Pipe budget on sm_100a (measured, profiles/r2_pipe_rates.md): a 32x32->64 multiply (IMAD.WIDE) holds the 16-lane
+// Pipe budget on sm_100a (measured, DESIGN.md Appendix A): a 32x32->64 multiply (IMAD.WIDE) holds the 16-lane
 // multiplier pipe of an SM sub-partition for 4.2 cycles per warp, so the 17-18 multiplies of one hoisted Philox call
 // (4 sites) alone cap the kernel near 7 site-updates per clock per SM.  Everything else is therefore kept OFF that
 // pipe where possible: field/index arithmetic is byte-SIMD logic on the ALU pipe (4 sites per instruction), the
