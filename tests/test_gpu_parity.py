@@ -419,6 +419,28 @@ def test_band_kernel_sweep_of_shapes_matches_oracle(L, n_chains, steps, obs):
         assert_same_state(s, o, f"L={L} chains={n_chains}")
 
 
+@pytest.mark.parametrize("L,n_chains,packed,variant,steps,obs", [
+    (16, 7, False, 8, 6, 1), (48, 5, False, 8, 5, 2), (144, 4, False, 8, 5, 1), (528, 3, False, 8, 4, 1), (1040, 2, False, 8, 3, 0),
+    (272, 6, False, 3, 5, 3), (1040, 1, False, 3, 4, 1), (96, 9, False, 3, 4, 1),
+    (64, 5, True, 0, 6, 1), (544, 2, True, 0, 4, 2), (1056, 3, True, 0, 3, 1)])
+def test_strip_kernels_sweep_of_shapes_matches_oracle(L, n_chains, packed, variant, steps, obs):
+    """The per-half-step strip kernels over a sweep of shapes: per-warp ranges that cross chain boundaries (rows narrower and
+    wider than a warp strip, ragged last ranges), block tasks, the packed layout; per-chain couplings, every record cadence,
+    each run split in two."""
+    seed = 2000 + L + 7 * n_chains
+    J = np.linspace(0.25, 0.85, n_chains)
+    q = np.linspace(1.0, 0.15, n_chains)
+    o = so.Oracle(L, n_chains, seed)
+    o.init(0)
+    o.run_grid(J, q, steps, obs)
+    with shaken.Shaken(L, n_chains, seed, packed=packed, max_records=steps) as s:
+        s.set_variant(variant)
+        s.init(0)
+        s.run_grid(J, q, steps - steps // 2, obs)
+        s.run_grid(J, q, steps // 2, obs)
+        assert_same_state(s, o, f"L={L} chains={n_chains} packed={packed} variant={variant}")
+
+
 # ----------------------------------------------------------------------------- coupled chains, coalescence (SURVEY 8(f) rank 1)
 @pytest.mark.parametrize("packed,variant", [(False, 0), (False, 3), (True, 0)])
 def test_coupled_chains_and_coalescence_times_match_oracle(packed, variant):
