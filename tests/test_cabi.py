@@ -68,6 +68,27 @@ COUPLINGS = [(0.5, 0.5), (0.6585, 0.6585), (0.7, 0.7), (0.45, 10.0), (0.44, 0.66
              (0.0, 1.0), (1.0, 0.0), (-0.3, 0.4), (2.0, 0.03)]
 
 
+def test_slab_and_hook_arguments_are_validated_without_a_device():
+    lib = shaken.lib()
+    h = C.c_void_p()
+    for L, row0, n in [(24, 0, 8), (64, -1, 8), (64, 0, 1), (64, 60, 8), (65552, 0, 8)]:
+        assert lib.shaken_create_slab(C.byref(h), L, row0, n, 1) == shaken.EINVAL, (L, row0, n)
+        assert not h.value
+    assert lib.shaken_create_slab(C.byref(h), 64, 16, 32, 1) == 0
+    assert lib.shaken_spin_bytes(h) == 32 * 64                      # the slab's own rows
+    assert lib.shaken_record_bytes(h) == 6 * 8
+    assert lib.shaken_bind(h, C.c_void_p(16), C.c_void_p(32), None, 0, None) == shaken.ESTATE   # a slab owns its buffers
+    assert lib.shaken_run(h, 0.5, 0.5, 1, 0) == shaken.ESTATE       # no sigma yet
+    assert lib.shaken_run_alternate(h, 0.5, 1, 0) == shaken.ESTATE
+    assert lib.shaken_slab_connect(h, None, None) == shaken.EINVAL
+    assert lib.shaken_test_band_hook(h, 7, 0) == shaken.EINVAL
+    assert lib.shaken_destroy(h) == 0
+    assert lib.shaken_create(C.byref(h), 64, 1, 1, 0) == 0
+    assert lib.shaken_slab_exchange(h) == shaken.EINVAL             # not a slab context
+    assert lib.shaken_slab_connect(h, C.c_void_p(16), C.c_void_p(16)) == shaken.EINVAL
+    assert lib.shaken_destroy(h) == 0
+
+
 def test_library_threshold_table_against_exact_decimal_arithmetic():
     """The library's own host table (not the oracle's) against 60-digit decimal evaluation of
     round(2^32 e^h / (2 cosh h)) -- same pin as the oracle's, applied independently."""
