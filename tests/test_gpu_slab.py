@@ -122,3 +122,62 @@ def test_bench_two_ranks_under_torchrun(extra):
     line = json.loads([ln for ln in out.stdout.splitlines() if ln.startswith("{")][-1])
     assert line["n_gpus"] == 2 and line["value"] > 0
     assert line["scaling"] == ("strong" if extra else "weak")
+
+
+def _ipc_worker(rank, world, L, seed, steps, J, q, barrier, handles, results):
+    """One slab per PROCESS, both on cuda:0, inboxes connected through CUDA IPC handles.  Host barriers around every step
+    make sure a rank's rows are published (and the stream drained) before the other rank's kernels look for them, so no
+    kernel ever waits for a kernel of the other process; what is exercised is the IPC mapping and the peer stores."""
+    import numpy as np
+    import torch
+
+    from paper_1908_07341_b200 import parallel, shaken
+
+    torch.cuda.set_device(0)
+    s = parallel.open_slab(L, seed, world, rank, max_records=steps)
+    try:
+        handles[rank] = s.ipc_export()
+        barrier.wait()
+        below, above = parallel.slab_neighbours(world, rank)
+        s.ipc_connect(bytes(handles[below]), bytes(handles[above]))
+        s.init(0)
+        for _ in range(steps):
+            s.exchange()
+            s.synchronize()
+            barrier.wait()
+            s.run(J, q, 1, 1)
+            s.synchronize()
+            barrier.wait()
+        s.exchange()
+        s.synchronize()
+        barrier.wait()
+        results[rank] = (s.get_spins(0).copy(), s.observables().copy())
+        barrier.wait()                                   # nobody unmaps while the neighbour may still be reading
+    finally:
+        s.close()
+
+
+def test_two_processes_exchange_slab_rows_through_cuda_ipc():
+    import torch.multiprocessing as mp
+
+    L, seed, steps, J, q = 272, 31, 4, 0.6, 0.5
+    ctx = mp.get_context("spawn")
+    mgr = ctx.Manager()
+    handles, results = mgr.dict(), mgr.dict()
+    barrier = ctx.Barrier(2)
+    procs = [ctx.Process(target=_ipc_worker, args=(r, 2, L, seed, steps, J, q, barrier, handles, results)) for r in range(2)]
+    for p in procs:
+        p.start()
+    for p in procs:
+        p.join(timeout=180)
+    alive = [p for p in procs if p.is_alive()]
+    for p in alive:
+        p.kill()
+    assert not alive, "a slab process did not finish"
+    assert all(p.exitcode == 0 for p in procs), [p.exitcode for p in procs]
+    o = so.Oracle(L, 1, seed)
+    o.init(0)
+    o.run(J, q, steps, 1)
+    sigma = np.vstack([results[0][0], results[1][0]])
+    assert np.array_equal(sigma, o.get_spins(0)[0]), "sigma differs"
+    assert np.array_equal(results[0][1] + results[1][1], o.observables()), "summed records differ"
