@@ -150,3 +150,33 @@ def test_derived_stats_exact_small_case_and_large_values():
     assert abs(st["m4"] - 1.0) < 1e-8 and abs(st["abs_m"] - 1.0) < 1e-8
     assert abs(st["binder"] - 2.0 / 3.0) < 1e-8
     assert shaken.energy(0.5, 2.0, 10, -3) == -(0.5 * 10 + 2.0 * -3)
+
+
+def test_header_compiles_as_c99_and_a_c_caller_links(tmp_path):
+    """include/shaken.h is a C header (no C++ types): a C99 program that includes it compiles with -pedantic, links against
+    libshaken.so and gets the host-side results (thresholds, moments) without a device."""
+    import shutil
+    import subprocess
+
+    gcc = shutil.which("gcc")
+    if gcc is None:
+        pytest.skip("gcc not found")
+    src = tmp_path / "caller.c"
+    src.write_text("""
+#include "shaken.h"
+#include <stdio.h>
+int main(void) {
+    uint32_t t[6]; double m[SHAKEN_N_MOMENTS]; int64_t M[3] = {4, -4, 0};
+    if (shaken_thresholds(0.0, 0.0, t) != SHAKEN_OK) return 1;
+    if (shaken_moments(M, 3, 1, 16, m) != SHAKEN_OK) return 2;
+    printf("%u %.6f %.6f\n", t[0], m[2], m[5]);
+    return 0;
+}
+""")
+    exe = tmp_path / "caller"
+    libdir = os.path.dirname(shaken.LIB_PATH)
+    subprocess.check_call([gcc, "-std=c99", "-Wall", "-Wextra", "-pedantic", "-Werror", "-I", os.path.join(ROOT, "include"), str(src), "-o", str(exe),
+                           "-L", libdir, "-l:libshaken.so", f"-Wl,-rpath,{libdir}"])
+    out = subprocess.run([str(exe)], capture_output=True, text=True, check=True).stdout.split()
+    assert out[0] == str(2**31)                     # T(0) = 2^31
+    assert abs(float(out[1]) - (32 / 3) / 256) < 1e-6 and abs(float(out[2]) - 0.5) < 1e-6
