@@ -169,7 +169,7 @@ int main(void) {
     uint32_t t[6]; double m[SHAKEN_N_MOMENTS]; int64_t M[3] = {4, -4, 0};
     if (shaken_thresholds(0.0, 0.0, t) != SHAKEN_OK) return 1;
     if (shaken_moments(M, 3, 1, 16, m) != SHAKEN_OK) return 2;
-    printf("%u %.6f %.6f\n", t[0], m[2], m[5]);
+    printf("%u %.6f %.6f\\n", t[0], m[2], m[5]);
     return 0;
 }
 """)
