@@ -441,6 +441,28 @@ def test_strip_kernels_sweep_of_shapes_matches_oracle(L, n_chains, packed, varia
         assert_same_state(s, o, f"L={L} chains={n_chains} packed={packed} variant={variant}")
 
 
+@pytest.mark.parametrize("L,n_chains", [(64, 1), (128, 3), (272, 2), (1024, 1), (48, 30)])
+def test_single_step_calls_with_a_record_on_every_step(L, n_chains):
+    """shaken_run(1) over and over with a record each time: every call is one launch of a one-launch kernel (cluster, band
+    or one-SM) whose only step is recorded, so its C_x, C_y are always closed by the end-of-launch path; interleaved with
+    shaken_run_alternate(1) on the same context."""
+    seed = 600 + L
+    J = np.linspace(0.4, 0.8, n_chains)
+    q = np.linspace(0.7, 0.3, n_chains)
+    o = so.Oracle(L, n_chains, seed)
+    o.init(0)
+    with shaken.Shaken(L, n_chains, seed, max_records=16) as s:
+        s.init(0)
+        for k in range(6):
+            if k % 3 == 2:
+                o.run_alternate(J, 1, 1)
+                s.run_alternate(J, 1, 1)
+            else:
+                o.run_grid(J, q, 1, 1)
+                s.run_grid(J, q, 1, 1)
+        assert_same_state(s, o, f"L={L} chains={n_chains}")
+
+
 # ----------------------------------------------------------------------------- coupled chains, coalescence (SURVEY 8(f) rank 1)
 @pytest.mark.parametrize("packed,variant", [(False, 0), (False, 3), (True, 0)])
 def test_coupled_chains_and_coalescence_times_match_oracle(packed, variant):
