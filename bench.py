@@ -482,7 +482,7 @@ def run_ours(args):
                                                     "from the committed ncu --set full capture of this kernel (not measured in this run)",
                 "peak_source": peak_src, "kernel": kernel,
                 "algorithmic_bytes_per_launch": rl["alg_bytes_per_launch"], "avg_launch_us": rl["avg_launch_us"],
-                "binding_resource": "integer multiplier pipe (Philox4x32-10, 32 random bits per site), not HBM",
+                "binding_resource": "integer pipes, not HBM: the ALU/dispatch port (83-85 % busy) ahead of the multiplier pipe (76 %); Philox4x32-10 at 32 random bits per site fills both (DESIGN.md Rooflines)",
                 "alu": {"achieved": rl["alu_achieved"], "peak": rl["alu_peak"], "unit": "G IMAD.WIDE/s", "frac": rl["alu_frac"],
                         "imad_wide_per_site_update": rl["muls_per_site"],
                         "peak_source": "derived (DESIGN.md Rooflines): %d SMs x 4 SMSP x 8 wide multiplies/clk x %.0f MHz"
