@@ -49,6 +49,49 @@ def test_slabs_of_one_lattice_match_the_unsplit_oracle(L, bounds):
             s.close()
 
 
+@pytest.mark.parametrize("k", range(16))
+def test_random_slab_splits_match_the_unsplit_oracle(k):
+    """Seeded random splits (1-5 slabs of at least two rows, any boundaries), sizes, starts, couplings, step counters and
+    record intervals; several steps per driver round where a single slab is its own neighbour."""
+    rng = np.random.default_rng(5100 + k)
+    L = int(rng.choice([32, 64, 144, 272, 400, 528, 1040]))
+    n_slabs = int(rng.integers(1, 6))
+    while True:
+        cuts = sorted(int(c) for c in rng.choice(np.arange(2, L - 1), size=n_slabs - 1, replace=False)) if n_slabs > 1 else []
+        bounds = [0] + cuts + [L]
+        if all(b - a >= 2 for a, b in zip(bounds[:-1], bounds[1:])):
+            break
+    seed, init = int(rng.integers(0, 2**62)), int(rng.choice([0, 0, 1, -1]))
+    J, q = float(rng.choice([0.0, 0.3, 0.6585, 0.9])), float(rng.choice([0.0, 0.4, 0.6585, 10.0]))
+    steps, obs = int(rng.integers(2, 9)), int(rng.choice([0, 1, 2, 3]))
+    t0 = int(rng.choice([0, 5, (1 << 32) - 2, (1 << 41) + 1]))
+    o = so.Oracle(L, 1, seed)
+    o.init(init)
+    o.step = t0
+    o.run(J, q, steps, obs)
+    slabs = open_ring(L, seed, bounds, steps + 1)
+    try:
+        for s in slabs:
+            s.init(init)
+            s.step = t0
+        for t in range(steps):
+            for s in slabs:
+                s.exchange()
+            for s in slabs:
+                s.run(J, q, 1, obs)
+        what = f"L={L} bounds={bounds} steps={steps} obs={obs} t0={t0}"
+        assert np.array_equal(np.vstack([s.get_spins(0) for s in slabs]), o.get_spins(0)[0]), "sigma differs " + what
+        assert np.array_equal(np.vstack([s.get_spins(1) for s in slabs]), o.get_spins(1)[0]), "tau differs " + what
+        want = o.observables()
+        if len(want):
+            assert np.array_equal(sum(s.observables() for s in slabs), want), "summed records differ " + what
+        else:
+            assert all(len(s.observables()) == 0 for s in slabs)
+    finally:
+        for s in slabs:
+            s.close()
+
+
 def test_single_slab_runs_many_steps_per_call_and_resumes():
     """One slab covering the whole lattice is its own neighbour: shaken_run(n) then needs no driver in between (each step
     publishes to itself), records every step, run split in two calls, set_spins in between."""
