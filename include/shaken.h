@@ -293,7 +293,8 @@ int shaken_selftest_philox_rate(int32_t blocks_per_sm, int32_t iters, int32_t re
  * shaken_test_band_hook: test hook for the one-launch band path (mid-size lattices).  what = 0: the
  * stamp counter of the hand-over buffer is set to `value` (a value near 2^32 exercises the wrap-around clearing);
  * what = 1: the next cooperative launch is treated as refused (value != 0), which exercises the fall-back to the
- * per-half-step kernels.  Results never depend on either.  SHAKEN_EINVAL for another selector.
+ * per-half-step kernels; what = 2: bands of at most seven rows are run by the two-phase band kernel instead of the
+ * data-flow one (value != 0) or by the default (0).  Results never depend on any of them.  SHAKEN_EINVAL for another selector.
  */
 int shaken_test_band_hook(shaken_ctx *ctx, int what, uint32_t value);
 

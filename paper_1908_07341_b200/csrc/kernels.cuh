@@ -6,6 +6,7 @@
 #include "kernel_pk.cuh"
 #include "kernel_small.cuh"
 #include "kernel_cluster.cuh"
+#include "kernel_flow.cuh"
 #include "kernel_band.cuh"
 #include "kernel_alt.cuh"
 #include "kernel_slab.cuh"

@@ -41,6 +41,7 @@ struct shaken_ctx {
     uint32_t xch_stamp = 0;       // last stamp written into d_xch
     int coop = -1;                // cooperative launch supported (-1: not queried yet)
     bool no_cluster = false;      // a cluster launch failed once: small chains stay on one SM each
+    bool no_flow = false;         // test hook: bands of <= 7 rows use the two-phase band kernel instead of the data-flow one
     bool band_refuse_next = false;   // test hook: treat the next cooperative launch as refused (exercises the fall-back)
     void *d_stage = nullptr;      // staging for packed <-> int8 conversion
     size_t stage_bytes = 0;
@@ -587,7 +588,9 @@ static int try_band_launch(shaken_ctx *ctx, bool alternate, const uint32_t *gtab
     bp.magicW = (uint32_t)(4294967296ull / (uint64_t)W) + 1u;
     bp.magicV = (uint32_t)(4294967296ull / (uint64_t)(W / 4)) + 1u;
     ctx->xch_stamp += (uint32_t)n_steps;                             // one stamp per full step
-    const void *kernel = alternate ? (const void *)alt_band_i8 : (const void *)band_run_i8;
+    // bands of at most 7 rows (cfg 2): the data-flow schedule (kernel_flow.cuh); taller bands: two phases per step
+    const bool flow = !alternate && !ctx->no_flow && flow_applies(ctx->L, rpb);
+    const void *kernel = alternate ? (const void *)alt_band_i8 : flow ? (const void *)band_flow_i8 : (const void *)band_run_i8;
     CU(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     void *args[] = {&bp};
     // the bands wait for one another, so they must all be resident: a cooperative launch either guarantees
@@ -1581,6 +1584,7 @@ extern "C" int shaken_test_band_hook(shaken_ctx *ctx, int what, uint32_t value)
     if (!ctx) return fail(nullptr, SHAKEN_EINVAL, "shaken_test_band_hook: ctx is NULL");
     if (what == 0) ctx->xch_stamp = value;              // next band launch starts its stamps here (wrap handling)
     else if (what == 1) ctx->band_refuse_next = value != 0;   // next cooperative launch counts as refused
+    else if (what == 2) ctx->no_flow = value != 0;            // bands of <= 7 rows: two-phase kernel instead of the data-flow one
     else return fail(ctx, SHAKEN_EINVAL, "shaken_test_band_hook: unknown selector %d", what);
     return SHAKEN_OK;
 }
