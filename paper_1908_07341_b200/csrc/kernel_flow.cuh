@@ -40,7 +40,7 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) band_flow_i8(const __grid_con
 {
     extern __shared__ __align__(16) uint32_t smem[];
     __shared__ uint2 s_pair[64][32];              // paired thresholds, lane-replicated (see kernel_i8.cuh)
-    __shared__ int s_acc[FLOW_RING][6];           // the band's partial sums of the records in flight
+    __shared__ int s_acc[FLOW_RING][3];           // the band's partial sums of the records in flight, two per word (see deliver)
     __shared__ int s_cnt[FLOW_RING][2];           // warps that have delivered their part: [0] sums of half-step 1, [1] C_x, C_y
     __shared__ long long s_red[BAND_THREADS / 32][2];
 
@@ -75,7 +75,7 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) band_flow_i8(const __grid_con
         }
         s_pair[e][t & 31] = make_uint2(T2[0], T2[1]);
     }
-    for (int t = tid; t < FLOW_RING * 6; t += BAND_THREADS) (&s_acc[0][0])[t] = 0;
+    for (int t = tid; t < FLOW_RING * 3; t += BAND_THREADS) (&s_acc[0][0])[t] = 0;
     for (int t = tid; t < FLOW_RING * 2; t += BAND_THREADS) (&s_cnt[0][0])[t] = 0;
     __syncthreads();
 
@@ -117,23 +117,29 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) band_flow_i8(const __grid_con
         }
         return make_uint4(o[0], o[1], o[2], o[3]);
     };
-    // a warp's part of `count` sums of record slot `slot` (fields first ..): warp sum -> shared-memory atomics; the last of the
-    // n_contrib warps to deliver adds the band's totals to the record (int64 atomics: the bands of a chain share it)
-    auto deliver = [&](const int (&v)[6], const int first, const int count, const int slot, const int which, long long *dst) {
-        for (int j = first; j < first + count; ++j) {
-            const int w = __reduce_add_sync(0xFFFFFFFFu, v[j]);
-            if (lane == 0 && w != 0) atomicAdd(&s_acc[slot][j], w);
-        }
-        __syncwarp();
+    // A warp's part of a record.  Two sums travel in one int, a * 65536 + b (a band has at most 7168 sites, so |a|, |b| <= 14336
+    // even for the band's totals): warp sum -> shared-memory atomic per packed word; the LAST of the n_contrib warps to deliver
+    // unpacks the band's totals and adds them to the record (int64 atomics: the bands of a chain share it).
+    // words [wfirst, wfirst + count) of the slot hold fields [2 wfirst, 2 wfirst + 2 count) of the record.
+    auto deliver = [&](const int x0, const int x1, const int count, const int wfirst, const int slot, const int which, long long *dst) {
+        const int w0 = __reduce_add_sync(0xFFFFFFFFu, x0);
+        const int w1 = count > 1 ? __reduce_add_sync(0xFFFFFFFFu, x1) : 0;
         if (lane == 0) {
+            if (w0 != 0) atomicAdd(&s_acc[slot][wfirst], w0);
+            if (count > 1 && w1 != 0) atomicAdd(&s_acc[slot][wfirst + 1], w1);
             __threadfence_block();
             if (atomicAdd(&s_cnt[slot][which], 1) == n_contrib - 1) {
                 __threadfence_block();
-                for (int j = first; j < first + count; ++j) {
-                    const int tot = atomicExch(&s_acc[slot][j], 0);
-                    atomicAdd(reinterpret_cast<unsigned long long *>(dst + j), (unsigned long long)(long long)tot);
+                volatile int *acc = &s_acc[slot][0];
+                int tot[2];
+                for (int k = 0; k < count; ++k) tot[k] = acc[wfirst + k];
+                for (int k = 0; k < count; ++k) {
+                    acc[wfirst + k] = 0;
+                    const int lo = (int)(short)(tot[k] & 0xFFFF), hi = (tot[k] - lo) >> 16;
+                    atomicAdd(reinterpret_cast<unsigned long long *>(dst + 2 * (wfirst + k)), (unsigned long long)(long long)hi);
+                    atomicAdd(reinterpret_cast<unsigned long long *>(dst + 2 * (wfirst + k) + 1), (unsigned long long)(long long)lo);
                 }
-                atomicExch(&s_cnt[slot][which], 0);
+                *reinterpret_cast<volatile int *>(&s_cnt[slot][which]) = 0;
             }
         }
     };
@@ -149,11 +155,11 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) band_flow_i8(const __grid_con
         const int cvs = mine ? cv : 0;            // (lanes beyond the row compute nothing but pass every barrier)
         uint32_t *self_s = sg + (gi + 1) * W, *down_s = sg + gi * W;     // sigma rows gi and gi-1
         uint32_t *self_t = ta + gi * W;                                  // tau row gi; row gi+1 is self_t + W
-#pragma unroll 1
-        for (long long s = 0; s < p.n_steps; ++s) {
+        // one full step of this group; two copies of the body: steps that touch a record (rec: this step is recorded; pending: the
+        // previous one was) carry the sums, the others do not pay for them (registers, schedule)
+        auto step = [&](auto with_sums, const long long s, const bool rec) {
+            constexpr bool SUMS = decltype(with_sums)::value;
             const unsigned long long t = p.t0 + (unsigned long long)s;
-            const bool rec = p.obs_every > 0 && --until_rec == 0;        // the same in every warp
-            if (rec) until_rec = p.obs_every;
             const uint32_t stamp_in = p.stamp0 + (uint32_t)s;
             const uint2 *in_below = p.xtop + ((size_t)((s + 1) & 1) * nb + below) * W;   // top row of the band below = row r0-1
             const uint2 *in_above = p.xbot + ((size_t)((s + 1) & 1) * nb + above) * W;   // bottom row of the band above = row r0+nr
@@ -190,7 +196,7 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) band_flow_i8(const __grid_con
                 }
                 const uint4 o = apply(0, s4, v4, e, R);
                 *reinterpret_cast<uint4 *>(self_t + 4 * cvs) = o;
-                if (__builtin_expect(pending != nullptr, 0) && gi < nr) {
+                if constexpr (SUMS) if (pending != nullptr && gi < nr) {
                     // C_x, C_y of the record taken after the previous step: sigma_x sigma_{x left}, sigma_x sigma_{x down}
                     const uint32_t w[4] = {s4.x, s4.y, s4.z, s4.w}, dw[4] = {v4.x, v4.y, v4.z, v4.w};
 #pragma unroll
@@ -201,8 +207,8 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) band_flow_i8(const __grid_con
                 }
             }
             if (gi >= 1) bar_arrive_n(X1 - 1, 2 * gt_threads);          // tau row gi exists: group gi-1 may start its half-step 1
-            if (pending) {
-                if (gi < nr) deliver(v, 4, 2, pending_slot, 1, pending);
+            if constexpr (SUMS) if (pending) {
+                if (gi < nr) deliver(v[4] * 65536 + v[5], 0, 1, 2, pending_slot, 1, pending);
                 pending = nullptr;
             }
 
@@ -226,7 +232,7 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) band_flow_i8(const __grid_con
                         uint2 *out_bot = p.xbot + ((size_t)(s & 1) * nb + band) * W;
                         st_pairs2(out_bot + 4 * cvs, o.x, o.y, stamp_out); st_pairs2(out_bot + 4 * cvs + 2, o.z, o.w, stamp_out);
                     }
-                    if (__builtin_expect(rec, 0)) {
+                    if constexpr (SUMS) if (rec) {
                         // M_sigma, M_tau, E_J = sigma'_x (tau_{x up} + tau_{x right}), E_q = sigma'_x tau_x
                         const uint32_t ow[4] = {o.x, o.y, o.z, o.w}, tw[4] = {s4.x, s4.y, s4.z, s4.w}, uw[4] = {v4.x, v4.y, v4.z, v4.w};
 #pragma unroll
@@ -241,14 +247,21 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) band_flow_i8(const __grid_con
                 }
                 if (s + 1 < p.n_steps) bar_arrive_n(X0 + 1, 2 * gt_threads);   // sigma row gi exists: group gi+1 may start the next step
             }
-            if (rec) {
+            if constexpr (SUMS) if (rec) {
                 long long *dst = p.rec + ((size_t)nrec * p.n_chains + chain) * 6;
                 const int slot = (int)(nrec & (FLOW_RING - 1));
-                if (gi < nr) deliver(v, 0, 4, slot, 0, dst);
+                if (gi < nr) deliver(v[0] * 65536 + v[1], v[2] * 65536 + v[3], 2, 0, slot, 0, dst);
                 pending = dst;
                 pending_slot = slot;
                 ++nrec;
             }
+        };
+#pragma unroll 1
+        for (long long s = 0; s < p.n_steps; ++s) {
+            const bool rec = p.obs_every > 0 && --until_rec == 0;        // the same in every warp
+            if (rec) until_rec = p.obs_every;
+            if (rec || pending) step(std::true_type{}, s, rec);
+            else step(std::false_type{}, s, false);
         }
     } else {
         // a warp without a row: only the bookkeeping that decides whether the last step was recorded

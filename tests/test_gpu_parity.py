@@ -398,10 +398,14 @@ def test_band_kernel_tall_bands_per_chain_tables_and_split_runs(L, n_chains):
 
 
 @pytest.mark.parametrize("L,n_chains,steps,obs", [(144, 1, 9, 1), (144, 5, 6, 2), (160, 148, 3, 1), (272, 2, 11, 3), (400, 3, 7, 0),
-                                                 (784, 1, 8, 1), (1040, 2, 5, 2), (1536, 1, 4, 1), (2048, 1, 3, 1), (304, 37, 4, 1)])
-def test_band_kernel_sweep_of_shapes_matches_oracle(L, n_chains, steps, obs):
+                                                 (528, 1, 9, 1), (784, 1, 8, 1), (1024, 1, 12, 1), (1040, 2, 5, 2), (1536, 1, 4, 1),
+                                                 (1552, 1, 3, 1), (2048, 1, 3, 1), (304, 37, 4, 1)])
+@pytest.mark.parametrize("two_phase", [0, 1])
+def test_band_kernel_sweep_of_shapes_matches_oracle(L, n_chains, steps, obs, two_phase):
     """The one-launch band path over the shapes it serves: 9 to 128 vectors per row, one-row bands (148 chains), bands of
-    28 rows, a ragged last band, several chains with their own couplings, every record cadence; each run split in two."""
+    28 rows, a ragged last band, several chains with their own couplings, every record cadence; each run split in two.
+    Bands of at most seven rows run the data-flow schedule (kernel_flow.cuh: one, two or three warps per row, a second
+    warp with a single active lane at L = 528 ...); two_phase = 1 forces the two-phase kernel for them as well."""
     if n_chains * L * L > 4.5e6:
         pytest.skip("beyond the band path")
     seed = 1000 + L + n_chains
@@ -411,6 +415,7 @@ def test_band_kernel_sweep_of_shapes_matches_oracle(L, n_chains, steps, obs):
     o.init(0)
     o.run_grid(J, q, steps, obs)
     with shaken.Shaken(L, n_chains, seed, max_records=steps) as s:
+        s.test_band_hook(2, two_phase)
         s.init(0)
         l0 = s.launch_count
         s.run_grid(J, q, steps // 2, obs)
