@@ -298,6 +298,37 @@ int shaken_selftest_philox_rate(int32_t blocks_per_sm, int32_t iters, int32_t re
  */
 int shaken_test_band_hook(shaken_ctx *ctx, int what, uint32_t value);
 
+/*
+ * shaken_run_static / shaken_static_setup: the shaken dynamics for callers that must not allocate (code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid cudaMalloc).  Same operation as shaken_run on an int8 context --
+ * n_steps full steps, half-step 0 tau <- sigma (eq. 15) then half-step 1 sigma <- tau (eq. 16,
+ * :169-172), thresholds of shaken_thresholds(J, q), random words of (seed, chain, step, half, site) -- in ONE cooperative
+ * launch of the band kernel (row bands resident in shared memory), whose only scratch memory, the
+ * hand-over rows between neighbouring bands, lives in a file-scope device array of SHAKEN_STATIC_SCRATCH_BYTES that
+ * every GPU which loads the library holds until exit.  There is no context: the caller owns every buffer.
+ *   sigma, tau   DEVICE [n_chains][L][L] int8 (+1 = 0x01, -1 = 0xFF), 16-byte aligned; sigma is read and both are
+ *                overwritten in place (tau need not be initialised: half-step 0 redraws all of it).
+ *   L, n_chains  128 < L <= 2048, L % 16 == 0, 1 <= n_chains <= number of SMs; the bands (ceil(L / floor(SMs / n_chains))
+ *                rows each) must fit 160 KiB of shared memory and their hand-over rows the static scratch array:
+ *                SHAKEN_EINVAL with a message naming the limit otherwise (e.g. 1 x 2048^2, 4 x 1024^2 fit).
+ *   seed, t0     Philox key and the 0-based global index of the first full step (chain c draws the words of chain c).
+ *   obs_every    0 = no records; else a record after every step whose 1-based global index is a multiple of it.
+ *   rec          DEVICE [max_records][n_chains][6] int64, may be NULL when no record falls into the run; the records of
+ *                this run are written from slot 0 (the call zeroes the slots it fills).  SHAKEN_ENOSPC if too small.
+ *   cuda_stream  a cudaStream_t (NULL = default stream); the call is asynchronous on it.
+ * The call issues two cudaMemsetAsync (scratch, records) and one kernel launch and calls no cudaMalloc, cudaFree or any
+ * allocating library routine; shaken_static_setup() (once per device, with that device current; shaken_run_static calls it
+ * when needed) looks up the scratch array's device address and the device's properties -- call it before a region that
+ * must not touch the module loader.  ALL calls on a device share the scratch array, which keeps the last call's contents:
+ * every call clears the part it uses first, and two calls that overlap on the GPU (different streams, concurrent graphs)
+ * race -- serialise them.  Errors: SHAKEN_EINVAL, SHAKEN_ENOSPC, SHAKEN_ECUDA (no device; cooperative launch refused:
+ * there is no fall-back here).
+ */
+#define SHAKEN_STATIC_SCRATCH_BYTES 2621440 /* 2.5 MiB = 2 parities x 2 sides x 160 bands x 512 words x 8 bytes */
+int shaken_static_setup(void);
+int shaken_run_static(void *sigma, void *tau, int32_t L, int32_t n_chains, uint64_t seed, uint64_t t0, double J, double q,
+                      int64_t n_steps, int64_t obs_every, int64_t *rec, int64_t max_records, void *cuda_stream);
+
 /* Number of kernels this context has launched so far (half-steps, init, conversions, reductions). */
 int64_t shaken_launch_count(const shaken_ctx *ctx);
 

@@ -13,6 +13,7 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -610,6 +611,126 @@ static int try_band_launch(shaken_ctx *ctx, bool alternate, const uint32_t *gtab
     if (le != cudaErrorCooperativeLaunchTooLarge && le != cudaErrorLaunchOutOfResources && le != cudaErrorNotSupported)
         return fail(ctx, SHAKEN_ECUDA, "band kernel launch: %s", cudaGetErrorString(le));
     return 1;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// shaken_run_static: the band path for callers that must not allocate.  The band kernels' only scratch memory -- the
+// hand-over rows xtop / xbot -- is a file-scope device array instead of a cudaMalloc'ed buffer.  In HOST code the array's
+// name is a host-side stand-in, not a device address: the address the kernels get comes from cudaGetSymbolAddress, looked
+// up once per device (with that device current) in shaken_static_setup.
+// ---------------------------------------------------------------------------------------------------
+constexpr size_t STATIC_XCH_PAIRS = (size_t)SHAKEN_STATIC_SCRATCH_BYTES / sizeof(uint2);
+static __device__ __align__(256) uint2 g_static_xch[STATIC_XCH_PAIRS];
+
+struct StaticDevice {
+    bool ready = false;
+    uint2 *xch = nullptr;       // device address of g_static_xch on this device
+    int num_sms = 0;
+    int coop = 0;
+};
+constexpr int STATIC_MAX_DEVICES = 64;
+static StaticDevice g_static_dev[STATIC_MAX_DEVICES];
+static std::mutex g_static_mutex;
+
+static int static_device(StaticDevice **out)
+{
+    shaken_ctx *ctx = nullptr;
+    int dev = -1;
+    CU(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= STATIC_MAX_DEVICES) return fail(nullptr, SHAKEN_EINVAL, "shaken_static_setup: device ordinal %d not supported", dev);
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    StaticDevice &d = g_static_dev[dev];
+    if (!d.ready) {
+        uint2 *ptr = nullptr;
+        CU(cudaGetSymbolAddress((void **)&ptr, g_static_xch));
+        if (!ptr) return fail(nullptr, SHAKEN_ECUDA, "shaken_static_setup: no device address for the scratch array");
+        CU(cudaDeviceGetAttribute(&d.num_sms, cudaDevAttrMultiProcessorCount, dev));
+        CU(cudaDeviceGetAttribute(&d.coop, cudaDevAttrCooperativeLaunch, dev));
+        d.xch = ptr;
+        d.ready = true;
+    }
+    *out = &d;
+    return SHAKEN_OK;
+}
+
+extern "C" int shaken_static_setup(void)
+{
+    StaticDevice *d = nullptr;
+    return static_device(&d);
+}
+
+extern "C" int shaken_run_static(void *sigma, void *tau, int32_t L, int32_t n_chains, uint64_t seed, uint64_t t0, double J, double q,
+                                 int64_t n_steps, int64_t obs_every, int64_t *rec, int64_t max_records, void *cuda_stream)
+{
+    shaken_ctx *ctx = nullptr;                                        // (errors go to the thread's message buffer)
+    if (!sigma || !tau || ((uintptr_t)sigma & 15) || ((uintptr_t)tau & 15))
+        return fail(nullptr, SHAKEN_EINVAL, "shaken_run_static: sigma and tau must be non-NULL, 16-byte aligned device pointers");
+    if (L <= SMALL_L_MAX || L > BAND_L_MAX || L % 16 != 0)
+        return fail(nullptr, SHAKEN_EINVAL, "shaken_run_static: L=%d must be a multiple of 16 in (%d, %d]", L, SMALL_L_MAX, BAND_L_MAX);
+    if (!isfinite(J) || !isfinite(q)) return fail(nullptr, SHAKEN_EINVAL, "shaken_run_static: non-finite coupling");
+    if (n_steps < 0 || obs_every < 0 || max_records < 0) return fail(nullptr, SHAKEN_EINVAL, "shaken_run_static: negative count");
+    if ((uint64_t)n_steps >= 0x7FFFFFF0ull) return fail(nullptr, SHAKEN_EINVAL, "shaken_run_static: n_steps too large for one call");
+    StaticDevice *d = nullptr;
+    int rc = static_device(&d);
+    if (rc) return rc;
+    if (n_chains < 1 || n_chains > d->num_sms)
+        return fail(nullptr, SHAKEN_EINVAL, "shaken_run_static: n_chains=%d must lie in [1, %d] (one band per SM at least)", n_chains, d->num_sms);
+    if (!d->coop) return fail(nullptr, SHAKEN_ECUDA, "shaken_run_static: the device has no cooperative launch");
+    // bands as in the context path (try_band_launch)
+    int bpc = d->num_sms / n_chains;
+    if (bpc > L) bpc = L;
+    const int rpb = (L + bpc - 1) / bpc;
+    bpc = (L + rpb - 1) / rpb;
+    const int W = L / 4;
+    const int n_bands = bpc * n_chains;
+    const size_t smem = band_smem_bytes(L, rpb);
+    if (smem > 160 * 1024)
+        return fail(nullptr, SHAKEN_EINVAL, "shaken_run_static: %d chains of %d^2 need bands of %d rows = %zu bytes of shared memory, beyond the maximum of %d",
+                    n_chains, L, rpb, smem, 160 * 1024);
+    const size_t xrow = (size_t)2 * n_bands * W;                      // uint2 elements per hand-over array (two parities)
+    const size_t need = 2 * xrow * sizeof(uint2);
+    if (need > (size_t)SHAKEN_STATIC_SCRATCH_BYTES)
+        return fail(nullptr, SHAKEN_EINVAL, "shaken_run_static: %d bands of %d-spin rows need %zu bytes of hand-over scratch, beyond the static maximum of %d",
+                    n_bands, L, need, SHAKEN_STATIC_SCRATCH_BYTES);
+    int64_t n_new = 0;
+    if (obs_every > 0) n_new = (int64_t)((t0 + (uint64_t)n_steps) / (uint64_t)obs_every - t0 / (uint64_t)obs_every);
+    if (n_new > 0 && !rec) return fail(nullptr, SHAKEN_EINVAL, "shaken_run_static: rec is NULL but the run takes %lld records", (long long)n_new);
+    if (n_new > max_records) return fail(nullptr, SHAKEN_ENOSPC, "shaken_run_static: the run takes %lld records, rec holds %lld", (long long)n_new, (long long)max_records);
+    if (n_steps == 0) return SHAKEN_OK;
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    // the array keeps the last call's contents: stamps must be new to it, so clear the part this call uses (stamp 0 = none)
+    CU(cudaMemsetAsync(d->xch, 0, need, stream));
+    if (n_new > 0) CU(cudaMemsetAsync(rec, 0, (size_t)n_new * n_chains * SHAKEN_N_OBS * sizeof(int64_t), stream));
+    BandParams bp;
+    memset(&bp, 0, sizeof(bp));
+    bp.sigma = (uint8_t *)sigma;
+    bp.tau = (uint8_t *)tau;
+    bp.L = L;
+    bp.n_chains = n_chains;
+    bp.chain0 = 0;
+    bp.t0 = t0;
+    bp.n_steps = n_steps;
+    bp.obs_every = obs_every;
+    bp.rec = n_new > 0 ? (long long *)rec : nullptr;
+    bp.gtab = nullptr;
+    kernel_table(J, q, bp.utab);
+    make_step_keys(seed, 0, bp.keys);
+    bp.bpc = bpc;
+    bp.rows_per_band = rpb;
+    bp.xtop = d->xch;                                                 // the DEVICE address from cudaGetSymbolAddress
+    bp.xbot = d->xch + xrow;
+    bp.stamp0 = 0;
+    bp.magicW = (uint32_t)(4294967296ull / (uint64_t)W) + 1u;
+    bp.magicV = (uint32_t)(4294967296ull / (uint64_t)(W / 4)) + 1u;
+    const void *kernel = flow_applies(L, rpb) ? (const void *)band_flow_i8 : (const void *)band_run_i8;
+    CU(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    void *args[] = {&bp};
+    const cudaError_t le = cudaLaunchCooperativeKernel(kernel, dim3(n_bands), dim3(BAND_THREADS), args, smem, stream);
+    if (le != cudaSuccess) {
+        cudaGetLastError();
+        return fail(nullptr, SHAKEN_ECUDA, "shaken_run_static: cooperative launch of %d bands: %s", n_bands, cudaGetErrorString(le));
+    }
+    return SHAKEN_OK;
 }
 
 // ---------------------------------------------------------------------------------------------------

@@ -64,6 +64,9 @@ SIGNATURES = {
     "shaken_slab_ipc_connect": (C.c_int, [_p, _p, _p]),
     "shaken_slab_exchange": (C.c_int, [_p]),
     "shaken_test_band_hook": (C.c_int, [_p, C.c_int, C.c_uint32]),
+    "shaken_static_setup": (C.c_int, []),
+    "shaken_run_static": (C.c_int, [_p, _p, C.c_int32, C.c_int32, C.c_uint64, C.c_uint64, C.c_double, C.c_double,
+                                    C.c_int64, C.c_int64, _p, C.c_int64, _p]),
     "shaken_moments": (C.c_int, [_p, C.c_int64, C.c_int64, C.c_int64, C.POINTER(C.c_double)]),
     "shaken_selftest_philox_rate": (C.c_int, [C.c_int32, C.c_int32, C.c_int32, C.POINTER(C.c_double)]),
     "shaken_last_error": (C.c_char_p, [_p]),
@@ -126,6 +129,26 @@ def philox_only_rate(blocks_per_sm: int = 8, iters: int = 2048, reps: int = 3) -
     if rc:
         raise ShakenError(rc, lib().shaken_last_error(None).decode())
     return float(v.value)
+
+
+STATIC_SCRATCH_BYTES = 2621440     # SHAKEN_STATIC_SCRATCH_BYTES of include/shaken.h
+
+
+def static_setup() -> None:
+    """shaken_static_setup: once per device, with that device current (looks up the static scratch array's address)."""
+    rc = lib().shaken_static_setup()
+    if rc:
+        raise ShakenError(rc, lib().shaken_last_error(None).decode())
+
+
+def run_static(sigma_ptr: int, tau_ptr: int, L: int, n_chains: int, seed: int, t0: int, J: float, q: float,
+               n_steps: int, obs_every: int = 0, rec_ptr: int = 0, max_records: int = 0, stream_ptr: int = 0) -> None:
+    """shaken_run_static: n_steps of the shaken dynamics on caller-owned DEVICE buffers (int8 sigma, tau; int64 records),
+    one cooperative launch, no allocation (the scratch is a static device array shared by all calls on the device)."""
+    rc = lib().shaken_run_static(int(sigma_ptr), int(tau_ptr), int(L), int(n_chains), int(seed), int(t0), float(J), float(q),
+                                 int(n_steps), int(obs_every), int(rec_ptr) or None, int(max_records), int(stream_ptr) or None)
+    if rc:
+        raise ShakenError(rc, lib().shaken_last_error(None).decode())
 
 
 def philox_words(ctr: np.ndarray, key: np.ndarray) -> np.ndarray:
