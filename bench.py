@@ -365,10 +365,20 @@ def run_ours(args):
         raise SystemExit("bench.py: no CUDA device; libshaken has no CPU fallback")
     if rank == 0:
         _build.build()
-    torch.cuda.set_device(local_rank)
-    dev = torch.device("cuda", local_rank)
+    # SHAKEN_BENCH_ONE_DEVICE=1 (tests on a one-GPU box): every rank uses device 0 and the control plane (barriers, the max
+    # over ranks) runs over gloo -- NCCL refuses two ranks on one device.  Replica arm only: slabs wait for each other.
+    one_dev = world > 1 and os.environ.get("SHAKEN_BENCH_ONE_DEVICE") == "1"
+    if one_dev and args.slabs:
+        raise SystemExit("bench.py: SHAKEN_BENCH_ONE_DEVICE is for the replica arm (the kernels of row slabs wait for each other)")
+    dev_index = 0 if one_dev else local_rank
+    torch.cuda.set_device(dev_index)
+    dev = torch.device("cuda", dev_index)
+    ctl = torch.device("cpu") if one_dev else dev           # where the tensors of the control-plane collectives live
     if world > 1:
-        dist.init_process_group("nccl", device_id=dev)
+        if one_dev:
+            dist.init_process_group("gloo")
+        else:
+            dist.init_process_group("nccl", device_id=dev)
         dist.barrier()
 
     w = workload(args.workload)
@@ -378,14 +388,14 @@ def run_ours(args):
     alt = args.dynamics == "alternate"
     uniform = len(set(w.J)) == 1 and len(set(w.q)) == 1
 
-    sampler = ClockSampler(local_rank)
+    sampler = ClockSampler(dev_index)
     slabs = bool(args.slabs)
     if slabs and (alt or w.packed or w.n_chains != 1):
         raise SystemExit("bench.py --slabs: needs a single-chain int8 workload of the shaken dynamics (cfg4, cfg2, paper<L>)")
     s, ms, launches, run = time_workload(shaken, torch, dist, w, K, W, dev, stream, rank, world, alt, args.variant,
                                          before_timed=sampler.start if rank == 0 else None, slabs=slabs)
     if world > 1:
-        t = torch.tensor([ms], device=dev, dtype=torch.float64)
+        t = torch.tensor([ms], device=ctl, dtype=torch.float64)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         ms = float(t.item())
     # nvidia-smi needs ~50 ms per sample: keep the same launch sequence running right after the timed region until at
@@ -433,7 +443,7 @@ def run_ours(args):
         torch.cuda.synchronize(dev)
         dt = time.perf_counter() - t0
         if world > 1:
-            t = torch.tensor([dt], device=dev, dtype=torch.float64)
+            t = torch.tensor([dt], device=ctl, dtype=torch.float64)
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
             dt = float(t.item())
         e2e = {"value": world * updates_per_rank / (dt * 1e9), "unit": UNIT,

@@ -167,6 +167,34 @@ def test_bench_two_ranks_under_torchrun(extra):
     assert line["scaling"] == ("strong" if extra else "weak")
 
 
+def test_bench_replica_arm_with_two_ranks_on_one_device():
+    """The N > 1 replica arm of bench.py (rank -> chain offset, barriers, max over ranks, rank 0 prints, the others exit 0)
+    under torchrun with two ranks that share cuda:0 (SHAKEN_BENCH_ONE_DEVICE=1: control plane over gloo, since NCCL refuses
+    two ranks on one device).  The replicas are independent -- no kernel of one rank waits for the other -- so this is safe
+    on one GPU; the value it prints is not a measurement.  The NCCL plumbing itself needs two devices (test above)."""
+    import json
+    import os
+    import socket
+    import subprocess
+    import sys
+
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.join(root, "bench.py"), "--gpus", "2", "--steps", "3", "--warmup", "3",
+           "--no-cpu-baseline", "--no-workloads", "--workload", "paper4096"]
+    env = dict(os.environ, SHAKEN_BENCH_ONE_DEVICE="1")
+    out = subprocess.run(cmd, capture_output=True, text=True, timeout=600, cwd=root, env=env)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [ln for ln in out.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1, "rank 0 alone prints the line"
+    line = json.loads(lines[0])
+    assert line["n_gpus"] == 2 and line["value"] > 0 and line["scaling"] == "weak"
+    assert line["e2e"]["value"] > 0 and line["gpu_launches"] >= 6
+
+
 def _ipc_worker(rank, world, L, seed, steps, J, q, barrier, handles, results):
     """One slab per PROCESS, both on cuda:0, inboxes connected through CUDA IPC handles.  Host barriers around every step
     make sure a rank's rows are published (and the stream drained) before the other rank's kernels look for them, so no
