@@ -14,7 +14,8 @@
 //   LOP3, no addition.  The byte is directly the BYTE OFFSET of the threshold in a 256-byte shared-memory table
 //   in which only the 8 reachable words are filled (8 distinct banks: the lookup never conflicts).
 //   The four z words go to a per-thread shared-memory slot and come back one byte at a time (LDS.U8): LSU slots
-//   instead of ALU slots (EXTRACT_SMEM).  Plain half-steps of block tasks use the paired lookup instead (EXTRACT_PAIR).
+//   instead of ALU slots (EXTRACT_SMEM: block tasks, launches with sums).  Plain half-steps of block tasks and all launches
+//   with per-warp task lists use the paired lookup instead (EXTRACT_PAIR).
 //   (Measured and dropped in round 1: PRMT extraction, IDP.4A extraction, 2 x 256-thread blocks per SM,
 //   one row of prefetch, XOR packing, observable sums on the tensor cores through int8 mma.sync.)
 #pragma once
@@ -38,10 +39,14 @@ __global__ void __launch_bounds__(I8_THREADS, 1) half_step_i8(const __grid_const
     // PER_WARP: a task is ONE warp strip and every warp walks its own task list with its own threshold table, so warps
     // of a block may work on different chains and never wait for each other (many small chains: the strips can be
     // tall and the last wave full at warp granularity).  Otherwise a task is WPB strips of one chain per block.
-    // Lookup: launches that also accumulate observables keep the multiplier pipe free of extra IDP.4A (index bytes go
-    // through shared memory); plain half-steps of block tasks use the paired lookup (one IDP.4A + one LDS.64 per two
-    // sites), which needs a 16 KiB table per block and so is not available to per-warp lists.
-    constexpr int EXTRACT = (PERWARP || (FLAGS & (F_OBS | F_BONDS)) != 0) ? EXTRACT_SMEM : EXTRACT_PAIR;
+    // Lookup, block tasks: launches that also accumulate observables keep the multiplier pipe free of extra IDP.4A (index
+    // bytes go through shared memory); plain half-steps use the paired lookup (one IDP.4A + one LDS.64 per two sites, a
+    // 16 KiB table per block).  Per-warp lists: always the paired lookup, with one 8 KiB table per warp (PWPAIR below) --
+    // a byte-indexed table per warp would cost one address add per lookup (the table base differs between the warps of a
+    // block and LDS takes one register), while the IDP.4A that forms the pair offset adds the base for free
+    // (cfg 3: 1204 -> 1228 with sums, 1291 -> 1355 without).
+    constexpr int EXTRACT = (!PERWARP && (FLAGS & (F_OBS | F_BONDS)) != 0) ? EXTRACT_SMEM : EXTRACT_PAIR;
+    constexpr bool PWPAIR = PERWARP && EXTRACT == EXTRACT_PAIR;   // per-warp paired tables in dynamic shared memory
     constexpr bool OBS = (FLAGS & F_OBS) != 0;
     constexpr bool BONDS = (FLAGS & F_BONDS) != 0;
     constexpr bool UPDATE = (FLAGS & F_NOUPDATE) == 0;
@@ -52,16 +57,21 @@ __global__ void __launch_bounds__(I8_THREADS, 1) half_step_i8(const __grid_const
     constexpr bool PRODUCT = (FLAGS & (F_OBS | F_BONDS)) != 0;
     static_assert(!(BONDS && HALF == 1), "bond sums ride on half-step 0");
 
-    __shared__ uint32_t s_tabs[PERWARP ? WPB : 1][64];
+    __shared__ uint32_t s_tab[64];                          // byte-indexed table (EXTRACT_SMEM: one per block)
     __shared__ uint32_t s_idx[EXTRACT == EXTRACT_SMEM ? 4 : 1][THREADS];
     // EXTRACT_PAIR: thresholds of TWO sites per lookup.  Entry e = c_even + 8 c_odd (c = m_self + 2 m_horizontal +
     // 4 m_vertical) holds {T(c_even), T(c_odd)}, replicated per lane: lane l reads 8 bytes at e * 256 + l * 8, i.e.
     // always banks 2l, 2l+1 -- conflict-free for any mix of indices.  16 KiB per block.
-    __shared__ uint2 s_pair[EXTRACT == EXTRACT_PAIR ? 64 : 1][32];
+    __shared__ uint2 s_pair[EXTRACT == EXTRACT_PAIR && !PWPAIR ? 64 : 1][32];
+    // PWPAIR: one paired table PER WARP, entry e replicated 16 times (a 64-bit shared load is served half a warp at a time, so
+    // lane l reading copy l & 15 of any entry is conflict-free): 64 x 16 x 8 B = 8 KiB per warp, 128 KiB per block.  The
+    // table's shared-memory address rides in the addend of the IDP.4A that forms the offset: no add per lookup.
+    extern __shared__ __align__(16) uint2 s_pw_pair[];
 
     const int lane = threadIdx.x & 31;
     const int warp = threadIdx.x >> 5;
-    uint32_t *const s_tab = s_tabs[PERWARP ? warp : 0];
+    uint2 *const my_pair = s_pw_pair + (PWPAIR ? warp * (64 * 16) : 0);
+    const uint32_t pw_base = PWPAIR ? (uint32_t)__cvta_generic_to_shared(my_pair) + (uint32_t)(lane & 15) * 8u : 0u;
     const int L = p.L;
     const int L4 = L >> 2;
     const int R = p.rows_per_task;
@@ -122,10 +132,17 @@ __global__ void __launch_bounds__(I8_THREADS, 1) half_step_i8(const __grid_const
             if (UPDATE) {
                 ck = make_chain_keys(p.keys, rng_chain(p, chain));
                 __syncwarp();
-                if (lane < 8) {
-                    const int ms = lane & 1, mh = (lane >> 1) & 1, mv = lane >> 2;
+                if (PWPAIR) {
+                    // lane l holds T(c = l & 7); entry e = c_even + 8 c_odd = {T(c_even), T(c_odd)}, 16 copies each
+                    const int ms = lane & 1, mh = (lane >> 1) & 1, mv = (lane >> 2) & 1;
                     const int idx = 2 * (2 - mh - mv) + (1 - ms);              // T[2k + c]
-                    s_tab[smem_code(ms, mh, mv) >> 2] = p.gtab ? p.gtab[(size_t)chain * 8 + idx] : p.utab[idx];
+                    const uint32_t Tl = p.gtab ? p.gtab[(size_t)chain * 8 + idx] : p.utab[idx];
+#pragma unroll 4
+                    for (int t = lane; t < 64 * 16; t += 32) {
+                        const int e = t >> 4;
+                        const uint32_t Te = __shfl_sync(0xFFFFFFFFu, Tl, e & 7), To = __shfl_sync(0xFFFFFFFFu, Tl, e >> 3);
+                        my_pair[t] = make_uint2(Te, To);
+                    }
                 }
                 __syncwarp();
             }
@@ -236,7 +253,12 @@ __global__ void __launch_bounds__(I8_THREADS, 1) half_step_i8(const __grid_const
                             philox_site_words(n + (uint32_t)j, p.keys, ck, rw);
                         }
                         uint32_t Tp[4];
-                        if (EXTRACT == EXTRACT_PAIR) {
+                        if (PWPAIR) {
+                            // (2 c_even) * 64 + (32 c_odd) * 32 = 128 e, plus the table's address and (lane & 15) * 8
+                            const uint32_t o01 = __dp4a(zw[j], 0x00002040u, pw_base), o23 = __dp4a(zw[j], 0x20400000u, pw_base);
+                            asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(Tp[0]), "=r"(Tp[1]) : "r"(o01));
+                            asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(Tp[2]), "=r"(Tp[3]) : "r"(o23));
+                        } else if (EXTRACT == EXTRACT_PAIR) {
                             // one IDP.4A per pair forms the whole byte offset: (2 c_even) * 128 + (32 c_odd) * 64 + lane * 8
                             const uint32_t o01 = __dp4a(zw[j], 0x00004080u, lane8), o23 = __dp4a(zw[j], 0x40800000u, lane8);
                             const uint2 t01 = *reinterpret_cast<const uint2 *>(reinterpret_cast<const char *>(s_pair) + o01);

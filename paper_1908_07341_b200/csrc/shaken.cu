@@ -42,6 +42,7 @@ struct shaken_ctx {
     uint32_t xch_stamp = 0;       // last stamp written into d_xch
     int coop = -1;                // cooperative launch supported (-1: not queried yet)
     bool no_cluster = false;      // a cluster launch failed once: small chains stay on one SM each
+    mutable uint32_t pw_attr_done = 0;   // per-warp strip kernels whose dynamic shared-memory limit has been raised (launch_half)
     bool no_flow = false;         // test hook: bands of <= 7 rows use the two-phase band kernel instead of the data-flow one
     bool band_refuse_next = false;   // test hook: treat the next cooperative launch as refused (exercises the fall-back)
     void *d_stage = nullptr;      // staging for packed <-> int8 conversion
@@ -466,12 +467,13 @@ extern "C" int shaken_init(shaken_ctx *ctx, int mode)
 // ---------------------------------------------------------------------------------------------------
 // launch with programmatic stream serialization (see kernels_common.cuh: wait_for_previous_kernel)
 template <typename K, typename P>
-static cudaError_t launch_pdl(K kernel, int grid, int threads, cudaStream_t stream, const P &p)
+static cudaError_t launch_pdl(K kernel, int grid, int threads, cudaStream_t stream, const P &p, size_t dyn_smem = 0)
 {
     cudaLaunchConfig_t cfg;
     memset(&cfg, 0, sizeof(cfg));
     cfg.gridDim = dim3((unsigned)grid);
     cfg.blockDim = dim3((unsigned)threads);
+    cfg.dynamicSmemBytes = dyn_smem;
     cfg.stream = stream;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
@@ -488,7 +490,18 @@ static cudaError_t launch_half(const shaken_ctx *ctx, const StepParams &p, int g
     // lists (kernel_i8.cuh); results are identical
     cudaError_t e;
     if (ctx->packed) e = launch_pdl(half_step_pk<HALF, FLAGS>, grid, PK_THREADS, ctx->stream, p);
-    else if (ctx->perwarp) e = launch_pdl(half_step_i8<HALF, FLAGS, true>, grid, I8_THREADS, ctx->stream, p);
+    else if (ctx->perwarp) {
+        // per-warp paired tables (kernel_i8.cuh PWPAIR): 16 warps x 64 entries x 16 copies x 8 B = 128 KiB of dynamic shared memory
+        constexpr size_t pw_smem = (FLAGS & F_NOUPDATE) ? 0 : (size_t)(I8_THREADS / 32) * 64 * 16 * sizeof(uint2);
+        constexpr uint32_t bit = 1u << (HALF * 16 + FLAGS);           // one bit per instantiation; a context lives on one device
+        static_assert(FLAGS < 16, "pw_attr_done holds 16 flag combinations per half-step");
+        if (pw_smem && !(ctx->pw_attr_done & bit)) {
+            e = cudaFuncSetAttribute(half_step_i8<HALF, FLAGS, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pw_smem);
+            if (e != cudaSuccess) return e;
+            ctx->pw_attr_done |= bit;
+        }
+        e = launch_pdl(half_step_i8<HALF, FLAGS, true>, grid, I8_THREADS, ctx->stream, p, pw_smem);
+    }
     else e = launch_pdl(half_step_i8<HALF, FLAGS, false>, grid, I8_THREADS, ctx->stream, p);
     return e != cudaSuccess ? e : cudaGetLastError();
 }
@@ -1014,7 +1027,7 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
     // many small chains: per-warp task lists (kernel_i8.cuh PERWARP).  Every warp gets a RANGE of the same number of
     // consecutive strip-rows (a strip-row = one row of one 32-vector column strip of one chain), so the launch is one full
     // wave whatever the chain size; a range is walked piece by piece, each piece paying the halo row and the two
-    // unprefetched rows of a strip start.  They cannot use the paired lookup, which is worth ~5 % on plain launches.
+    // unprefetched rows of a strip start.
     ctx->perwarp = false;
     if (!ctx->packed && (ctx->variant == SHAKEN_VARIANT_PERWARP || ctx->n_chains > 1)) {
         const long long S = (long long)ctx->n_chains * p.nseg * ctx->L;              // strip-rows per launch
@@ -1028,8 +1041,9 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
         const double fill = (double)S / (double)(waves_r * warps * len);
         const double pieces = 1.0 + (double)len / (double)ctx->L;                     // strip starts per range, on average
         const double score_pw = fill * (double)len / ((double)len + 3.0 * pieces);
+        // (launches with sums: block tasks keep their index bytes off the multiplier pipe, per-warp lists cannot: about 3 %)
         const bool mostly_plain = obs_every == 0 || obs_every > 4;
-        if (ctx->variant == SHAKEN_VARIANT_PERWARP || score_pw * (mostly_plain ? 0.95 : 1.0) > score_block + 0.02) {
+        if (ctx->variant == SHAKEN_VARIANT_PERWARP || score_pw * (mostly_plain ? 1.0 : 0.97) > score_block + 0.02) {
             ctx->perwarp = true;
             p.rows_total = S;
             p.range_len = (int)len;
