@@ -45,6 +45,7 @@ struct BandParams {
     uint2 *xbot;             // [2][n_bands][L/4] {word, stamp}: BOTTOM sigma row of each band after a full step
     uint32_t magicV;         // floor(2^32 / (L/16)) + 1: c / (L/16) == __umulhi(c, magicV) for the small c used here
     uint32_t magicW;         // floor(2^32 / (L/4)) + 1: the same for word indices c / W
+    unsigned long long slot_group;   // band_flow_i8: nibble s = the group (row) that warp slot s works for, 15 = none (flow_slot_groups)
     uint32_t stamp0;         // stamps of this launch are stamp0 + 1 .. stamp0 + n_steps (never seen before in xtop, xbot)
 };
 

@@ -36,6 +36,32 @@ __host__ __device__ inline bool flow_applies(int L, int rows_per_band)
     return rows_per_band <= FLOW_MAX_ROWS && wpr * (rows_per_band + 1) <= BAND_THREADS / 32;
 }
 
+// Which warps work for which group.  A slot = wpr consecutive warps; slot s sits on SM sub-partition(s) s % ncol (ncol = 4
+// sub-partitions for one warp per row, 2 pairs of them for two).  Group 0 is on the critical cycle between neighbouring bands
+// twice per step (it waits for the band below AND publishes the row that band waits for), the redundant last group has half
+// the work of the others: group 0 goes where the load is lightest (alone, or with the last group), the others are spread
+// evenly.  Measured at 1024^2: 1.98 us per step against 2.21 with groups simply in warp order (which puts group 0 on the
+// fully loaded sub-partitions), 768^2 1.84 against 2.09, 512^2 1.37 against 1.50; all 35 / 70 placements were timed.
+inline unsigned long long flow_slot_groups(int L, int rows_per_band)
+{
+    const int wpr = (L / 16 + 31) / 32, ncol = wpr == 1 ? 4 : 2, depth = (BAND_THREADS / 32) / wpr / ncol;
+    const int ng = rows_per_band + 1;
+    double load[4] = {0.0, 0.0, 0.0, 0.0};
+    int used[4] = {0, 0, 0, 0};
+    unsigned long long map = ~0ull;                                   // every nibble 15 = no group
+    for (int g = 0; g < ng; ++g) {
+        const double w = g == 0 ? 1.5 : (g == ng - 1 ? 0.5 : 1.0);    // group 0 counts as one and a half: it ends up lightest
+        int best = -1;
+        for (int c = 0; c < ncol; ++c)
+            if (used[c] < depth && (best < 0 || load[c] < load[best])) best = c;
+        const int slot = best + ncol * used[best];
+        map = (map & ~(15ull << (4 * slot))) | ((unsigned long long)g << (4 * slot));
+        load[best] += w;
+        used[best]++;
+    }
+    return map;
+}
+
 __global__ void __launch_bounds__(BAND_THREADS, 1) band_flow_i8(const __grid_constant__ BandParams p)
 {
     extern __shared__ __align__(16) uint32_t smem[];
@@ -80,8 +106,9 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) band_flow_i8(const __grid_con
     __syncthreads();
 
     const int wpr = (nvec + 31) >> 5;             // warps per row
-    const int gi = warp / wpr;                    // this warp's group = its row of the band (nr: the redundant row above)
-    const int cv = (warp - gi * wpr) * 32 + lane; // its vector of the row
+    const int slot = warp / wpr;                  // wpr consecutive warps form a slot; the host decides which group a slot serves
+    const int gi = (int)((p.slot_group >> (4 * slot)) & 15ull);   // this warp's group = its row of the band (nr: the redundant row above)
+    const int cv = (warp - slot * wpr) * 32 + lane; // its vector of the row
     const bool member = gi <= nr;                 // (warps beyond the last group only help with loading and storing)
     const bool mine = member && cv < nvec;
     const int gt_threads = wpr * 32;              // threads of one group

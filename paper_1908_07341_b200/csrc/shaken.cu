@@ -605,6 +605,7 @@ static int try_band_launch(shaken_ctx *ctx, bool alternate, const uint32_t *gtab
     // bands of at most 7 rows (cfg 2): the data-flow schedule (kernel_flow.cuh); taller bands: two phases per step
     const bool flow = !alternate && !ctx->no_flow && flow_applies(ctx->L, rpb);
     const void *kernel = alternate ? (const void *)alt_band_i8 : flow ? (const void *)band_flow_i8 : (const void *)band_run_i8;
+    if (flow) bp.slot_group = flow_slot_groups(ctx->L, rpb);
     CU(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     void *args[] = {&bp};
     // the bands wait for one another, so they must all be resident: a cooperative launch either guarantees
@@ -736,6 +737,7 @@ extern "C" int shaken_run_static(void *sigma, void *tau, int32_t L, int32_t n_ch
     bp.magicW = (uint32_t)(4294967296ull / (uint64_t)W) + 1u;
     bp.magicV = (uint32_t)(4294967296ull / (uint64_t)(W / 4)) + 1u;
     const void *kernel = flow_applies(L, rpb) ? (const void *)band_flow_i8 : (const void *)band_run_i8;
+    bp.slot_group = flow_slot_groups(L, rpb);
     CU(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     void *args[] = {&bp};
     const cudaError_t le = cudaLaunchCooperativeKernel(kernel, dim3(n_bands), dim3(BAND_THREADS), args, smem, stream);
