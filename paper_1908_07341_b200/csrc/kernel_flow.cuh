@@ -15,8 +15,8 @@
 // of the phases.  Write-after-read hazards are covered by the same edges: group i overwrites tau row i in half-step 0 of
 // step s+1 only after group i-1 arrived at X0_i, i.e. after its half-step 1 of step s, the last reader of that row;
 // group i overwrites sigma row i in half-step 1 only after group i+1 arrived at X1_i, i.e. after its half-step 0.
-// Records: per-warp partial sums go to a ring of shared-memory accumulators, and the LAST warp to deliver its part of a
-// record adds the band's totals to the record in global memory (no barrier either).
+// Records: per-warp partial sums go to a ring of shared-memory slots by atomics that count their contributors, and the LAST
+// warp to deliver its part of a sum adds the band's total to the record in global memory (no barrier, no fence: `deliver`).
 // Exchange protocol ({word, stamp} pairs), site -> random word mapping, thresholds and rule: exactly band_run_i8's.
 #pragma once
 #include "kernel_band.cuh"
@@ -24,6 +24,7 @@
 namespace shaken {
 
 constexpr int FLOW_MAX_ROWS = 7;           // rows per band: 2 * 7 + 1 named barriers (+ barrier 0)
+constexpr int FLOW_BIAS = 2048;            // makes a warp's part of a sum non-negative (|part| <= 1024)
 constexpr int FLOW_RING = 8;               // records in flight inside a band: groups drift at most nr + 1 half-steps apart
 
 __device__ __forceinline__ void bar_sync_n(int id, int n) { __syncwarp(); asm volatile("bar.sync %0, %1;" :: "r"(id), "r"(n) : "memory"); }
@@ -66,8 +67,7 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) band_flow_i8(const __grid_con
 {
     extern __shared__ __align__(16) uint32_t smem[];
     __shared__ uint2 s_pair[64][32];              // paired thresholds, lane-replicated (see kernel_i8.cuh)
-    __shared__ int s_acc[FLOW_RING][3];           // the band's partial sums of the records in flight, two per word (see deliver)
-    __shared__ int s_cnt[FLOW_RING][2];           // warps that have delivered their part: [0] sums of half-step 1, [1] C_x, C_y
+    __shared__ int s_acc[FLOW_RING][6];           // the band's partial sums of the records in flight, with their contributor counts (see deliver)
     __shared__ long long s_red[BAND_THREADS / 32][2];
 
     const int L = p.L, W = L >> 2, nvec = W >> 2;
@@ -101,8 +101,7 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) band_flow_i8(const __grid_con
         }
         s_pair[e][t & 31] = make_uint2(T2[0], T2[1]);
     }
-    for (int t = tid; t < FLOW_RING * 3; t += BAND_THREADS) (&s_acc[0][0])[t] = 0;
-    for (int t = tid; t < FLOW_RING * 2; t += BAND_THREADS) (&s_cnt[0][0])[t] = 0;
+    for (int t = tid; t < FLOW_RING * 6; t += BAND_THREADS) (&s_acc[0][0])[t] = 0;
     __syncthreads();
 
     const int wpr = (nvec + 31) >> 5;             // warps per row
@@ -144,29 +143,25 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) band_flow_i8(const __grid_con
         }
         return make_uint4(o[0], o[1], o[2], o[3]);
     };
-    // A warp's part of a record.  Two sums travel in one int, a * 65536 + b (a band has at most 7168 sites, so |a|, |b| <= 14336
-    // even for the band's totals): warp sum -> shared-memory atomic per packed word; the LAST of the n_contrib warps to deliver
-    // unpacks the band's totals and adds them to the record (int64 atomics: the bands of a chain share it).
-    // words [wfirst, wfirst + count) of the slot hold fields [2 wfirst, 2 wfirst + 2 count) of the record.
-    auto deliver = [&](const int x0, const int x1, const int count, const int wfirst, const int slot, const int which, long long *dst) {
+    // A warp's part of a record.  The lanes' partial sums travel two to an int through the warp reduction (a * 65536 + b; a warp
+    // holds 512 sites of a row, so |a|, |b| <= 1024).  Lane k then adds sum k to its word of the record's slot in shared
+    // memory with ONE atomic that also counts the contributors: word = count * 2^26 + sum of (v + FLOW_BIAS).  The warp whose
+    // atomic returns count == n_contrib - 1 is the last one for that word: old value + own part is the band's total, which it
+    // adds to the record in global memory (int64 atomics: the bands of a chain share it), and it clears the word.  Data and count
+    // in one atomic: no fence, no ordering between separate words to rely on.  Fields [first, first + 2 count) of the record.
+    auto deliver = [&](const int x0, const int x1, const int count, const int first, const int slot, long long *dst) {
         const int w0 = __reduce_add_sync(0xFFFFFFFFu, x0);
         const int w1 = count > 1 ? __reduce_add_sync(0xFFFFFFFFu, x1) : 0;
-        if (lane == 0) {
-            if (w0 != 0) atomicAdd(&s_acc[slot][wfirst], w0);
-            if (count > 1 && w1 != 0) atomicAdd(&s_acc[slot][wfirst + 1], w1);
-            __threadfence_block();
-            if (atomicAdd(&s_cnt[slot][which], 1) == n_contrib - 1) {
-                __threadfence_block();
-                volatile int *acc = &s_acc[slot][0];
-                int tot[2];
-                for (int k = 0; k < count; ++k) tot[k] = acc[wfirst + k];
-                for (int k = 0; k < count; ++k) {
-                    acc[wfirst + k] = 0;
-                    const int lo = (int)(short)(tot[k] & 0xFFFF), hi = (tot[k] - lo) >> 16;
-                    atomicAdd(reinterpret_cast<unsigned long long *>(dst + 2 * (wfirst + k)), (unsigned long long)(long long)hi);
-                    atomicAdd(reinterpret_cast<unsigned long long *>(dst + 2 * (wfirst + k) + 1), (unsigned long long)(long long)lo);
-                }
-                *reinterpret_cast<volatile int *>(&s_cnt[slot][which]) = 0;
+        if (lane < 2 * count) {                                       // lane k carries field first + k
+            const int wk = lane < 2 ? w0 : w1;
+            const int lo = (int)(short)(wk & 0xFFFF);
+            const int fk = (lane & 1) ? lo : (wk - lo) >> 16;
+            unsigned int *acc = reinterpret_cast<unsigned int *>(&s_acc[slot][first + lane]);
+            const unsigned int old = atomicAdd(acc, (1u << 26) + (unsigned int)(fk + FLOW_BIAS));
+            if ((old >> 26) == (unsigned int)(n_contrib - 1)) {
+                const int tot = (int)(old & 0x3FFFFFFu) + fk + FLOW_BIAS - n_contrib * FLOW_BIAS;
+                *reinterpret_cast<volatile unsigned int *>(acc) = 0u;               // (the slot is next used FLOW_RING records later)
+                atomicAdd(reinterpret_cast<unsigned long long *>(dst + first + lane), (unsigned long long)(long long)tot);
             }
         }
     };
@@ -235,7 +230,7 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) band_flow_i8(const __grid_con
             }
             if (gi >= 1) bar_arrive_n(X1 - 1, 2 * gt_threads);          // tau row gi exists: group gi-1 may start its half-step 1
             if constexpr (SUMS) if (pending) {
-                if (gi < nr) deliver(v[4] * 65536 + v[5], 0, 1, 2, pending_slot, 1, pending);
+                if (gi < nr) deliver(v[4] * 65536 + v[5], 0, 1, 4, pending_slot, pending);
                 pending = nullptr;
             }
 
@@ -277,7 +272,7 @@ __global__ void __launch_bounds__(BAND_THREADS, 1) band_flow_i8(const __grid_con
             if constexpr (SUMS) if (rec) {
                 long long *dst = p.rec + ((size_t)nrec * p.n_chains + chain) * 6;
                 const int slot = (int)(nrec & (FLOW_RING - 1));
-                if (gi < nr) deliver(v[0] * 65536 + v[1], v[2] * 65536 + v[3], 2, 0, slot, 0, dst);
+                if (gi < nr) deliver(v[0] * 65536 + v[1], v[2] * 65536 + v[3], 2, 0, slot, dst);
                 pending = dst;
                 pending_slot = slot;
                 ++nrec;
