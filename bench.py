@@ -23,7 +23,9 @@ configuration the metric is quoted on.
                 bounded band of rows of the same workload.
 
 N > 1 (torchrun): the workload is replicated as independent chains, rank r simulating global chain r of an
-N-chain batch (chains are independent units -- no data-path collective).
+N-chain batch (chains are independent units -- no data-path collective); ``--slabs`` shares ONE
+lattice between the ranks instead (row slabs, one sigma row each way per step by peer stores: strong scaling).
+SHAKEN_BENCH_ONE_DEVICE=1 (tests on a one-GPU box) lets all ranks of the replica arm use cuda:0, control plane over gloo.
 """
 from __future__ import annotations
 
