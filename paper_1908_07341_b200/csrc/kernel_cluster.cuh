@@ -8,7 +8,10 @@
 // the down row in half-step 0, the up row in half-step 1) is read straight out of that CTA's shared memory
 // (distributed shared memory); a cluster barrier separates the half-steps, and a thread draws the random words of the
 // next half-step between its arrival at that barrier and its wait.  The sums of a recorded step are fused into the
-// half-steps (operands in registers), reduced per warp and per CTA, and added to the record with int64 atomics.
+// half-steps (operands in registers), reduced per warp and collected per CTA in a shared-memory ring of CLUSTER_STAGE
+// records, which is added to the records in global memory (int64 atomics: the 8 CTAs share a record) once it is full and
+// at the end: a global atomic inside the step loop would make the next `barrier.cluster.arrive.release` wait for it
+// (measured: 1.49 us per recorded step with a flush per step, 1.21 without).
 // Site -> random word mapping, thresholds and rule are those of kernel_i8.cuh; only the schedule differs.
 #pragma once
 #include <cooperative_groups.h>
@@ -19,6 +22,7 @@
 namespace shaken {
 
 constexpr int CLUSTER_CTAS = 8;            // portable cluster size; L % 16 == 0 makes L / 8 an integer
+constexpr int CLUSTER_STAGE = 64;          // records a CTA collects in shared memory between two flushes to global memory
 
 // dynamic shared memory of cluster_run_i8: the CTA's rows of sigma and of tau
 __host__ __device__ inline size_t cluster_smem_bytes(int L) { return (size_t)2 * (L / CLUSTER_CTAS) * (L / 4) * sizeof(uint32_t); }
@@ -29,7 +33,7 @@ __global__ void __launch_bounds__(512, 1) cluster_run_i8(const __grid_constant__
     cg::cluster_group cluster = cg::this_cluster();
     extern __shared__ __align__(16) uint32_t smem[];
     __shared__ uint2 s_pair[64][32];              // paired thresholds, lane-replicated (see kernel_i8.cuh)
-    __shared__ int s_acc[6];                      // this CTA's partial sums of the record in progress
+    __shared__ int s_stage[CLUSTER_STAGE][6];     // this CTA's partial sums of the records not yet flushed (ring, by record index)
 
     const int L = p.L, W = L >> 2, rpb = L / CLUSTER_CTAS;
     const int rank = (int)cluster.block_rank();
@@ -59,11 +63,25 @@ __global__ void __launch_bounds__(512, 1) cluster_run_i8(const __grid_constant__
         }
         s_pair[e][t & 31] = make_uint2(T2[0], T2[1]);
     }
-    if (tid < 6) s_acc[tid] = 0;
+    for (int i = tid; i < CLUSTER_STAGE * 6; i += blockDim.x) (&s_stage[0][0])[i] = 0;
     cluster.sync();
 
-    long long nrec = 0;
-    long long *pending = nullptr;                 // record that still lacks C_x, C_y (taken in the next half-step 0)
+    long long nrec = 0, flushed = 0;              // records begun / added to global memory so far
+    bool pending = false;                         // the last record still lacks C_x, C_y (taken in the next half-step 0)
+    // records [flushed, upto) of the ring -> global memory; every thread of the CTA calls it at the same point
+    auto flush = [&](const long long upto) {
+        const int count = (int)(upto - flushed);
+        for (int i = tid; i < count * 6; i += blockDim.x) {
+            const long long r = flushed + i / 6;
+            const int f = i - (i / 6) * 6;
+            int *src = &s_stage[(int)(r % CLUSTER_STAGE)][f];
+            const int v = *reinterpret_cast<volatile int *>(src);
+            *reinterpret_cast<volatile int *>(src) = 0;
+            if (v != 0) atomicAdd(reinterpret_cast<unsigned long long *>(p.rec + ((size_t)r * p.n_chains + chain) * 6 + f), (unsigned long long)(long long)v);
+        }
+        flushed = upto;
+        __syncthreads();                          // the cleared slots are used again right away
+    };
     long long until_rec = p.obs_every > 0 ? p.obs_every - (long long)(p.t0 % (unsigned long long)p.obs_every) : 0;
     // A CTA has at most L^2 / 32 <= 512 words: one word per thread, no loop.  The random words of a half-step depend on no
     // spin, so a thread draws them BETWEEN its arrival at the cluster barrier and its wait: the Philox call (most of a
@@ -88,7 +106,7 @@ __global__ void __launch_bounds__(512, 1) cluster_run_i8(const __grid_constant__
         }
         const uint32_t *src = half ? ta : sg;
         uint32_t *dst = half ? sg : ta;
-        const bool sums1 = half == 1 && rec, sums0 = half == 0 && pending != nullptr;
+        const bool sums1 = half == 1 && rec, sums0 = half == 0 && pending;
         int a0 = 0, a1 = 0, a2 = 0, a3 = 0;
         if (active) {
             const uint32_t sw = src[tid];
@@ -129,8 +147,8 @@ __global__ void __launch_bounds__(512, 1) cluster_run_i8(const __grid_constant__
             a2 = __reduce_add_sync(0xFFFFFFFFu, a2);
             a3 = __reduce_add_sync(0xFFFFFFFFu, a3);
             if (lane == 0) {
-                if (sums1) { atomicAdd(&s_acc[0], a0); atomicAdd(&s_acc[1], a1); atomicAdd(&s_acc[2], a2); atomicAdd(&s_acc[3], a3); }
-                else { atomicAdd(&s_acc[4], a0); atomicAdd(&s_acc[5], a1); }
+                if (sums1) { int *d = s_stage[(int)(nrec % CLUSTER_STAGE)]; atomicAdd(d + 0, a0); atomicAdd(d + 1, a1); atomicAdd(d + 2, a2); atomicAdd(d + 3, a3); }
+                else { int *d = s_stage[(int)((nrec - 1) % CLUSTER_STAGE)]; atomicAdd(d + 4, a0); atomicAdd(d + 5, a1); }
             }
         }
         asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");   // my part of the new sublattice is written
@@ -142,13 +160,11 @@ __global__ void __launch_bounds__(512, 1) cluster_run_i8(const __grid_constant__
         }
         asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");     // ... and so is everybody else's
         if (sums0) {
-            if (tid >= 4 && tid < 6) { atomicAdd(reinterpret_cast<unsigned long long *>(pending + tid), (unsigned long long)(long long)s_acc[tid]); s_acc[tid] = 0; }
-            pending = nullptr;
+            pending = false;
+            if (nrec - flushed == CLUSTER_STAGE) flush(nrec);        // the ring is full of complete records
         }
         if (sums1) {
-            long long *dstrec = p.rec + ((size_t)nrec * p.n_chains + chain) * 6;
-            if (tid < 4) { atomicAdd(reinterpret_cast<unsigned long long *>(dstrec + tid), (unsigned long long)(long long)s_acc[tid]); s_acc[tid] = 0; }
-            pending = dstrec;
+            pending = true;
             ++nrec;
         }
     }
@@ -163,10 +179,10 @@ __global__ void __launch_bounds__(512, 1) cluster_run_i8(const __grid_constant__
         }
         a0 = __reduce_add_sync(0xFFFFFFFFu, a0);
         a1 = __reduce_add_sync(0xFFFFFFFFu, a1);
-        if (lane == 0) { atomicAdd(&s_acc[4], a0); atomicAdd(&s_acc[5], a1); }
+        if (lane == 0) { int *d = s_stage[(int)((nrec - 1) % CLUSTER_STAGE)]; atomicAdd(d + 4, a0); atomicAdd(d + 5, a1); }
         __syncthreads();
-        if (tid >= 4 && tid < 6) atomicAdd(reinterpret_cast<unsigned long long *>(pending + tid), (unsigned long long)(long long)s_acc[tid]);
     }
+    flush(nrec);
     for (int i = tid; i < nwords; i += blockDim.x) { gs[i] = sg[i]; gt[i] = ta[i]; }
     cluster.sync();                               // nobody leaves while a neighbour may still read its shared memory
 }

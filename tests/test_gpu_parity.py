@@ -339,6 +339,23 @@ def test_cluster_path_for_few_small_chains_and_one_sm_path_for_many(L, n_chains)
             assert_same_state(s, o, f"L={L} chains={n_chains} obs={obs}")
 
 
+@pytest.mark.parametrize("calls,obs", [((64,), 1), ((65,), 1), ((63, 1, 1), 1), ((128, 1), 1), ((129,), 1), ((130, 61), 3), ((127, 2, 70), 2),
+                                       ((200,), 1)])
+def test_cluster_kernel_record_ring_boundaries(calls, obs):
+    """The cluster kernel collects a CTA's partial sums in a shared-memory ring of 64 records and adds it to the records in
+    global memory when it is full and at the end of a launch: runs whose record counts end just before, on and just after a
+    multiple of 64, with and without a record on the very last step of a call, against the oracle."""
+    L, n_chains, seed, J, q = 64, 2, 77, 0.5, 0.6
+    o = so.Oracle(L, n_chains, seed)
+    o.init(0)
+    with shaken.Shaken(L, n_chains, seed, max_records=sum(calls) // obs + 2) as s:
+        s.init(0)
+        for n in calls:
+            o.run(J, q, n, obs)
+            s.run(J, q, n, obs)
+            assert_same_state(s, o, f"calls={calls} obs={obs} after {n}")
+
+
 @pytest.mark.parametrize("variant", [0, 3, 8])
 def test_every_int8_code_path_matches_oracle_on_a_ragged_lattice(variant):
     """L = 272: 17 vectors per row (ragged warp strip), several row blocks per chain, three chains with different
