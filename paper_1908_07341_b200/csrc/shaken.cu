@@ -1076,7 +1076,7 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
                             small_smem_bytes(ctx->L, ctx->group) <= 200 * 1024 &&
                             (ctx->L <= SMALL_L_MAX || (ctx->L <= SMALL_L_BATCH_MAX && 2 * (ctx->n_chains / ctx->group) >= ctx->num_sms));
     // A few small chains: one chain per CLUSTER of 8 SMs (kernel_cluster.cuh) instead of one per SM -- rows in the shared
-    // memory of 8 CTAs, the neighbour's row read through distributed shared memory, a cluster barrier per half-step.
+    // memory of 8 CTAs, the neighbours' rows read through distributed shared memory, one cluster barrier per full step.
     const bool cluster_path = small_path && ctx->group == 1 && ctx->L >= 32 && ctx->L <= SMALL_L_MAX && !ctx->no_cluster &&
                               (long long)ctx->n_chains * CLUSTER_CTAS <= ctx->num_sms;
     if (cluster_path) {
@@ -1095,8 +1095,7 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
         sp.gtab = p.gtab;
         memcpy(sp.utab, p.utab, sizeof(sp.utab));
         make_step_keys(ctx->seed, 0, sp.keys);
-        const int nwords = (ctx->L / CLUSTER_CTAS) * (ctx->L / 4);
-        const int threads = nwords >= 512 ? 512 : ((nwords + 31) / 32) * 32;
+        const int threads = cluster_threads(ctx->L);
         cudaLaunchConfig_t cfg;
         memset(&cfg, 0, sizeof(cfg));
         cfg.gridDim = dim3((unsigned)(ctx->n_chains * CLUSTER_CTAS));
