@@ -1077,8 +1077,12 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
                             (ctx->L <= SMALL_L_MAX || (ctx->L <= SMALL_L_BATCH_MAX && 2 * (ctx->n_chains / ctx->group) >= ctx->num_sms));
     // A few small chains: one chain per CLUSTER of 8 SMs (kernel_cluster.cuh) instead of one per SM -- rows in the shared
     // memory of 8 CTAs, the neighbours' rows read through distributed shared memory, one cluster barrier per full step.
+    // Which of the two is faster was measured at L = 32, 64, 128 for 19 ... 1024 chains: the cluster kernel (one word per thread:
+    // short latency, less instruction-level parallelism) wins while the machine is not full -- up to about 110 / 95 / 58 chains
+    // with records on every step, 80 / 74 / 30 without -- e.g. 37 chains of 64^2: 1.17 against 2.10 us per step.
+    const int cluster_max_chains = max(ctx->num_sms / CLUSTER_CTAS, (obs_every == 1 || obs_every == 2 ? 128 : 100) - (9 * ctx->L) / 16);
     const bool cluster_path = small_path && ctx->group == 1 && ctx->L >= 32 && ctx->L <= SMALL_L_MAX && !ctx->no_cluster &&
-                              (long long)ctx->n_chains * CLUSTER_CTAS <= ctx->num_sms;
+                              ctx->n_chains <= cluster_max_chains;
     if (cluster_path) {
         SmallParams sp;
         memset(&sp, 0, sizeof(sp));

@@ -316,11 +316,13 @@ def test_small_lattice_path_and_generic_kernels_both_match_oracle(L, n_chains):
             assert_same_state(s, o, f"L={L} variant={variant}")
 
 
-@pytest.mark.parametrize("L,n_chains", [(32, 1), (64, 1), (80, 3), (128, 1), (128, 18), (64, 19)])
+@pytest.mark.parametrize("L,n_chains", [(32, 1), (64, 1), (80, 3), (128, 1), (128, 18), (64, 19), (32, 82), (32, 83), (64, 64), (64, 65),
+                                        (128, 28), (128, 29), (128, 56), (128, 57), (64, 92), (64, 93), (112, 40), (48, 150)])
 def test_cluster_path_for_few_small_chains_and_one_sm_path_for_many(L, n_chains):
-    """Up to 18 small chains (L >= 32) run one chain per CLUSTER of 8 SMs (kernel_cluster.cuh: rows in the shared memory of 8
-    CTAs, neighbour rows through distributed shared memory, fused sums); from 19 chains on one chain per SM
-    (kernel_small.cuh).  Per-chain couplings, records on some steps only and on every step, split runs, a record on the very
+    """Small chains (32 <= L <= 128) run one chain per CLUSTER of 8 SMs while the machine is not full (kernel_cluster.cuh: rows in
+    the shared memory of 8 CTAs, neighbour rows through distributed shared memory, fused sums; up to max(18, 100 - 9 L / 16)
+    chains, 28 more when records are taken on every or every other step: 82 / 110 at L = 32, 64 / 92 at 64, 28 / 56 at 128), larger batches one chain per SM (kernel_small.cuh): both sides of the
+    switch.  Per-chain couplings, records on some steps only and on every step, split runs, a record on the very
     last step of a call (its C_x, C_y are closed from the final sigma)."""
     seed = 300 + L + n_chains
     J = np.linspace(0.3, 0.8, n_chains)
