@@ -1142,8 +1142,20 @@ static int run_impl(shaken_ctx *ctx, const double *J, const double *q, bool unif
         memcpy(sp.utab, p.utab, sizeof(sp.utab));
         make_step_keys(ctx->seed, 0, sp.keys);
         const int nvecs = ctx->L * ctx->L / 16;             // one 16-byte vector per thread per trip
-        const int threads = nvecs <= 256 ? ((nvecs + 31) / 32) * 32 : 512;
         const size_t smem = small_smem_bytes(ctx->L, ctx->group);
+        // Block size.  Up to 256 vectors: one per thread.  Beyond: 512 threads, unless two CTAs fit an SM (shared memory) and
+        // there are more CTAs than SMs -- then blocks of at most 256 threads, so that two or three resident CTAs hide each
+        // other's block barriers (1024 chains of 128^2: 773 -> 840 site-updates/ns, 1600 of 208^2: 863 -> 922), a little
+        // smaller where that fills the last trip much better (576 vectors at L = 96: 3 x 192 instead of 2 x 512: 553 -> 681).
+        int threads = nvecs <= 256 ? ((nvecs + 31) / 32) * 32 : 512;
+        if (nvecs > 256 && 2 * (smem + 2048) <= 220 * 1024 && ctx->n_chains / ctx->group > ctx->num_sms) {
+            threads = 256;
+            double best = (double)nvecs / (double)(((nvecs + 255) / 256) * 256);
+            for (int t = 224; t >= 192; t -= 32) {
+                const double eff = (double)nvecs / (double)(((nvecs + t - 1) / t) * t);
+                if (eff > best * 1.05) { best = eff; threads = t; }
+            }
+        }
         if (threads <= 256) {
             if (smem > 40 * 1024) CU(cudaFuncSetAttribute(small_run_i8<256>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
             small_run_i8<256><<<ctx->n_chains / ctx->group, threads, smem, ctx->stream>>>(sp);

@@ -341,6 +341,23 @@ def test_cluster_path_for_few_small_chains_and_one_sm_path_for_many(L, n_chains)
             assert_same_state(s, o, f"L={L} chains={n_chains} obs={obs}")
 
 
+@pytest.mark.parametrize("L,n_chains", [(80, 160), (96, 150), (112, 150), (128, 149), (160, 150), (208, 150), (224, 150)])
+def test_one_sm_kernel_block_sizes_for_batches_larger_than_the_machine(L, n_chains):
+    """kernel_small.cuh with more chains than SMs: the host picks blocks of 192, 224 or 256 threads (two or three resident CTAs
+    per SM, last trip well filled) where two CTAs fit an SM, 512 otherwise; several trips per thread, ragged last trips."""
+    J = np.linspace(0.3, 0.8, n_chains)
+    q = np.linspace(1.0, 0.2, n_chains)
+    o = so.Oracle(L, n_chains, 5)
+    o.init(0)
+    o.run_grid(J, q, 3, 1)
+    with shaken.Shaken(L, n_chains, 5, max_records=4) as s:
+        s.init(0)
+        s.run_grid(J, q, 2, 1)
+        s.run_grid(J, q, 1, 1)
+        assert s.launch_count == 3, "init + one launch per run call expected"
+        assert_same_state(s, o, f"L={L} chains={n_chains}")
+
+
 @pytest.mark.parametrize("calls,obs", [((64,), 1), ((65,), 1), ((63, 1, 1), 1), ((128, 1), 1), ((129,), 1), ((130, 61), 3), ((127, 2, 70), 2),
                                        ((200,), 1)])
 def test_cluster_kernel_record_ring_boundaries(calls, obs):
